@@ -1,0 +1,114 @@
+/*
+ * cpm.h -- C ABI of the B200-native checkerboard Cellular Potts sweep (arXiv 2312.09317).
+ *
+ * The library implements ONE thing: the data-parallel hot path of the paper's parallel CPM --
+ * the checkerboard-partitioned Metropolis copy-attempt sweep over a 2D/3D lattice of cell ids
+ * ("Designing a parallel execution scheme", Methods L218-264 Eq 1-3, 8-9, and
+ * "GPU implementation details" L270-284).  All compute runs in hand-written CUDA kernels for
+ * sm_100a; there is no CPU fallback: every entry point that needs the device fails with
+ * CPM_ERR_CUDA when no usable GPU is present.
+ *
+ * Conventions
+ *   - every call returns CPM_OK (0) or a negative CPM_ERR_* code; nothing throws or aborts;
+ *     cpm_last_error() returns a message for the last failing call on that context.
+ *   - the CALLER owns every buffer it passes.  "set" calls copy from it, "get" calls fill it.
+ *     `on_device` says whether the pointer is a device pointer (1; must be on the context's
+ *     device) or a host pointer (0).  NULL output pointers are skipped.
+ *   - lattice arrays are dense, x fastest: index = x + dims[0]*(y + dims[1]*z); N = prod(dims).
+ *     per-cell arrays have max_cells+1 entries (entry 0 = medium, always reported as 0).
+ *   - the context owns all device state until cpm_destroy.  One context is not thread-safe.
+ *   - cpm_step is asynchronous on the context's stream; getters synchronise that stream.
+ */
+#ifndef CPM_H
+#define CPM_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cpm_ctx cpm_ctx; /* opaque; owned by the library */
+
+enum { CPM_OK = 0, CPM_ERR_ARG = -1, CPM_ERR_DIMS = -2, CPM_ERR_UNSUPPORTED = -3,
+       CPM_ERR_CUDA = -4, CPM_ERR_OOM = -5, CPM_ERR_STATE = -6 };
+enum { CPM_MOORE = 0 }; /* the only neighbourhood the paper uses (L225): 8 / 26 neighbours */
+enum {
+  CPM_MODE_DETERMINISTIC = 0, /* per-cell state read from a phase-start snapshot + the worker's own
+                                 deltas; integer atomic deltas applied after (bit-exact, schedule-free) */
+  CPM_MODE_LIVE_ATOMICS = 1   /* paper-faithful: live reads (possibly stale, L53), immediate atomics (L51) */
+};
+
+/* Problem statement (L220-234, Tables 1-3): lattice geometry, J between cell TYPES,
+ * lambda / target per type, temperature, RNG seed, and the checkerboard schedule knobs (L77). */
+typedef struct {
+  int32_t  ndim;                  /* 2 or 3 */
+  int32_t  dims[3];               /* x fastest; dims[2] ignored (1) when ndim == 2 */
+  int32_t  neighbourhood;         /* CPM_MOORE */
+  int32_t  periodic[3];           /* 0 = closed: the lattice is embedded in immutable medium */
+  int32_t  n_types;               /* 1..127; type 0 = medium */
+  const int32_t *J;               /* host, n_types*n_types, symmetric, |J| <= 2^24 (Eq 1) */
+  const int32_t *lambda_V, *target_V;   /* host [n_types] or NULL (= 0): volume constraint, Eq 1 */
+  const int32_t *lambda_P, *target_P;   /* perimeter constraint, Eq 3 */
+  const int32_t *lambda_act, *max_act;  /* Act model, Eq 8-9; max_act in [0,255] */
+  double   T;                     /* >= 0; 0 = no uphill move, +inf = accept every evaluated move (Eq 2) */
+  uint64_t seed;                  /* Philox4x32-10 key */
+  int32_t  subsection;            /* S, checkerboard subsection edge; 0 = scheduler's choice */
+  int32_t  attempts_per_activation; /* k; 0 = S^d (one activation per subsection per MCS) */
+  int32_t  mode;                  /* CPM_MODE_* */
+  uint32_t max_cells;             /* cell ids are 0..max_cells; < 2^24 */
+  int32_t  device;                /* CUDA device ordinal */
+  void    *stream;                /* cudaStream_t (e.g. torch's current stream); NULL = default stream */
+} cpm_params;
+
+/* Validate parameters, build the type tables, the Metropolis threshold table (Eq 2) and the
+ * Act log/exp tables on the host, allocate device state, choose S, k and the phase list
+ * (checkerboard scheduler, L49/L77).  Errors: CPM_ERR_ARG (bad value, non-symmetric J, T < 0),
+ * CPM_ERR_DIMS (dims not a multiple of S, odd subsection count on a periodic axis),
+ * CPM_ERR_UNSUPPORTED (max_cells >= 2^24, S too large for shared memory), CPM_ERR_CUDA,
+ * CPM_ERR_OOM. */
+int  cpm_create(const cpm_params *params, cpm_ctx **out);
+int  cpm_destroy(cpm_ctx *ctx);
+
+/* Load the state of the model: ids[N] cell id per site (0 = medium), frozen[N] (NULL = none;
+ * non-zero = obstacle voxel that is never copied from or into, L139 stroma), cell_type
+ * [max_cells+1] (type of each cell id; cell_type[0] must be 0).  Resets the Act field to 0 and
+ * recounts volume, perimeter (Eq 3's A) and coordinate sums (L288) on the device.
+ * Errors: CPM_ERR_ARG (NULL ids/cell_type, an id > max_cells or a type >= n_types). */
+int  cpm_set_lattice(cpm_ctx *ctx, const uint32_t *ids, const uint8_t *frozen,
+                     const uint8_t *cell_type, int on_device);
+/* Optional: set the per-site Act field (integers 0..255 stored as float, L255). */
+int  cpm_set_act(cpm_ctx *ctx, const float *act, int on_device);
+/* Set the MCS counter (checkpoint/resume: the RNG is keyed by (seed, MCS, phase, subsection, attempt)). */
+int  cpm_set_mcs(cpm_ctx *ctx, uint32_t mcs);
+
+/* Run n_mcs Monte Carlo steps (one MCS = N copy attempts, L65): for each repetition and each
+ * of the 2^d checkerboard colours, all subsections of that colour run k sequential copy
+ * attempts concurrently (L49); then the Act field decays by 1 (L255).  Asynchronous. */
+int  cpm_step(cpm_ctx *ctx, uint32_t n_mcs);
+
+int  cpm_get_lattice(cpm_ctx *ctx, uint32_t *ids, int on_device);
+int  cpm_get_act(cpm_ctx *ctx, float *act, int on_device);
+/* Per-cell globals kept by integer atomics (L51, L57, L288): volume, perimeter, coordinate sums. */
+int  cpm_get_cell_stats(cpm_ctx *ctx, uint32_t *volume, uint32_t *perimeter,
+                        uint64_t *sum_x, uint64_t *sum_y, uint64_t *sum_z, int on_device);
+/* out (host) = {attempts, evaluated, accepted, mcs}. */
+int  cpm_get_counters(cpm_ctx *ctx, uint64_t out[4]);
+int  cpm_get_schedule(cpm_ctx *ctx, int32_t *S, int32_t *k, int32_t *phase_steps_per_mcs);
+/* Introspection for tests: host copy of the Metropolis table, thr[h] = floor(exp(-h/T) 2^32),
+ * h = 1..Hmax; returns Hmax (>= 0) or a negative error; fills at most cap entries (thr[0] unused). */
+int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);
+/* Introspection: kernels launched by this context so far, and the launch geometry of the sweep
+ * kernel: out = {launches, sweep_launches, warps_per_cta, smem_bytes_per_cta, uses_tma}. */
+int  cpm_get_launch_info(cpm_ctx *ctx, uint64_t out[5]);
+/* Average device time (ms) of the sweep kernel launches since the last call with reset != 0,
+ * measured with CUDA events on the context's stream when timing is enabled. */
+int  cpm_set_kernel_timing(cpm_ctx *ctx, int enabled);
+int  cpm_get_kernel_timing(cpm_ctx *ctx, double *sweep_ms_total, uint64_t *sweep_launches, int reset);
+const char *cpm_last_error(const cpm_ctx *ctx);
+/* Device-side Philox4x32-10 of n (ctr[4], key[2]) pairs (host arrays) -> out[4n]; test hook that
+ * runs the same device function the sweep uses. */
+int  cpm_debug_philox(int device, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

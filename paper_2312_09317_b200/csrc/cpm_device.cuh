@@ -1,0 +1,690 @@
+// cpm_device.cuh -- sm_100a device code of the checkerboard CPM sweep.
+//
+// One WARP owns one active checkerboard subsection for one activation:
+//   a2  id tile + halo staged into shared memory by TMA (cp.async.bulk.tensor, OOB zero-fill =
+//       "outside is medium"), completion on a per-warp mbarrier.  TMA needs the innermost start
+//       coordinate at a 16-byte boundary (measured on B200: a 4-byte-aligned start raises
+//       "illegal instruction"), so the tile starts at x0-4 words; the 1-byte Act tile is staged
+//       with plain 32-bit loads while the TMA is in flight;
+//   a3  Philox4x32-10: every lane draws one 128-bit block = 4 proposals -> 128 proposals / batch;
+//   a4  all 128 proposals are screened in parallel against the tile (same cell / frozen);
+//   a5-a9 the surviving ("interesting") proposals are processed strictly in attempt order, one at
+//       a time, with lanes = Moore neighbours: ballot/popc for n_A, n_B, REDUX for the adhesion sum;
+//       after an accepted copy the not-yet-processed proposals are re-screened, so the result is
+//       exactly that of k sequential attempts;
+//   a10 tile written back with 128-bit stores, integer deltas flushed with 64-bit atomics.
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cpm {
+
+constexpr uint32_t ID_MASK = 0x00FFFFFFu;   // lattice word = [frozen:1 | type:7 | id:24]
+constexpr uint32_t FULL = 0xFFFFFFFFu;
+constexpr int COUNTER_SLOTS = 256;
+
+struct __align__(16) TypeParams {  // per cell type, Tables 1-3 of the paper
+  int32_t lamV, tgtV, lamP, tgtP;
+  int32_t lamA, maxA, pad0, pad1;
+};
+
+struct SweepParams {
+  uint32_t *lat;            // pitched lattice words
+  uint8_t *act;             // pitched Act bytes (may be null)
+  long long pitch;          // words per lattice row
+  long long apitch;         // bytes per Act row
+  int X, Y, Z;
+  int per[3];
+  int S, log2S, sites, k;   // subsection edge, log2 (or -1), S^d, attempts per activation
+  int nsub[3];              // subsections per axis
+  int nact[3];              // active subsections per axis for this colour
+  int col[3];               // colour bits of this phase-step
+  unsigned long long n_active;
+  uint32_t p;               // phase-step index rep*2^d + colour
+  const uint32_t *mcs_ptr;  // device MCS counter
+  uint32_t key0, key1;      // Philox key = seed
+  int h;                    // halo (1; 2 with Act) in y and z
+  int hx;                   // x offset of the subsection inside the tile (4: TMA start alignment)
+  int TX, TY, TZ;           // tile extents in words (TX = S + 2*hx rounded up to 4)
+  int AX;                   // Act tile row pitch in bytes (same x origin as the id tile)
+  int tile_bytes, act_tile_bytes, warp_smem_bytes;
+  int use_tma;
+  const int32_t *J; int nT;
+  const TypeParams *types;
+  const uint32_t *thr; long long Hmax; int accept_all;
+  const int32_t *logq16;    // [256]
+  const int32_t *expq16;    // [1024]
+  const unsigned long long *snapVP;  // {V:hi32, P:lo32} per cell, phase-start snapshot
+  unsigned long long *liveVP;
+  unsigned long long *sumx, *sumy, *sumz;
+  unsigned long long *counters;      // [COUNTER_SLOTS][2] evaluated, accepted
+  int *error_flag;
+};
+
+// ------------------------------------------------------------------ PTX wrappers ----------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, uint64_t *bar, int x, int y, int z) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+               ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *tm, uint64_t *bar, int x, int y) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+
+// ------------------------------------------------------------------ Philox4x32-10 ---------
+// Salmon et al. 2011; counter-based, so any schedule reproduces the same stream (north_star (d)).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c.x;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c.z;
+    c = make_uint4((uint32_t)(p1 >> 32) ^ c.y ^ k0, (uint32_t)p1, (uint32_t)(p0 >> 32) ^ c.w ^ k1, (uint32_t)p0);
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  return c;
+}
+__device__ __forceinline__ uint32_t pick(const uint4 &v, int j) { return j == 0 ? v.x : j == 1 ? v.y : j == 2 ? v.z : v.w; }
+
+// neighbour index (0..nNb-1, centre skipped) -> (dx,dy,dz); order: (dz,dy,dx) lexicographic, dx fastest
+template <int DIM>
+__device__ __forceinline__ void nb_delta(int nb, int &dx, int &dy, int &dz) {
+  constexpr int half = (DIM == 2) ? 4 : 13;
+  const int i = nb + (nb >= half ? 1 : 0);
+  dx = i % 3 - 1;
+  dy = (i / 3) % 3 - 1;
+  dz = (DIM == 3) ? (i / 9 - 1) : 0;
+}
+
+// per-warp table of the cells this activation touched (own deltas, deterministic mode):
+// entry e lives in lane e%32 of set e/32.
+template <int NSETS>
+struct CellTable {
+  uint32_t key[NSETS];
+  unsigned long long base[NSETS];  // snapshot {V,P}
+  unsigned long long dvp[NSETS];   // own composite delta: dV*2^32 + dP (mod 2^64)
+  int dsx[NSETS], dsy[NSETS], dsz[NSETS];
+};
+
+template <int DIM, bool ACT, bool LIVE, int NSETS>
+struct Sweep {
+  static constexpr int NNB = (DIM == 2) ? 8 : 26;
+
+  const SweepParams &P;
+  uint32_t *tile;
+  uint8_t *atile;
+  int lane;
+  int doff, adoff;     // this lane's neighbour offset in the tile / Act tile (lane < NNB)
+  int ox, oy, oz;      // lattice origin of the subsection
+  uint32_t b;          // subsection index
+  uint32_t mcs;
+  CellTable<NSETS> tab;
+  int n_entries;
+  bool dirty;
+  bool overflow;
+
+  __device__ Sweep(const SweepParams &p) : P(p) {}
+
+  __device__ __forceinline__ void local_coords(int l, int &lx, int &ly, int &lz) const {
+    if (P.log2S >= 0) {
+      lx = l & (P.S - 1);
+      ly = (l >> P.log2S) & (P.S - 1);
+      lz = (DIM == 3) ? (l >> (2 * P.log2S)) : 0;
+    } else {
+      lx = l % P.S;
+      const int r = l / P.S;
+      ly = r % P.S;
+      lz = (DIM == 3) ? (r / P.S) : 0;
+    }
+  }
+  __device__ __forceinline__ int tile_pos(int lx, int ly, int lz) const {
+    return ((DIM == 3 ? (lz + P.h) * P.TY : 0) + (ly + P.h)) * P.TX + lx + P.hx;
+  }
+  __device__ __forceinline__ int atile_pos(int lx, int ly, int lz) const {
+    return ((DIM == 3 ? (lz + P.h) * P.TY : 0) + (ly + P.h)) * P.AX + lx + P.hx;
+  }
+
+  // ---- per-cell state as this attempt sees it (a6) ----
+  // deterministic: snapshot + own deltas; returns the entry index through e
+  __device__ __forceinline__ unsigned long long lookup(uint32_t cell, int &e) {
+    if (LIVE) {
+      e = -1;
+      return __ldcg(P.liveVP + cell);  // live, possibly stale (L53)
+    }
+    unsigned long long cur = 0;
+    bool found = false;
+#pragma unroll
+    for (int s = 0; s < NSETS; ++s) {
+      const unsigned m = __ballot_sync(FULL, tab.key[s] == cell);
+      if (m != 0 && !found) {
+        const int src = __ffs(m) - 1;
+        cur = __shfl_sync(FULL, tab.base[s] + tab.dvp[s], src);
+        e = s * 32 + src;
+        found = true;
+      }
+    }
+    if (found) return cur;
+    const unsigned long long base = __ldg(P.snapVP + cell);
+    if (n_entries >= 32 * NSETS) {  // table full: cannot keep own deltas -> report, keep going
+      overflow = true;
+      e = -1;
+      return base;
+    }
+    e = n_entries++;
+#pragma unroll
+    for (int s = 0; s < NSETS; ++s)
+      if ((e >> 5) == s && lane == (e & 31)) {
+        tab.key[s] = cell; tab.base[s] = base; tab.dvp[s] = 0ull; tab.dsx[s] = 0; tab.dsy[s] = 0; tab.dsz[s] = 0;
+      }
+    return base;
+  }
+
+  __device__ __forceinline__ void add_delta(uint32_t cell, int e, long long dV, long long dP, int x, int y, int z, int sgn) {
+    const unsigned long long d = ((unsigned long long)dV << 32) + (unsigned long long)dP;  // composite, mod 2^64
+    if (LIVE) {
+      if (lane == 0) {
+        atomicAdd(P.liveVP + cell, d);
+        atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
+        atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
+        if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
+      }
+      return;
+    }
+    if (e < 0) return;  // overflowed table: error already flagged
+#pragma unroll
+    for (int s = 0; s < NSETS; ++s)
+      if ((e >> 5) == s && lane == (e & 31)) {
+        tab.dvp[s] += d; tab.dsx[s] += sgn * x; tab.dsy[s] += sgn * y; tab.dsz[s] += sgn * z;
+      }
+  }
+
+  // fixed-point geometric mean of Act over {x} + same-cell Moore neighbours of x (Eq 9, reading S8)
+  __device__ __forceinline__ int gm_q16(int pos, int apos, uint32_t id) {
+    const bool in = lane <= NNB;
+    const int mypos = pos + (lane < NNB ? doff : 0);
+    const int myapos = apos + (lane < NNB ? adoff : 0);
+    bool same = false;
+    int a = 1;
+    if (in) {
+      same = (lane == NNB) || ((tile[mypos] & ID_MASK) == id);
+      if (same) a = atile[myapos];
+    }
+    const unsigned msame = __ballot_sync(FULL, same);
+    const unsigned mzero = __ballot_sync(FULL, same && a == 0);
+    const int lg = same ? __ldg(P.logq16 + a) : 0;
+    const int ssum = __reduce_add_sync(FULL, lg);
+    if (mzero) return 0;
+    const int n = __popc(msame);
+    const int m = ssum / n;
+    return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
+  }
+
+  // One evaluated copy attempt (a5-a9): target tile position tpos, neighbour index nb, attempt a.
+  // Warp-uniform control flow.  Returns true if the copy was accepted and committed.
+  __device__ __forceinline__ bool evaluate(int l, int nb, uint32_t a) {
+    int lx, ly, lz;
+    local_coords(l, lx, ly, lz);
+    const int tpos = tile_pos(lx, ly, lz);
+    int dx, dy, dz;
+    nb_delta<DIM>(nb, dx, dy, dz);
+    const int spos = tpos + (dz * P.TY + dy) * P.TX + dx;
+    const uint32_t wA = tile[spos], wB = tile[tpos];
+    const uint32_t A = wA & ID_MASK, B = wB & ID_MASK;
+    const int tA = (wA >> 24) & 127, tB = (wB >> 24) & 127;
+
+    // neighbour census, lanes = Moore neighbours of t
+    const bool nl = lane < NNB;
+    const uint32_t wn = nl ? tile[tpos + doff] : 0u;
+    const uint32_t idn = wn & ID_MASK;
+    const int tn = (wn >> 24) & 127;
+    const bool eA = nl && idn == A, eB = nl && idn == B;
+    const int nA = __popc(__ballot_sync(FULL, eA));
+    const int nB = __popc(__ballot_sync(FULL, eB));
+    int adh_l = 0;
+    if (nl) {
+      if (!eA) adh_l += __ldg(P.J + tA * P.nT + tn);
+      if (!eB) adh_l -= __ldg(P.J + tB * P.nT + tn);
+    }
+    long long dH = __reduce_add_sync(FULL, adh_l);
+
+    int entA = -1, entB = -1;
+    unsigned long long vpA = 0, vpB = 0;
+    if (A != 0) vpA = lookup(A, entA);
+    if (B != 0) vpB = lookup(B, entB);
+    const long long VA = (long long)(vpA >> 32), PA = (long long)(uint32_t)vpA;
+    const long long VB = (long long)(vpB >> 32), PB = (long long)(uint32_t)vpB;
+    if (B != 0 && VB <= 1) return false;  // a cell is never erased (reading S13)
+
+    const TypeParams pa = P.types[tA], pb = P.types[tB];
+    const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
+    if (A != 0) {
+      dH += (long long)pa.lamV * (2 * (VA - pa.tgtV) + 1);
+      dH += (long long)pa.lamP * dPA * (2 * (PA - pa.tgtP) + dPA);
+    }
+    if (B != 0) {
+      dH += (long long)pb.lamV * (1 - 2 * (VB - pb.tgtV));
+      dH += (long long)pb.lamP * dPB * (2 * (PB - pb.tgtP) + dPB);
+    }
+    int atpos = 0;
+    if (ACT) {
+      atpos = atile_pos(lx, ly, lz);
+      long long sideA = 0, sideB = 0;
+      if (A != 0 && pa.lamA != 0 && pa.maxA != 0) {
+        const int g = gm_q16(spos, atpos + (dz * P.TY + dy) * P.AX + dx, A);
+        if (g != 0) sideA = ((long long)pa.lamA * g) / pa.maxA;
+      }
+      if (B != 0 && pb.lamA != 0 && pb.maxA != 0) {
+        const int g = gm_q16(tpos, atpos, B);
+        if (g != 0) sideB = ((long long)pb.lamA * g) / pb.maxA;
+      }
+      dH -= (sideA - sideB + 32768) >> 16;  // copies FROM active areas are favoured (L259)
+    }
+
+    // Metropolis (Eq 2) with the integer threshold table
+    bool acc;
+    if (dH <= 0 || P.accept_all) acc = true;
+    else if (dH > P.Hmax) acc = false;
+    else {
+      const uint4 u = philox4x32_10(make_uint4(a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
+      acc = pick(u, a & 3) < __ldg(P.thr + dH);
+    }
+    if (!acc) return false;
+
+    // commit (a9)
+    if (lane == 0) {
+      tile[tpos] = wA;  // id and type of the source; neither site is frozen
+      if (ACT) atile[atpos] = (A != 0) ? (uint8_t)pa.maxA : (uint8_t)0;
+    }
+    __syncwarp();
+    dirty = true;
+    const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
+    if (A != 0) add_delta(A, entA, 1, dPA, gx, gy, gz, +1);
+    if (B != 0) add_delta(B, entB, -1, dPB, gx, gy, gz, -1);
+    return true;
+  }
+
+  // lattice coordinate of tile element (lx,ly,lz) under the boundary rule; false = outside (medium)
+  __device__ __forceinline__ bool resolve(int lx, int ly, int lz, int &gx, int &gy, int &gz) const {
+    int g[3] = {ox - P.hx + lx, oy - P.h + ly, (DIM == 3) ? oz - P.h + lz : 0};
+    const int dimv[3] = {P.X, P.Y, P.Z};
+    bool inside = true;
+#pragma unroll
+    for (int ax = 0; ax < DIM; ++ax) {
+      if (g[ax] < 0 || g[ax] >= dimv[ax]) {
+        if (P.per[ax]) g[ax] = (g[ax] % dimv[ax] + dimv[ax]) % dimv[ax];
+        else inside = false;
+      }
+    }
+    gx = g[0]; gy = g[1]; gz = g[2];
+    return inside;
+  }
+
+  // ---- id tile staging without TMA (periodic wrap across the lattice border, S % 4 != 0, or TMA off) ----
+  __device__ void load_tile_manual() {
+    const int n = P.TX * P.TY * P.TZ;
+    for (int i = lane; i < n; i += 32) {
+      const int lx = i % P.TX;
+      const int r = i / P.TX;
+      int gx, gy, gz;
+      const bool inside = resolve(lx, r % P.TY, r / P.TY, gx, gy, gz);
+      tile[i] = inside ? P.lat[(long long)gx + P.pitch * ((long long)gy + (long long)P.Y * gz)] : 0u;
+    }
+  }
+
+  // ---- Act tile staging: 32-bit loads (4 voxels) when rows are word aligned, bytes otherwise ----
+  __device__ void load_act_tile() {
+    if ((P.S & 3) == 0) {
+      const int wpr = P.AX >> 2;
+      const int n = wpr * P.TY * P.TZ;
+      uint32_t *at32 = reinterpret_cast<uint32_t *>(atile);
+      for (int i = lane; i < n; i += 32) {
+        const int q = i % wpr;
+        const int r = i / wpr;
+        int gx, gy, gz;
+        // X is a multiple of S (hence of 4): a word never straddles the lattice border
+        const bool inside = resolve(4 * q, r % P.TY, r / P.TY, gx, gy, gz);
+        at32[i] = inside ? *reinterpret_cast<const uint32_t *>(P.act + (long long)gx + P.apitch * ((long long)gy + (long long)P.Y * gz)) : 0u;
+      }
+    } else {
+      const int n = P.AX * P.TY * P.TZ;
+      for (int i = lane; i < n; i += 32) {
+        const int lx = i % P.AX;
+        const int r = i / P.AX;
+        int gx, gy, gz;
+        const bool inside = resolve(lx, r % P.TY, r / P.TY, gx, gy, gz);
+        atile[i] = inside ? P.act[(long long)gx + P.apitch * ((long long)gy + (long long)P.Y * gz)] : (uint8_t)0;
+      }
+    }
+  }
+
+  // ---- write the interior of the tile back (a10) ----
+  __device__ void store_tile() {
+    const int S = P.S;
+    const int rows = (DIM == 3) ? S * S : S;
+    if ((S & 3) == 0) {  // 128-bit stores: x0 is a multiple of S, the pitch a multiple of 4 words
+      const int qpr = S >> 2;
+      for (int i = lane; i < rows * qpr; i += 32) {
+        const int q = i % qpr, r = i / qpr;
+        const int ly = r % S, lz = r / S;
+        const int tp = tile_pos(4 * q, ly, lz);
+        const uint4 v = make_uint4(tile[tp], tile[tp + 1], tile[tp + 2], tile[tp + 3]);
+        const long long gi = (long long)(ox + 4 * q) + P.pitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+        *reinterpret_cast<uint4 *>(P.lat + gi) = v;
+      }
+    } else {
+      for (int i = lane; i < rows * S; i += 32) {
+        const int lx = i % S, r = i / S;
+        const int ly = r % S, lz = r / S;
+        const long long gi = (long long)(ox + lx) + P.pitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+        P.lat[gi] = tile[tile_pos(lx, ly, lz)];
+      }
+    }
+    if (ACT) {
+      if ((S & 3) == 0) {
+        const int qpr = S >> 2;
+        for (int i = lane; i < rows * qpr; i += 32) {
+          const int q = i % qpr, r = i / qpr;
+          const int ly = r % S, lz = r / S;
+          const long long gi = (long long)(ox + 4 * q) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+          *reinterpret_cast<uint32_t *>(P.act + gi) = *reinterpret_cast<const uint32_t *>(atile + atile_pos(4 * q, ly, lz));
+        }
+      } else {
+        for (int i = lane; i < rows * S; i += 32) {
+          const int lx = i % S, r = i / S;
+          const int ly = r % S, lz = r / S;
+          const long long gi = (long long)(ox + lx) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+          P.act[gi] = atile[atile_pos(lx, ly, lz)];
+        }
+      }
+    }
+  }
+
+  __device__ void flush_table() {
+    if constexpr (!LIVE) {
+#pragma unroll
+    for (int s = 0; s < NSETS; ++s) {
+      if (s * 32 + lane < n_entries) {
+        const uint32_t c = tab.key[s];
+        if (tab.dvp[s] != 0ull) atomicAdd(P.liveVP + c, tab.dvp[s]);
+        if (tab.dsx[s] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)tab.dsx[s]);
+        if (tab.dsy[s] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)tab.dsy[s]);
+        if (DIM == 3 && tab.dsz[s] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)tab.dsz[s]);
+      }
+    }
+    }
+  }
+
+  // ---- the whole activation of one subsection ----
+  __device__ void run(unsigned long long w, uint32_t *tile_, uint8_t *atile_, uint64_t *bar,
+                      const CUtensorMap *tm_lat) {
+    tile = tile_; atile = atile_;
+    lane = threadIdx.x & 31;
+    dirty = false; overflow = false; n_entries = 0;
+#pragma unroll
+    for (int s = 0; s < NSETS; ++s) { tab.key[s] = 0xFFFFFFFFu; tab.base[s] = 0; tab.dvp[s] = 0; tab.dsx[s] = tab.dsy[s] = tab.dsz[s] = 0; }
+    mcs = *P.mcs_ptr;
+
+    // active subsection -> lattice origin
+    const int ax = (int)(w % (unsigned)P.nact[0]);
+    const unsigned long long r1 = w / (unsigned)P.nact[0];
+    const int ay = (int)(r1 % (unsigned)P.nact[1]);
+    const int az = (int)(r1 / (unsigned)P.nact[1]);
+    const int bx = 2 * ax + P.col[0], by = 2 * ay + P.col[1], bz = (DIM == 3) ? 2 * az + P.col[2] : 0;
+    b = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
+    ox = bx * P.S; oy = by * P.S; oz = (DIM == 3) ? bz * P.S : 0;
+
+    {  // this lane's neighbour offsets
+      int dx = 0, dy = 0, dz = 0;
+      if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
+      doff = (dz * P.TY + dy) * P.TX + dx;
+      adoff = (dz * P.TY + dy) * P.AX + dx;
+    }
+
+    // a2: stage tile + halo
+    bool tma = P.use_tma != 0;
+    if (tma) {
+      const int lo[3] = {ox - P.hx, oy - P.h, oz - P.h};
+      const int ext[3] = {P.TX, P.TY, P.TZ};
+      const int dimv[3] = {P.X, P.Y, P.Z};
+#pragma unroll
+      for (int a2 = 0; a2 < DIM; ++a2)
+        if (P.per[a2] && (lo[a2] < 0 || lo[a2] + ext[a2] > dimv[a2])) tma = false;  // wrap: manual path
+    }
+    if (tma) {
+      if (lane == 0) {
+        mbar_expect_tx(bar, (uint32_t)P.tile_bytes);
+        if (DIM == 3) tma_load_3d(tile, tm_lat, bar, ox - P.hx, oy - P.h, oz - P.h);
+        else tma_load_2d(tile, tm_lat, bar, ox - P.hx, oy - P.h);
+      }
+      if (ACT) load_act_tile();  // overlaps the TMA
+      while (!mbar_try_wait(bar, 0)) {}
+    } else {
+      load_tile_manual();
+      if (ACT) load_act_tile();
+    }
+    __syncwarp();
+
+    // a3-a9: k sequential attempts, 128 proposals per batch
+    const uint32_t k = (uint32_t)P.k;
+    const uint32_t ncalls = (k + 3) >> 2;
+    uint32_t n_eval = 0, n_acc = 0;
+    for (uint32_t q0 = 0; q0 < ncalls; q0 += 32) {
+      const uint32_t q = q0 + lane;
+      int prop[4];  // l | nb << 24
+      int ts[4];    // tpos | spos << 16
+      uint32_t valid = 0;
+      if (q < ncalls) {
+        const uint4 r = philox4x32_10(make_uint4(q, b, 2u * P.p, mcs), P.key0, P.key1);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t wj = pick(r, j);
+          const uint64_t prod = (uint64_t)wj * (uint32_t)P.sites;
+          const int l = (int)(prod >> 32);
+          const int nb = (int)(((uint64_t)(uint32_t)prod * (uint32_t)NNB) >> 32);
+          int lx, ly, lz, dx, dy, dz;
+          local_coords(l, lx, ly, lz);
+          nb_delta<DIM>(nb, dx, dy, dz);
+          const int tp = tile_pos(lx, ly, lz);
+          const int sp = tp + (dz * P.TY + dy) * P.TX + dx;
+          prop[j] = l | (nb << 24);
+          ts[j] = tp | (sp << 16);
+          if (4 * q + j < k) valid |= 1u << j;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { prop[j] = 0; ts[j] = 0; }
+      }
+      // a4: screen all proposals of the batch against the current tile
+      auto screen = [&]() -> uint32_t {
+        uint32_t m = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t wt = tile[ts[j] & 0xFFFF], ws = tile[(uint32_t)ts[j] >> 16];
+          const bool interesting = (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
+          m |= interesting ? (1u << j) : 0u;
+        }
+        return m & valid;
+      };
+      uint32_t alive = screen();
+      while (true) {
+        const unsigned bal = __ballot_sync(FULL, alive != 0u);
+        if (bal == 0u) break;
+        const int src = __ffs(bal) - 1;
+        const uint32_t nib = __shfl_sync(FULL, alive, src);
+        const int j = __ffs(nib) - 1;
+        const int mine = (j == 0) ? prop[0] : (j == 1) ? prop[1] : (j == 2) ? prop[2] : prop[3];
+        const int pr = __shfl_sync(FULL, mine, src);
+        ++n_eval;
+        const bool acc = evaluate(pr & 0xFFFFFF, (pr >> 24) & 31, 4u * (q0 + (uint32_t)src) + (uint32_t)j);
+        if (lane == src) alive &= ~(1u << j);
+        if (acc) {
+          ++n_acc;
+          const uint32_t later = (lane > src) ? 0xFu : (lane == src) ? ((0xFu << (j + 1)) & 0xFu) : 0u;
+          alive = screen() & later;
+        }
+      }
+    }
+
+    // a10: write back, flush deltas
+    if (dirty) store_tile();
+    flush_table();
+    if (lane == 0) {
+      const int slot = (int)(blockIdx.x % COUNTER_SLOTS);
+      if (n_eval) atomicAdd(P.counters + 2 * slot, (unsigned long long)n_eval);
+      if (n_acc) atomicAdd(P.counters + 2 * slot + 1, (unsigned long long)n_acc);
+      if (overflow) atomicOr(P.error_flag, 1);
+    }
+  }
+};
+
+// One warp per active subsection.  Dynamic smem: per warp [tile | act tile], then the mbarriers.
+template <int DIM, bool ACT, bool LIVE, int NSETS>
+__global__ void __launch_bounds__(128) sweep_kernel(const __grid_constant__ CUtensorMap tm_lat,
+                                                    const __grid_constant__ SweepParams P) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int warp = threadIdx.x >> 5;
+  const int nwarps = blockDim.x >> 5;
+  const unsigned long long w = (unsigned long long)blockIdx.x * nwarps + warp;
+  uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)nwarps * P.warp_smem_bytes);
+  if (w >= P.n_active) return;
+  unsigned char *mine = smem + (size_t)warp * P.warp_smem_bytes;
+  uint32_t *tile = reinterpret_cast<uint32_t *>(mine);
+  uint8_t *atile = mine + ((P.tile_bytes + 127) & ~127);
+  if ((threadIdx.x & 31) == 0) {
+    mbar_init(&bars[warp], 1);
+    fence_mbar_init();
+  }
+  __syncwarp();
+  Sweep<DIM, ACT, LIVE, NSETS> sw(P);
+  sw.run(w, tile, atile, &bars[warp], &tm_lat);
+}
+
+// ------------------------------------------------------------------ auxiliary kernels ------
+// a11: Act decays by 1 per MCS down to 0 (L255); 16 bytes per thread, saturating byte subtract.
+__global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *mcs_ptr += 1;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long j = i; j < n_vec; j += stride) {
+    uint4 v = act[j];
+    v.x = __vsubus4(v.x, 0x01010101u); v.y = __vsubus4(v.y, 0x01010101u);
+    v.z = __vsubus4(v.z, 0x01010101u); v.w = __vsubus4(v.w, 0x01010101u);
+    act[j] = v;
+  }
+}
+__global__ void mcs_increment_kernel(uint32_t *mcs_ptr) { *mcs_ptr += 1; }
+
+// set_lattice: ids (+frozen, cell types) -> packed pitched words; flags ids above max_cells
+__global__ void pack_kernel(const uint32_t *ids, const uint8_t *frozen, const uint8_t *ctype, uint32_t max_cells,
+                            uint32_t *lat, long long pitch, int X, int Y, int Z, int *error_flag) {
+  const long long N = (long long)X * Y * Z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const int x = (int)(i % X);
+    const long long r = i / X;
+    uint32_t id = ids[i];
+    if (id > max_cells) { atomicOr(error_flag, 2); id = 0; }
+    const uint32_t w = id | ((uint32_t)ctype[id] << 24) | ((frozen && frozen[i]) ? 0x80000000u : 0u);
+    lat[(long long)x + pitch * r] = w;
+  }
+}
+__global__ void unpack_kernel(const uint32_t *lat, long long pitch, int X, int Y, int Z, uint32_t *ids) {
+  const long long N = (long long)X * Y * Z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const int x = (int)(i % X);
+    const long long r = i / X;
+    ids[i] = lat[(long long)x + pitch * r] & ID_MASK;
+  }
+}
+__global__ void act_set_kernel(const float *src, uint8_t *act, long long apitch, int X, int Y, int Z, int *error_flag) {
+  const long long N = (long long)X * Y * Z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const int x = (int)(i % X);
+    const long long r = i / X;
+    const float v = src[i];
+    if (!(v >= 0.f) || v > 255.f || v != floorf(v)) atomicOr(error_flag, 4);
+    act[(long long)x + apitch * r] = (uint8_t)fminf(fmaxf(v, 0.f), 255.f);
+  }
+}
+__global__ void act_get_kernel(const uint8_t *act, long long apitch, int X, int Y, int Z, float *dst) {
+  const long long N = (long long)X * Y * Z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const int x = (int)(i % X);
+    const long long r = i / X;
+    dst[i] = act ? (float)act[(long long)x + apitch * r] : 0.f;
+  }
+}
+
+// recount of the per-cell globals from the lattice: V (L225), A = Moore interfaces with sites not
+// of the same cell (L234; outside-medium counts as foreign), coordinate sums (L288).
+template <int DIM>
+__global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int Y, int Z, int perx, int pery, int perz,
+                               unsigned long long *liveVP, unsigned long long *sumx, unsigned long long *sumy,
+                               unsigned long long *sumz) {
+  const long long N = (long long)X * Y * Z;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  const int per[3] = {perx, pery, perz};
+  const int dimv[3] = {X, Y, Z};
+  constexpr int NNB = (DIM == 2) ? 8 : 26;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const int x = (int)(i % X);
+    const long long r = i / X;
+    const int y = (int)(r % Y), z = (int)(r / Y);
+    const uint32_t me = lat[(long long)x + pitch * r] & ID_MASK;
+    if (me == 0) continue;
+    int foreign = 0;
+    for (int nb = 0; nb < NNB; ++nb) {
+      int dx, dy, dz;
+      nb_delta<DIM>(nb, dx, dy, dz);
+      int g[3] = {x + dx, y + dy, z + dz};
+      bool inside = true;
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        if (g[a] < 0 || g[a] >= dimv[a]) {
+          if (per[a]) g[a] = (g[a] + dimv[a]) % dimv[a];
+          else inside = false;
+        }
+      }
+      const uint32_t other = inside ? (lat[(long long)g[0] + pitch * ((long long)g[1] + (long long)Y * g[2])] & ID_MASK) : 0u;
+      foreign += (other != me);
+    }
+    atomicAdd(liveVP + me, (1ull << 32) + (unsigned long long)foreign);
+    atomicAdd(sumx + me, (unsigned long long)x);
+    atomicAdd(sumy + me, (unsigned long long)y);
+    if (DIM == 3) atomicAdd(sumz + me, (unsigned long long)z);
+  }
+}
+__global__ void stats_unpack_kernel(const unsigned long long *liveVP, long long n, uint32_t *V, uint32_t *Pm) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const unsigned long long v = (i == 0) ? 0ull : liveVP[i];
+  if (V) V[i] = (uint32_t)(v >> 32);
+  if (Pm) Pm[i] = (uint32_t)v;
+}
+__global__ void philox_debug_kernel(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 r = philox4x32_10(make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]), key[2 * i], key[2 * i + 1]);
+  out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+
+}  // namespace cpm

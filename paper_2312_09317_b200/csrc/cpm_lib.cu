@@ -1,0 +1,582 @@
+// cpm_lib.cu -- host side of the C ABI declared in include/cpm.h: parameter validation, the
+// checkerboard phase scheduler (a1), host-built tables (Metropolis thresholds, Act log/exp),
+// device state, TMA descriptors, kernel launches.  No compute happens on the host; without a
+// usable CUDA device every entry point that needs one returns CPM_ERR_CUDA.
+#include "../../include/cpm.h"
+#include "cpm_device.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace cpm;
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+typedef void (*SweepFn)(const CUtensorMap, const SweepParams);
+
+struct cpm_ctx {
+  int d = 0, device = 0;
+  cudaStream_t stream = nullptr;
+  int dim[3] = {1, 1, 1};
+  int per[3] = {0, 0, 0};
+  int nT = 0;
+  double T = 0;
+  uint64_t seed = 0;
+  int mode = 0;
+  uint32_t max_cells = 0;
+  long long N = 0;
+  int S = 0, sites = 0, k = 0, R = 0, nNb = 0;
+  int nsub[3] = {1, 1, 1};
+  bool act_enabled = false;
+  bool have_lattice = false;
+  int nsets = 1;
+  int wpc = 4;           // warps per CTA
+  size_t cta_smem = 0;
+  bool use_tma = true;
+  SweepFn fn = nullptr;
+  SweepParams sp;        // template of the launch parameters
+  CUtensorMap tm_lat;
+
+  // device state
+  uint32_t *lat = nullptr;
+  uint8_t *act = nullptr;
+  unsigned long long *liveVP = nullptr, *snapVP = nullptr, *sumx = nullptr, *sumy = nullptr, *sumz = nullptr;
+  unsigned long long *counters = nullptr;
+  int *error_flag = nullptr;
+  uint32_t *mcs_dev = nullptr;
+  int32_t *J_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
+  TypeParams *types_dev = nullptr;
+  uint32_t *thr_dev = nullptr;
+
+  std::vector<uint32_t> thr;
+  long long Hmax = 0;
+  uint32_t mcs_host = 0;      // mirror of the device counter
+  uint64_t mcs_run = 0;       // MCS executed by this context (for the attempts counter)
+  uint64_t launches = 0, sweep_launches = 0;
+
+  bool timing = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+
+  std::string err;
+};
+
+namespace {
+
+int fail(cpm_ctx *c, int code, const std::string &msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define CK(call)                                                                                      \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess)                                                                            \
+      return fail(c, e_ == cudaErrorMemoryAllocation ? CPM_ERR_OOM : CPM_ERR_CUDA,                    \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                                \
+  } while (0)
+
+template <int DIM, bool ACT, bool LIVE>
+SweepFn pick_sets(int nsets) {
+  return nsets == 1 ? (SweepFn)sweep_kernel<DIM, ACT, LIVE, 1> : (SweepFn)sweep_kernel<DIM, ACT, LIVE, 4>;
+}
+template <int DIM>
+SweepFn pick_flags(bool act, bool live, int nsets) {
+  if (act) return live ? pick_sets<DIM, true, true>(nsets) : pick_sets<DIM, true, false>(nsets);
+  return live ? pick_sets<DIM, false, true>(nsets) : pick_sets<DIM, false, false>(nsets);
+}
+// pre-generated specialised kernels per extension set
+SweepFn pick_kernel(int d, bool act, bool live, int nsets) {
+  return d == 2 ? pick_flags<2>(act, live, nsets) : pick_flags<3>(act, live, nsets);
+}
+
+int grid_for(long long n, int block = 256) {
+  long long g = (n + block - 1) / block;
+  const long long cap = 148LL * 32;  // grid-stride loops: a few waves over the 148 SMs
+  if (g > cap) g = cap;
+  if (g < 1) g = 1;
+  return (int)g;
+}
+
+int roundup(int v, int m) { return (v + m - 1) / m * m; }
+
+// a device pointer to n elements of T holding the caller's data: the caller's own pointer when it
+// is already on the device, otherwise a temporary copy
+template <class T>
+struct Staged {
+  T *p = nullptr;
+  bool owned = false;
+  ~Staged() { if (owned && p) cudaFree(p); }
+};
+template <class T>
+cudaError_t stage_in(Staged<T> &s, const T *src, size_t n, int on_device, cudaStream_t st) {
+  if (!src) return cudaSuccess;
+  if (on_device) { s.p = const_cast<T *>(src); return cudaSuccess; }
+  cudaError_t e = cudaMalloc(&s.p, n * sizeof(T));
+  if (e != cudaSuccess) return e;
+  s.owned = true;
+  return cudaMemcpyAsync(s.p, src, n * sizeof(T), cudaMemcpyHostToDevice, st);
+}
+template <class T>
+cudaError_t stage_out_begin(Staged<T> &s, T *dst, size_t n, int on_device) {
+  if (!dst) return cudaSuccess;
+  if (on_device) { s.p = dst; return cudaSuccess; }
+  cudaError_t e = cudaMalloc(&s.p, n * sizeof(T));
+  if (e == cudaSuccess) s.owned = true;
+  return e;
+}
+template <class T>
+cudaError_t stage_out_end(Staged<T> &s, T *dst, size_t n, int on_device, cudaStream_t st) {
+  if (!dst || on_device) return cudaSuccess;
+  return cudaMemcpyAsync(dst, s.p, n * sizeof(T), cudaMemcpyDeviceToHost, st);
+}
+
+int make_tensor_map(cpm_ctx *c, CUtensorMap *tm, CUtensorMapDataType dt, int elem, void *base, long long pitch_elems,
+                    int bx) {
+  void *fnp = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fnp, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fnp)
+    return fail(c, CPM_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+  PFN_encodeTiled enc = (PFN_encodeTiled)fnp;
+  const cuuint32_t rank = (cuuint32_t)c->d;
+  cuuint64_t gdim[3] = {(cuuint64_t)c->dim[0], (cuuint64_t)c->dim[1], (cuuint64_t)c->dim[2]};
+  cuuint64_t gstr[2] = {(cuuint64_t)pitch_elems * elem, (cuuint64_t)pitch_elems * elem * c->dim[1]};
+  cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)c->sp.TY, (cuuint32_t)c->sp.TZ};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(tm, dt, rank, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(c, CPM_ERR_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
+  return CPM_OK;
+}
+
+int check_device_flag(cpm_ctx *c) {
+  int flag = 0;
+  CK(cudaMemcpyAsync(&flag, c->error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (flag & 1) return fail(c, CPM_ERR_UNSUPPORTED, "a subsection touched more distinct cells in one activation than the per-warp delta table holds");
+  if (flag & 2) return fail(c, CPM_ERR_ARG, "cell id above max_cells in the lattice");
+  if (flag & 4) return fail(c, CPM_ERR_ARG, "Act values must be integers in [0,255]");
+  return CPM_OK;
+}
+
+void free_all(cpm_ctx *c) {
+  cudaFree(c->lat); cudaFree(c->act); cudaFree(c->liveVP); cudaFree(c->snapVP); cudaFree(c->sumx); cudaFree(c->sumy);
+  cudaFree(c->sumz); cudaFree(c->counters); cudaFree(c->error_flag); cudaFree(c->mcs_dev); cudaFree(c->J_dev);
+  cudaFree(c->log_dev); cudaFree(c->exp_dev); cudaFree(c->types_dev); cudaFree(c->thr_dev);
+  for (auto e : c->ev_pool) cudaEventDestroy(e);
+}
+
+}  // namespace
+
+extern "C" {
+
+int cpm_create(const cpm_params *p, cpm_ctx **out) {
+  if (!p || !out) return CPM_ERR_ARG;
+  *out = nullptr;
+  if (p->ndim != 2 && p->ndim != 3) return CPM_ERR_DIMS;
+  if (p->neighbourhood != CPM_MOORE) return CPM_ERR_UNSUPPORTED;
+  if (p->n_types < 1 || p->n_types > 127 || !p->J) return CPM_ERR_ARG;
+  if (!(p->T >= 0)) return CPM_ERR_ARG;
+  if (p->mode != CPM_MODE_DETERMINISTIC && p->mode != CPM_MODE_LIVE_ATOMICS) return CPM_ERR_ARG;
+  if (p->max_cells >= (1u << 24)) return CPM_ERR_UNSUPPORTED;
+  const int d = p->ndim, nT = p->n_types;
+  for (int a = 0; a < d; ++a) if (p->dims[a] < 1) return CPM_ERR_DIMS;
+  for (int i = 0; i < nT; ++i)
+    for (int j = 0; j < nT; ++j) {
+      if (p->J[i * nT + j] != p->J[j * nT + i]) return CPM_ERR_ARG;
+      if (p->J[i * nT + j] > (1 << 24) || p->J[i * nT + j] < -(1 << 24)) return CPM_ERR_ARG;
+    }
+  bool any_act = false;
+  for (int i = 0; i < nT; ++i) {
+    if (p->max_act && (p->max_act[i] < 0 || p->max_act[i] > 255)) return CPM_ERR_ARG;
+    if (p->lambda_act && p->lambda_act[i] < 0) return CPM_ERR_ARG;
+    if (p->max_act && p->max_act[i] != 0) any_act = true;
+  }
+
+  // ---- checkerboard scheduler (a1): subsection edge S, attempts per activation k ----
+  int S = p->subsection;
+  if (S == 0) {
+    S = (d == 2) ? 16 : 8;
+    auto divides = [&](int s) { for (int a = 0; a < d; ++a) if (p->dims[a] % s) return false; return true; };
+    while (S > 2 && !divides(S)) S /= 2;
+  }
+  if (S < 2) return CPM_ERR_DIMS;
+  long long sites = 1;
+  for (int a = 0; a < d; ++a) {
+    if (p->dims[a] % S) return CPM_ERR_DIMS;
+    if (p->periodic[a] && ((p->dims[a] / S) & 1)) return CPM_ERR_DIMS;
+    sites *= S;
+  }
+  if (sites > (1 << 24)) return CPM_ERR_UNSUPPORTED;
+  long long k = p->attempts_per_activation ? p->attempts_per_activation : sites;
+  if (k < 1 || sites % k) return CPM_ERR_ARG;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || p->device < 0 || p->device >= ndev) return CPM_ERR_CUDA;
+  if (cudaSetDevice(p->device) != cudaSuccess) return CPM_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) return CPM_ERR_CUDA;
+  if (prop.major < 10) return CPM_ERR_CUDA;  // kernels are built for sm_100a only
+
+  cpm_ctx *c = new cpm_ctx();
+  c->d = d; c->device = p->device; c->stream = (cudaStream_t)p->stream;
+  c->nT = nT; c->T = p->T; c->seed = p->seed; c->mode = p->mode; c->max_cells = p->max_cells;
+  c->N = 1;
+  for (int a = 0; a < 3; ++a) {
+    c->dim[a] = (a < d) ? p->dims[a] : 1;
+    c->per[a] = (a < d) ? (p->periodic[a] != 0) : 0;
+    c->nsub[a] = (a < d) ? c->dim[a] / S : 1;
+    c->N *= c->dim[a];
+  }
+  c->S = S; c->sites = (int)sites; c->k = (int)k; c->R = (int)(sites / k);
+  c->nNb = (d == 2) ? 8 : 26;
+  c->act_enabled = any_act;
+  c->nsets = (sites <= 512) ? 1 : 4;
+  // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
+  c->use_tma = getenv("CPM_NO_TMA") == nullptr && (S % 4 == 0);
+
+  // ---- tile geometry (a2) ----
+  SweepParams &sp = c->sp;
+  memset(&sp, 0, sizeof(sp));
+  sp.h = c->act_enabled ? 2 : 1;
+  sp.hx = 4;
+  sp.TX = roundup(S + 2 * sp.hx, 4);
+  sp.TY = S + 2 * sp.h;
+  sp.TZ = (d == 3) ? S + 2 * sp.h : 1;
+  sp.AX = sp.TX;
+  sp.tile_bytes = sp.TX * sp.TY * sp.TZ * 4;
+  sp.act_tile_bytes = c->act_enabled ? sp.AX * sp.TY * sp.TZ : 0;
+  sp.warp_smem_bytes = roundup(sp.tile_bytes, 128) + roundup(sp.act_tile_bytes, 128);
+  if ((long long)sp.TX * sp.TY * sp.TZ > 65535 || sp.TX > 256 || sp.TY > 256 || sp.AX > 256) {
+    delete c;
+    return CPM_ERR_UNSUPPORTED;
+  }
+  const size_t smem_cap = 227 * 1024;
+  c->wpc = 4;
+  while (c->wpc > 1 && (size_t)c->wpc * sp.warp_smem_bytes + 64 > 100 * 1024) c->wpc /= 2;
+  c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + 8 * c->wpc;
+  if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
+
+  // ---- host-built tables ----
+  // Metropolis thresholds (Eq 2): thr[h] = floor(exp(-h/T) 2^32), h = 1..Hmax = floor(T 32 ln 2)
+  const bool accept_all = std::isinf(p->T);
+  c->Hmax = (p->T > 0 && !accept_all) ? (long long)std::floor(p->T * 32.0 * std::log(2.0)) : 0;
+  c->thr.assign((size_t)c->Hmax + 1, 0xffffffffu);
+  for (long long h = 1; h <= c->Hmax; ++h) {
+    double v = std::floor(std::exp(-(double)h / p->T) * 4294967296.0);
+    c->thr[(size_t)h] = v >= 4294967295.0 ? 0xffffffffu : (v < 0 ? 0u : (uint32_t)v);
+  }
+  // Act fixed-point tables: log2 in Q16 for 1..255, 2^(f/1024) in Q16
+  std::vector<int32_t> logq(256, 0), expq(1024, 0);
+  for (int a = 1; a < 256; ++a) logq[a] = (int32_t)std::llround(65536.0 * std::log2((double)a));
+  for (int f = 0; f < 1024; ++f) expq[f] = (int32_t)std::llround(65536.0 * std::exp2((double)f / 1024.0));
+  std::vector<TypeParams> types(nT);
+  for (int i = 0; i < nT; ++i) {
+    TypeParams t{};
+    t.lamV = p->lambda_V ? p->lambda_V[i] : 0; t.tgtV = p->target_V ? p->target_V[i] : 0;
+    t.lamP = p->lambda_P ? p->lambda_P[i] : 0; t.tgtP = p->target_P ? p->target_P[i] : 0;
+    t.lamA = p->lambda_act ? p->lambda_act[i] : 0; t.maxA = p->max_act ? p->max_act[i] : 0;
+    types[i] = t;
+  }
+
+  // ---- device state ----
+  const long long pitch = roundup(c->dim[0], 4), apitch = roundup(c->dim[0], 16);
+  const long long rows = (long long)c->dim[1] * c->dim[2];
+  const size_t ncell = (size_t)c->max_cells + 1;
+  int rc = CPM_OK;
+  auto alloc = [&](void **ptr, size_t bytes) {
+    if (rc != CPM_OK) return;
+    cudaError_t e = cudaMalloc(ptr, bytes);
+    if (e != cudaSuccess) rc = fail(c, e == cudaErrorMemoryAllocation ? CPM_ERR_OOM : CPM_ERR_CUDA, cudaGetErrorString(e));
+    else if (cudaMemsetAsync(*ptr, 0, bytes, c->stream) != cudaSuccess) rc = CPM_ERR_CUDA;
+  };
+  alloc((void **)&c->lat, (size_t)pitch * rows * 4);
+  if (c->act_enabled) alloc((void **)&c->act, (size_t)apitch * rows);
+  alloc((void **)&c->liveVP, ncell * 8);
+  if (c->mode == CPM_MODE_DETERMINISTIC) alloc((void **)&c->snapVP, ncell * 8);
+  alloc((void **)&c->sumx, ncell * 8); alloc((void **)&c->sumy, ncell * 8); alloc((void **)&c->sumz, ncell * 8);
+  alloc((void **)&c->counters, COUNTER_SLOTS * 2 * 8);
+  alloc((void **)&c->error_flag, 4); alloc((void **)&c->mcs_dev, 4);
+  alloc((void **)&c->J_dev, (size_t)nT * nT * 4); alloc((void **)&c->log_dev, 256 * 4); alloc((void **)&c->exp_dev, 1024 * 4);
+  alloc((void **)&c->types_dev, nT * sizeof(TypeParams)); alloc((void **)&c->thr_dev, c->thr.size() * 4);
+  if (rc == CPM_OK) {
+    cudaError_t e = cudaMemcpyAsync(c->J_dev, p->J, (size_t)nT * nT * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->log_dev, logq.data(), 256 * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->exp_dev, expq.data(), 1024 * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->types_dev, types.data(), nT * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->thr_dev, c->thr.data(), c->thr.size() * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) rc = fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
+  }
+  if (rc != CPM_OK) { free_all(c); delete c; return rc; }
+
+  // ---- launch-parameter template ----
+  sp.lat = c->lat; sp.act = c->act; sp.pitch = pitch; sp.apitch = apitch;
+  sp.X = c->dim[0]; sp.Y = c->dim[1]; sp.Z = c->dim[2];
+  for (int a = 0; a < 3; ++a) { sp.per[a] = c->per[a]; sp.nsub[a] = c->nsub[a]; }
+  sp.S = S; sp.sites = c->sites; sp.k = c->k;
+  sp.log2S = -1;
+  for (int b = 1; b < 16; ++b) if ((1 << b) == S) sp.log2S = b;
+  sp.mcs_ptr = c->mcs_dev;
+  sp.key0 = (uint32_t)c->seed; sp.key1 = (uint32_t)(c->seed >> 32);
+  sp.use_tma = c->use_tma ? 1 : 0;
+  sp.J = c->J_dev; sp.nT = nT; sp.types = c->types_dev;
+  sp.thr = c->thr_dev; sp.Hmax = c->Hmax; sp.accept_all = accept_all ? 1 : 0;
+  sp.logq16 = c->log_dev; sp.expq16 = c->exp_dev;
+  sp.snapVP = c->snapVP; sp.liveVP = c->liveVP; sp.sumx = c->sumx; sp.sumy = c->sumy; sp.sumz = c->sumz;
+  sp.counters = c->counters; sp.error_flag = c->error_flag;
+
+  memset(&c->tm_lat, 0, sizeof(CUtensorMap));
+  if (c->use_tma) {
+    rc = make_tensor_map(c, &c->tm_lat, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, c->lat, pitch, sp.TX);
+    if (rc != CPM_OK) { free_all(c); delete c; return rc; }
+  }
+  c->fn = pick_kernel(d, c->act_enabled, c->mode == CPM_MODE_LIVE_ATOMICS, c->nsets);
+  cudaError_t e = cudaFuncSetAttribute((const void *)c->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cta_smem);
+  if (e != cudaSuccess) { free_all(c); delete c; return CPM_ERR_CUDA; }
+  *out = c;
+  return CPM_OK;
+}
+
+int cpm_destroy(cpm_ctx *c) {
+  if (!c) return CPM_OK;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  free_all(c);
+  delete c;
+  return CPM_OK;
+}
+
+int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, const uint8_t *cell_type, int on_device) {
+  if (!c) return CPM_ERR_ARG;
+  if (!ids || !cell_type) return fail(c, CPM_ERR_ARG, "ids and cell_type are required");
+  CK(cudaSetDevice(c->device));
+  const size_t ncell = (size_t)c->max_cells + 1;
+  Staged<uint32_t> sid; Staged<uint8_t> sfz, sct;
+  CK(stage_in(sid, ids, (size_t)c->N, on_device, c->stream));
+  CK(stage_in(sfz, frozen, (size_t)c->N, on_device, c->stream));
+  // the type table is validated on the host
+  std::vector<uint8_t> ct(ncell);
+  if (on_device) { CK(cudaMemcpyAsync(ct.data(), cell_type, ncell, cudaMemcpyDeviceToHost, c->stream)); CK(cudaStreamSynchronize(c->stream)); }
+  else memcpy(ct.data(), cell_type, ncell);
+  if (ct[0] != 0) return fail(c, CPM_ERR_ARG, "cell 0 must have type 0 (medium)");
+  for (size_t i = 0; i < ncell; ++i) if (ct[i] >= c->nT) return fail(c, CPM_ERR_ARG, "cell type out of range");
+  CK(stage_in(sct, cell_type, ncell, on_device, c->stream));
+
+  CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
+  pack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(sid.p, sfz.p, sct.p, c->max_cells, c->lat, c->sp.pitch, c->dim[0],
+                                                      c->dim[1], c->dim[2], c->error_flag);
+  c->launches++;
+  if (c->act) CK(cudaMemsetAsync(c->act, 0, (size_t)c->sp.apitch * c->dim[1] * c->dim[2], c->stream));
+  CK(cudaMemsetAsync(c->liveVP, 0, ncell * 8, c->stream));
+  CK(cudaMemsetAsync(c->sumx, 0, ncell * 8, c->stream));
+  CK(cudaMemsetAsync(c->sumy, 0, ncell * 8, c->stream));
+  CK(cudaMemsetAsync(c->sumz, 0, ncell * 8, c->stream));
+  if (c->d == 2)
+    recount_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
+                                                              c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+  else
+    recount_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
+                                                              c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+  c->launches++;
+  if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
+  CK(cudaGetLastError());
+  int rc = check_device_flag(c);
+  if (rc != CPM_OK) return rc;
+  c->have_lattice = true;
+  return CPM_OK;
+}
+
+int cpm_set_act(cpm_ctx *c, const float *act, int on_device) {
+  if (!c || !act) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->act_enabled) return fail(c, CPM_ERR_UNSUPPORTED, "the Act field needs at least one type with max_act > 0");
+  CK(cudaSetDevice(c->device));
+  Staged<float> s;
+  CK(stage_in(s, act, (size_t)c->N, on_device, c->stream));
+  CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
+  act_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s.p, c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], c->error_flag);
+  c->launches++;
+  CK(cudaGetLastError());
+  return check_device_flag(c);
+}
+
+int cpm_set_mcs(cpm_ctx *c, uint32_t mcs) {
+  if (!c) return CPM_ERR_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaMemcpyAsync(c->mcs_dev, &mcs, 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->mcs_host = mcs;
+  return CPM_OK;
+}
+
+int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
+  if (!c) return CPM_ERR_ARG;
+  if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CK(cudaSetDevice(c->device));
+  const int ncol = 1 << c->d;
+  const size_t ncell = (size_t)c->max_cells + 1;
+  for (uint32_t m = 0; m < n_mcs; ++m) {
+    for (int rep = 0; rep < c->R; ++rep)
+      for (int col = 0; col < ncol; ++col) {
+        SweepParams sp = c->sp;
+        sp.p = (uint32_t)(rep * ncol + col);
+        unsigned long long n_active = 1;
+        for (int a = 0; a < 3; ++a) {
+          sp.col[a] = (a < c->d) ? ((col >> a) & 1) : 0;
+          sp.nact[a] = (a < c->d) ? (c->nsub[a] - sp.col[a] + 1) / 2 : 1;
+          n_active *= (unsigned long long)sp.nact[a];
+        }
+        if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
+        sp.n_active = n_active;
+        const unsigned long long grid = (n_active + c->wpc - 1) / c->wpc;
+        if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (c->timing) {
+          while (c->ev_pool.size() < c->ev_used + 2) { cudaEvent_t e; CK(cudaEventCreate(&e)); c->ev_pool.push_back(e); }
+          e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
+          CK(cudaEventRecord(e0, c->stream));
+        }
+        c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
+        if (c->timing) CK(cudaEventRecord(e1, c->stream));
+        c->launches++; c->sweep_launches++;
+        // deterministic mode: the next phase-step reads the values as of its own start
+        if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
+      }
+    if (c->act_enabled) {
+      const long long n_vec = c->sp.apitch * c->dim[1] * c->dim[2] / 16;
+      act_decay_kernel<<<grid_for(n_vec), 256, 0, c->stream>>>((uint4 *)c->act, n_vec, c->mcs_dev);
+    } else {
+      mcs_increment_kernel<<<1, 1, 0, c->stream>>>(c->mcs_dev);
+    }
+    c->launches++;
+    c->mcs_host++; c->mcs_run++;
+  }
+  CK(cudaGetLastError());
+  return CPM_OK;
+}
+
+int cpm_get_lattice(cpm_ctx *c, uint32_t *ids, int on_device) {
+  if (!c || !ids) return fail(c, CPM_ERR_ARG, "null argument");
+  CK(cudaSetDevice(c->device));
+  Staged<uint32_t> s;
+  CK(stage_out_begin(s, ids, (size_t)c->N, on_device));
+  unpack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], s.p);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(stage_out_end(s, ids, (size_t)c->N, on_device, c->stream));
+  return check_device_flag(c);
+}
+
+int cpm_get_act(cpm_ctx *c, float *act, int on_device) {
+  if (!c || !act) return fail(c, CPM_ERR_ARG, "null argument");
+  CK(cudaSetDevice(c->device));
+  Staged<float> s;
+  CK(stage_out_begin(s, act, (size_t)c->N, on_device));
+  act_get_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], s.p);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(stage_out_end(s, act, (size_t)c->N, on_device, c->stream));
+  return check_device_flag(c);
+}
+
+int cpm_get_cell_stats(cpm_ctx *c, uint32_t *volume, uint32_t *perimeter, uint64_t *sx, uint64_t *sy, uint64_t *sz,
+                       int on_device) {
+  if (!c) return CPM_ERR_ARG;
+  CK(cudaSetDevice(c->device));
+  const size_t n = (size_t)c->max_cells + 1;
+  Staged<uint32_t> sv, spm;
+  CK(stage_out_begin(sv, volume, n, on_device));
+  CK(stage_out_begin(spm, perimeter, n, on_device));
+  if (volume || perimeter) {
+    stats_unpack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->liveVP, (long long)n, sv.p, spm.p);
+    c->launches++;
+    CK(cudaGetLastError());
+  }
+  CK(stage_out_end(sv, volume, n, on_device, c->stream));
+  CK(stage_out_end(spm, perimeter, n, on_device, c->stream));
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  if (sx) CK(cudaMemcpyAsync(sx, c->sumx, n * 8, kind, c->stream));
+  if (sy) CK(cudaMemcpyAsync(sy, c->sumy, n * 8, kind, c->stream));
+  if (sz) CK(cudaMemcpyAsync(sz, c->sumz, n * 8, kind, c->stream));
+  return check_device_flag(c);
+}
+
+int cpm_get_counters(cpm_ctx *c, uint64_t out[4]) {
+  if (!c || !out) return fail(c, CPM_ERR_ARG, "null argument");
+  CK(cudaSetDevice(c->device));
+  std::vector<unsigned long long> h(COUNTER_SLOTS * 2);
+  CK(cudaMemcpyAsync(h.data(), c->counters, h.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  uint64_t ev = 0, ac = 0;
+  for (int i = 0; i < COUNTER_SLOTS; ++i) { ev += h[2 * i]; ac += h[2 * i + 1]; }
+  out[0] = (uint64_t)c->N * c->mcs_run; out[1] = ev; out[2] = ac; out[3] = c->mcs_host;
+  return CPM_OK;
+}
+
+int cpm_get_schedule(cpm_ctx *c, int32_t *S, int32_t *k, int32_t *steps) {
+  if (!c) return CPM_ERR_ARG;
+  if (S) *S = c->S;
+  if (k) *k = c->k;
+  if (steps) *steps = (1 << c->d) * c->R;
+  return CPM_OK;
+}
+
+int64_t cpm_get_threshold_table(cpm_ctx *c, uint32_t *thr, uint64_t cap) {
+  if (!c) return CPM_ERR_ARG;
+  for (uint64_t h = 0; thr && h < cap && h < c->thr.size(); ++h) thr[h] = c->thr[(size_t)h];
+  return (int64_t)c->Hmax;
+}
+
+int cpm_get_launch_info(cpm_ctx *c, uint64_t out[5]) {
+  if (!c || !out) return CPM_ERR_ARG;
+  out[0] = c->launches; out[1] = c->sweep_launches; out[2] = (uint64_t)c->wpc; out[3] = (uint64_t)c->cta_smem;
+  out[4] = c->use_tma ? 1 : 0;
+  return CPM_OK;
+}
+
+int cpm_set_kernel_timing(cpm_ctx *c, int enabled) {
+  if (!c) return CPM_ERR_ARG;
+  c->timing = enabled != 0;
+  return CPM_OK;
+}
+
+int cpm_get_kernel_timing(cpm_ctx *c, double *ms_total, uint64_t *n, int reset) {
+  if (!c) return CPM_ERR_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  double tot = 0;
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, c->ev_pool[i], c->ev_pool[i + 1]));
+    tot += ms;
+  }
+  if (ms_total) *ms_total = tot;
+  if (n) *n = c->ev_used / 2;
+  if (reset) c->ev_used = 0;
+  return CPM_OK;
+}
+
+const char *cpm_last_error(const cpm_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+int cpm_debug_philox(int device, const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n) {
+  if (!ctr || !key || !out) return CPM_ERR_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) return CPM_ERR_CUDA;
+  uint32_t *dc = nullptr, *dk = nullptr, *dout = nullptr;
+  int rc = CPM_OK;
+  if (cudaMalloc(&dc, n * 16) != cudaSuccess || cudaMalloc(&dk, n * 8) != cudaSuccess || cudaMalloc(&dout, n * 16) != cudaSuccess) rc = CPM_ERR_OOM;
+  if (rc == CPM_OK) {
+    cudaMemcpy(dc, ctr, n * 16, cudaMemcpyHostToDevice);
+    cudaMemcpy(dk, key, n * 8, cudaMemcpyHostToDevice);
+    philox_debug_kernel<<<(unsigned)((n + 255) / 256), 256>>>(dc, dk, dout, (long long)n);
+    if (cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost) != cudaSuccess) rc = CPM_ERR_CUDA;
+  }
+  cudaFree(dc); cudaFree(dk); cudaFree(dout);
+  return rc;
+}
+
+}  // extern "C"

@@ -326,13 +326,18 @@ void run_subsection(oracle_ctx *c, int64_t b, uint32_t p) {
   const uint32_t key[2] = {(uint32_t)c->seed, (uint32_t)(c->seed >> 32)};
   std::map<uint32_t, Delta> loc; /* own deltas of this activation (reading S12) */
 
-  uint32_t w4[4] = {0, 0, 0, 0};
+  /* Reading S15: attempts are taken in blocks of 128; attempt a of a block uses word
+   * (a>>5)&3 of the Philox call with counter word 0 = 32*(a>>7) + (a&31).  (The paper is silent on
+   * the generator's indexing, L284; any fixed assignment of i.i.d. words to attempts is equivalent.) */
   for (int64_t a = 0; a < c->k; ++a) {
-    if ((a & 3) == 0) {
-      uint32_t ctr[4] = {(uint32_t)(a >> 2), (uint32_t)b, 2 * p + 0, c->mcs};
+    const uint32_t call = (uint32_t)(32 * (a >> 7) + (a & 31));
+    const int word = (int)((a >> 5) & 3);
+    uint32_t w4[4];
+    {
+      uint32_t ctr[4] = {call, (uint32_t)b, 2 * p + 0, c->mcs};
       philox(ctr, key, w4);
     }
-    uint32_t w = w4[a & 3];
+    uint32_t w = w4[word];
     uint32_t l, nb;
     decode_proposal(w, (uint32_t)c->sites, (uint32_t)c->nNb, &l, &nb);
     const int tx = ox + (int)(l % S);
@@ -359,10 +364,10 @@ void run_subsection(oracle_ctx *c, int64_t b, uint32_t p) {
       if (dH <= 0 || c->accept_all) acc = true;          /* Eq 2, reading S6 */
       else if (dH > c->Hmax) acc = false;                /* exp(-dH/T) < 2^-32, reading S7 */
       else {
-        uint32_t ctr[4] = {(uint32_t)(a >> 2), (uint32_t)b, 2 * p + 1, c->mcs};
+        uint32_t ctr[4] = {call, (uint32_t)b, 2 * p + 1, c->mcs};
         uint32_t u4[4];
         philox(ctr, key, u4);
-        rec_u = u4[a & 3];
+        rec_u = u4[word];
         acc = rec_u < c->thr[(size_t)dH];
       }
       if (acc) {
@@ -454,7 +459,7 @@ int oracle_create(const oracle_params *p, oracle_ctx **out) {
   };
   take(p->lambda_V, c->lamV); take(p->target_V, c->tgtV); take(p->lambda_P, c->lamP);
   take(p->target_P, c->tgtP); take(p->lambda_act, c->lamA); take(p->max_act, c->maxA);
-  for (int i = 0; i < nT; ++i) if (c->maxA[i] < 0 || c->maxA[i] > 255) { delete c; return ORACLE_ERR_ARG; }
+  for (int i = 0; i < nT; ++i) if (c->maxA[i] < 0 || c->maxA[i] > 255 || c->lamA[i] < 0) { delete c; return ORACLE_ERR_ARG; }
   c->T = p->T;
   c->accept_all = std::isinf(p->T);
   c->seed = p->seed;

@@ -11,7 +11,7 @@
 //   a5-a9 the surviving ("interesting") proposals are processed strictly in attempt order, one at
 //       a time, with lanes = Moore neighbours: ballot/popc for n_A, n_B, REDUX for the adhesion sum;
 //       after an accepted copy the not-yet-processed proposals are re-screened, so the result is
-//       exactly that of k sequential attempts;
+//       exactly that of k sequential attempts; acceptance words are drawn up front with the proposals;
 //   a10 tile written back with 128-bit stores, integer deltas flushed with 64-bit atomics.
 // Nothing here is shared with oracle/.
 #pragma once
@@ -117,7 +117,7 @@ __device__ __forceinline__ void nb_delta(int nb, int &dx, int &dy, int &dz) {
 template <int NSETS>
 struct CellTable {
   uint32_t key[NSETS];
-  unsigned long long base[NSETS];  // snapshot {V,P}
+  unsigned long long cur[NSETS];   // snapshot {V,P} + own composite delta
   unsigned long long dvp[NSETS];   // own composite delta: dV*2^32 + dP (mod 2^64)
   int dsx[NSETS], dsy[NSETS], dsz[NSETS];
 };
@@ -129,11 +129,13 @@ struct Sweep {
   const SweepParams &P;
   uint32_t *tile;
   uint8_t *atile;
+  const int32_t *sJ;        // shared copies of the small tables
+  const TypeParams *sT;
+  const int *sOff, *sAOff;  // neighbour index -> offset in the id tile / Act tile
   int lane;
   int doff, adoff;     // this lane's neighbour offset in the tile / Act tile (lane < NNB)
   int ox, oy, oz;      // lattice origin of the subsection
   uint32_t b;          // subsection index
-  uint32_t mcs;
   CellTable<NSETS> tab;
   int n_entries;
   bool dirty;
@@ -174,7 +176,7 @@ struct Sweep {
       const unsigned m = __ballot_sync(FULL, tab.key[s] == cell);
       if (m != 0 && !found) {
         const int src = __ffs(m) - 1;
-        cur = __shfl_sync(FULL, tab.base[s] + tab.dvp[s], src);
+        cur = __shfl_sync(FULL, tab.cur[s], src);
         e = s * 32 + src;
         found = true;
       }
@@ -190,13 +192,14 @@ struct Sweep {
 #pragma unroll
     for (int s = 0; s < NSETS; ++s)
       if ((e >> 5) == s && lane == (e & 31)) {
-        tab.key[s] = cell; tab.base[s] = base; tab.dvp[s] = 0ull; tab.dsx[s] = 0; tab.dsy[s] = 0; tab.dsz[s] = 0;
+        tab.key[s] = cell; tab.cur[s] = base; tab.dvp[s] = 0ull; tab.dsx[s] = 0; tab.dsy[s] = 0; tab.dsz[s] = 0;
       }
     return base;
   }
 
-  __device__ __forceinline__ void add_delta(uint32_t cell, int e, long long dV, long long dP, int x, int y, int z, int sgn) {
-    const unsigned long long d = ((unsigned long long)dV << 32) + (unsigned long long)dP;  // composite, mod 2^64
+  __device__ __forceinline__ void add_delta(uint32_t cell, int e, int dV, int dP, int x, int y, int z, int sgn) {
+    // composite delta dV*2^32 + dP, mod 2^64 (the paper's interleaved pair, L297, updated by one add)
+    const unsigned long long d = ((unsigned long long)(long long)dV << 32) + (unsigned long long)(long long)dP;
     if (LIVE) {
       if (lane == 0) {
         atomicAdd(P.liveVP + cell, d);
@@ -210,7 +213,7 @@ struct Sweep {
 #pragma unroll
     for (int s = 0; s < NSETS; ++s)
       if ((e >> 5) == s && lane == (e & 31)) {
-        tab.dvp[s] += d; tab.dsx[s] += sgn * x; tab.dsy[s] += sgn * y; tab.dsz[s] += sgn * z;
+        tab.cur[s] += d; tab.dvp[s] += d; tab.dsx[s] += sgn * x; tab.dsy[s] += sgn * y; tab.dsz[s] += sgn * z;
       }
   }
 
@@ -227,26 +230,24 @@ struct Sweep {
     }
     const unsigned msame = __ballot_sync(FULL, same);
     const unsigned mzero = __ballot_sync(FULL, same && a == 0);
+    if (mzero) return 0;
     const int lg = same ? __ldg(P.logq16 + a) : 0;
     const int ssum = __reduce_add_sync(FULL, lg);
-    if (mzero) return 0;
     const int n = __popc(msame);
     const int m = ssum / n;
     return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
   }
 
-  // One evaluated copy attempt (a5-a9): target tile position tpos, neighbour index nb, attempt a.
-  // Warp-uniform control flow.  Returns true if the copy was accepted and committed.
-  __device__ __forceinline__ bool evaluate(int l, int nb, uint32_t a) {
-    int lx, ly, lz;
-    local_coords(l, lx, ly, lz);
-    const int tpos = tile_pos(lx, ly, lz);
-    int dx, dy, dz;
-    nb_delta<DIM>(nb, dx, dy, dz);
-    const int spos = tpos + (dz * P.TY + dy) * P.TX + dx;
+  // One evaluated copy attempt (a5-a9) on tile positions tpos (target) / spos (source).
+  // Warp-uniform control flow.  ureg / preg are THIS lane's acceptance word and packed (l | nb<<24)
+  // of the current slot; the attempt's own values live in lane src and are fetched only when needed.
+  // Returns true if the copy was committed.
+  __device__ __forceinline__ bool evaluate(int tpos, int spos, int src, uint32_t ureg, int preg) {
     const uint32_t wA = tile[spos], wB = tile[tpos];
     const uint32_t A = wA & ID_MASK, B = wB & ID_MASK;
+    // medium (id 0) has no constraints (reading S3): it reads the all-zero parameter row nT
     const int tA = (wA >> 24) & 127, tB = (wB >> 24) & 127;
+    const int rA = (A != 0) ? tA : P.nT, rB = (B != 0) ? tB : P.nT;
 
     // neighbour census, lanes = Moore neighbours of t
     const bool nl = lane < NNB;
@@ -258,58 +259,60 @@ struct Sweep {
     const int nB = __popc(__ballot_sync(FULL, eB));
     int adh_l = 0;
     if (nl) {
-      if (!eA) adh_l += __ldg(P.J + tA * P.nT + tn);
-      if (!eB) adh_l -= __ldg(P.J + tB * P.nT + tn);
+      const int ja = sJ[tA * P.nT + tn], jb = sJ[tB * P.nT + tn];
+      adh_l = (eA ? 0 : ja) - (eB ? 0 : jb);
     }
     long long dH = __reduce_add_sync(FULL, adh_l);
 
     int entA = -1, entB = -1;
     unsigned long long vpA = 0, vpB = 0;
     if (A != 0) vpA = lookup(A, entA);
-    if (B != 0) vpB = lookup(B, entB);
-    const long long VA = (long long)(vpA >> 32), PA = (long long)(uint32_t)vpA;
-    const long long VB = (long long)(vpB >> 32), PB = (long long)(uint32_t)vpB;
-    if (B != 0 && VB <= 1) return false;  // a cell is never erased (reading S13)
-
-    const TypeParams pa = P.types[tA], pb = P.types[tB];
-    const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
-    if (A != 0) {
-      dH += (long long)pa.lamV * (2 * (VA - pa.tgtV) + 1);
-      dH += (long long)pa.lamP * dPA * (2 * (PA - pa.tgtP) + dPA);
-    }
     if (B != 0) {
-      dH += (long long)pb.lamV * (1 - 2 * (VB - pb.tgtV));
-      dH += (long long)pb.lamP * dPB * (2 * (PB - pb.tgtP) + dPB);
+      vpB = lookup(B, entB);
+      if ((uint32_t)(vpB >> 32) <= 1u) return false;  // a cell is never erased (reading S13)
     }
-    int atpos = 0;
+
+    // dH assembly (a7): every product is 32x32 -> 64 or 64x32 (ranges validated by cpm_create)
+    const TypeParams pa = sT[rA], pb = sT[rB];
+    const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
+    {
+      const int dva = (int)(uint32_t)(vpA >> 32) - pa.tgtV, dvb = (int)(uint32_t)(vpB >> 32) - pb.tgtV;
+      dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
+      const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
+      dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
+    }
     if (ACT) {
-      atpos = atile_pos(lx, ly, lz);
-      long long sideA = 0, sideB = 0;
-      if (A != 0 && pa.lamA != 0 && pa.maxA != 0) {
-        const int g = gm_q16(spos, atpos + (dz * P.TY + dy) * P.AX + dx, A);
-        if (g != 0) sideA = ((long long)pa.lamA * g) / pa.maxA;
+      if ((pa.lamA | pb.lamA) != 0) {  // lamA is stored as 0 when the type's Max_act is 0
+        const int pr = __shfl_sync(FULL, preg, src);
+        int lx, ly, lz;
+        local_coords(pr & 0xFFFFFF, lx, ly, lz);
+        const int atpos = atile_pos(lx, ly, lz);
+        long long sideA = 0, sideB = 0;
+        if (pa.lamA != 0) {
+          const int g = gm_q16(spos, atpos + sAOff[(pr >> 24) & 31], A);
+          if (g != 0) sideA = ((long long)pa.lamA * g) / pa.maxA;
+        }
+        if (pb.lamA != 0) {
+          const int g = gm_q16(tpos, atpos, B);
+          if (g != 0) sideB = ((long long)pb.lamA * g) / pb.maxA;
+        }
+        dH -= (sideA - sideB + 32768) >> 16;  // copies FROM active areas are favoured (L259)
       }
-      if (B != 0 && pb.lamA != 0 && pb.maxA != 0) {
-        const int g = gm_q16(tpos, atpos, B);
-        if (g != 0) sideB = ((long long)pb.lamA * g) / pb.maxA;
-      }
-      dH -= (sideA - sideB + 32768) >> 16;  // copies FROM active areas are favoured (L259)
     }
 
     // Metropolis (Eq 2) with the integer threshold table
-    bool acc;
-    if (dH <= 0 || P.accept_all) acc = true;
-    else if (dH > P.Hmax) acc = false;
-    else {
-      const uint4 u = philox4x32_10(make_uint4(a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
-      acc = pick(u, a & 3) < __ldg(P.thr + dH);
+    if (dH > 0 && !P.accept_all) {
+      if (dH > P.Hmax) return false;
+      if (__shfl_sync(FULL, ureg, src) >= __ldg(P.thr + dH)) return false;
     }
-    if (!acc) return false;
 
     // commit (a9)
+    const int l = __shfl_sync(FULL, preg, src) & 0xFFFFFF;
+    int lx, ly, lz;
+    local_coords(l, lx, ly, lz);
     if (lane == 0) {
       tile[tpos] = wA;  // id and type of the source; neither site is frozen
-      if (ACT) atile[atpos] = (A != 0) ? (uint8_t)pa.maxA : (uint8_t)0;
+      if (ACT) atile[atile_pos(lx, ly, lz)] = (uint8_t)pa.maxA;   // Max_act of the new owner; 0 for medium
     }
     __syncwarp();
     dirty = true;
@@ -349,20 +352,26 @@ struct Sweep {
 
   // ---- Act tile staging: 32-bit loads (4 voxels) when rows are word aligned, bytes otherwise ----
   __device__ void load_act_tile() {
+    const int rows = P.TY * P.TZ;
     if ((P.S & 3) == 0) {
-      const int wpr = P.AX >> 2;
-      const int n = wpr * P.TY * P.TZ;
+      const int wpr = P.AX >> 2;   // words per tile row
       uint32_t *at32 = reinterpret_cast<uint32_t *>(atile);
-      for (int i = lane; i < n; i += 32) {
-        const int q = i % wpr;
-        const int r = i / wpr;
+      // lanes walk the (row, word) grid without divisions: lane -> (r0, q0), then fixed strides
+      int q = lane % wpr, r = lane / wpr;
+      const int dq = 32 % wpr, dr = 32 / wpr;
+      int ly = r % P.TY, lz = r / P.TY;
+      while (r < rows) {
         int gx, gy, gz;
         // X is a multiple of S (hence of 4): a word never straddles the lattice border
-        const bool inside = resolve(4 * q, r % P.TY, r / P.TY, gx, gy, gz);
-        at32[i] = inside ? *reinterpret_cast<const uint32_t *>(P.act + (long long)gx + P.apitch * ((long long)gy + (long long)P.Y * gz)) : 0u;
+        const bool inside = resolve(4 * q, ly, lz, gx, gy, gz);
+        at32[r * wpr + q] = inside ? *reinterpret_cast<const uint32_t *>(P.act + (long long)gx + P.apitch * ((long long)gy + (long long)P.Y * gz)) : 0u;
+        q += dq; int adv = dr;
+        if (q >= wpr) { q -= wpr; ++adv; }
+        r += adv; ly += adv;
+        while (ly >= P.TY) { ly -= P.TY; ++lz; }
       }
     } else {
-      const int n = P.AX * P.TY * P.TZ;
+      const int n = P.AX * rows;
       for (int i = lane; i < n; i += 32) {
         const int lx = i % P.AX;
         const int r = i / P.AX;
@@ -377,15 +386,19 @@ struct Sweep {
   __device__ void store_tile() {
     const int S = P.S;
     const int rows = (DIM == 3) ? S * S : S;
-    if ((S & 3) == 0) {  // 128-bit stores: x0 is a multiple of S, the pitch a multiple of 4 words
-      const int qpr = S >> 2;
-      for (int i = lane; i < rows * qpr; i += 32) {
-        const int q = i % qpr, r = i / qpr;
-        const int ly = r % S, lz = r / S;
+    if (P.log2S >= 2) {  // 128-bit stores: x0 is a multiple of S, the pitch a multiple of 4 words
+      const int lq = P.log2S - 2;  // log2(quads per row)
+      for (int i = lane; i < (rows << lq); i += 32) {
+        const int q = i & ((1 << lq) - 1), r = i >> lq;
+        const int ly = r & (S - 1), lz = r >> P.log2S;
         const int tp = tile_pos(4 * q, ly, lz);
         const uint4 v = make_uint4(tile[tp], tile[tp + 1], tile[tp + 2], tile[tp + 3]);
         const long long gi = (long long)(ox + 4 * q) + P.pitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
         *reinterpret_cast<uint4 *>(P.lat + gi) = v;
+        if (ACT) {
+          const long long ga = (long long)(ox + 4 * q) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+          *reinterpret_cast<uint32_t *>(P.act + ga) = *reinterpret_cast<const uint32_t *>(atile + atile_pos(4 * q, ly, lz));
+        }
       }
     } else {
       for (int i = lane; i < rows * S; i += 32) {
@@ -393,23 +406,9 @@ struct Sweep {
         const int ly = r % S, lz = r / S;
         const long long gi = (long long)(ox + lx) + P.pitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
         P.lat[gi] = tile[tile_pos(lx, ly, lz)];
-      }
-    }
-    if (ACT) {
-      if ((S & 3) == 0) {
-        const int qpr = S >> 2;
-        for (int i = lane; i < rows * qpr; i += 32) {
-          const int q = i % qpr, r = i / qpr;
-          const int ly = r % S, lz = r / S;
-          const long long gi = (long long)(ox + 4 * q) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
-          *reinterpret_cast<uint32_t *>(P.act + gi) = *reinterpret_cast<const uint32_t *>(atile + atile_pos(4 * q, ly, lz));
-        }
-      } else {
-        for (int i = lane; i < rows * S; i += 32) {
-          const int lx = i % S, r = i / S;
-          const int ly = r % S, lz = r / S;
-          const long long gi = (long long)(ox + lx) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
-          P.act[gi] = atile[atile_pos(lx, ly, lz)];
+        if (ACT) {
+          const long long ga = (long long)(ox + lx) + P.apitch * ((long long)(oy + ly) + (long long)P.Y * (oz + lz));
+          P.act[ga] = atile[atile_pos(lx, ly, lz)];
         }
       }
     }
@@ -418,15 +417,15 @@ struct Sweep {
   __device__ void flush_table() {
     if constexpr (!LIVE) {
 #pragma unroll
-    for (int s = 0; s < NSETS; ++s) {
-      if (s * 32 + lane < n_entries) {
-        const uint32_t c = tab.key[s];
-        if (tab.dvp[s] != 0ull) atomicAdd(P.liveVP + c, tab.dvp[s]);
-        if (tab.dsx[s] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)tab.dsx[s]);
-        if (tab.dsy[s] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)tab.dsy[s]);
-        if (DIM == 3 && tab.dsz[s] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)tab.dsz[s]);
+      for (int s = 0; s < NSETS; ++s) {
+        if (s * 32 + lane < n_entries) {
+          const uint32_t c = tab.key[s];
+          if (tab.dvp[s] != 0ull) atomicAdd(P.liveVP + c, tab.dvp[s]);
+          if (tab.dsx[s] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)tab.dsx[s]);
+          if (tab.dsy[s] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)tab.dsy[s]);
+          if (DIM == 3 && tab.dsz[s] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)tab.dsz[s]);
+        }
       }
-    }
     }
   }
 
@@ -437,8 +436,8 @@ struct Sweep {
     lane = threadIdx.x & 31;
     dirty = false; overflow = false; n_entries = 0;
 #pragma unroll
-    for (int s = 0; s < NSETS; ++s) { tab.key[s] = 0xFFFFFFFFu; tab.base[s] = 0; tab.dvp[s] = 0; tab.dsx[s] = tab.dsy[s] = tab.dsz[s] = 0; }
-    mcs = *P.mcs_ptr;
+    for (int s = 0; s < NSETS; ++s) { tab.key[s] = 0xFFFFFFFFu; tab.cur[s] = 0; tab.dvp[s] = 0; tab.dsx[s] = tab.dsy[s] = tab.dsz[s] = 0; }
+    const uint32_t mcs = *P.mcs_ptr;
 
     // active subsection -> lattice origin
     const int ax = (int)(w % (unsigned)P.nact[0]);
@@ -448,13 +447,8 @@ struct Sweep {
     const int bx = 2 * ax + P.col[0], by = 2 * ay + P.col[1], bz = (DIM == 3) ? 2 * az + P.col[2] : 0;
     b = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
     ox = bx * P.S; oy = by * P.S; oz = (DIM == 3) ? bz * P.S : 0;
-
-    {  // this lane's neighbour offsets
-      int dx = 0, dy = 0, dz = 0;
-      if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
-      doff = (dz * P.TY + dy) * P.TX + dx;
-      adoff = (dz * P.TY + dy) * P.AX + dx;
-    }
+    doff = (lane < NNB) ? sOff[lane] : 0;
+    adoff = (lane < NNB) ? sAOff[lane] : 0;
 
     // a2: stage tile + halo
     bool tma = P.use_tma != 0;
@@ -473,71 +467,67 @@ struct Sweep {
         else tma_load_2d(tile, tm_lat, bar, ox - P.hx, oy - P.h);
       }
       if (ACT) load_act_tile();  // overlaps the TMA
-      while (!mbar_try_wait(bar, 0)) {}
     } else {
       load_tile_manual();
       if (ACT) load_act_tile();
     }
-    __syncwarp();
 
-    // a3-a9: k sequential attempts, 128 proposals per batch
+    // a3-a9: k sequential attempts in blocks of 128: lane L draws Philox call 32*block + L (4 words);
+    // attempt a of the block is word (a>>5)&3 of lane a&31, so slot j of all lanes = 32 consecutive
+    // attempts and the slots are handled one after the other (reading S15).
     const uint32_t k = (uint32_t)P.k;
-    const uint32_t ncalls = (k + 3) >> 2;
     uint32_t n_eval = 0, n_acc = 0;
-    for (uint32_t q0 = 0; q0 < ncalls; q0 += 32) {
-      const uint32_t q = q0 + lane;
-      int prop[4];  // l | nb << 24
-      int ts[4];    // tpos | spos << 16
-      uint32_t valid = 0;
-      if (q < ncalls) {
+    bool staged = false;
+    for (uint32_t a0 = 0; a0 < k; a0 += 128) {
+      const uint32_t q = (a0 >> 2) + lane;
+      int prop[4];       // l | nb << 24
+      int ts[4];         // tpos | spos << 16
+      uint32_t u[4];     // acceptance words (Philox stream 1), drawn with the proposals so that the
+                         // sequential part below never waits for a Philox
+      {
         const uint4 r = philox4x32_10(make_uint4(q, b, 2u * P.p, mcs), P.key0, P.key1);
+        const uint4 ua = philox4x32_10(make_uint4(q, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
+        u[0] = ua.x; u[1] = ua.y; u[2] = ua.z; u[3] = ua.w;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           const uint32_t wj = pick(r, j);
           const uint64_t prod = (uint64_t)wj * (uint32_t)P.sites;
           const int l = (int)(prod >> 32);
           const int nb = (int)(((uint64_t)(uint32_t)prod * (uint32_t)NNB) >> 32);
-          int lx, ly, lz, dx, dy, dz;
+          int lx, ly, lz;
           local_coords(l, lx, ly, lz);
-          nb_delta<DIM>(nb, dx, dy, dz);
           const int tp = tile_pos(lx, ly, lz);
-          const int sp = tp + (dz * P.TY + dy) * P.TX + dx;
+          const int sp = tp + sOff[nb];
           prop[j] = l | (nb << 24);
           ts[j] = tp | (sp << 16);
-          if (4 * q + j < k) valid |= 1u << j;
         }
-      } else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { prop[j] = 0; ts[j] = 0; }
       }
-      // a4: screen all proposals of the batch against the current tile
-      auto screen = [&]() -> uint32_t {
-        uint32_t m = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t wt = tile[ts[j] & 0xFFFF], ws = tile[(uint32_t)ts[j] >> 16];
-          const bool interesting = (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
-          m |= interesting ? (1u << j) : 0u;
+      if (!staged) {  // first use of the tile: wait for the TMA (the Philox above overlapped it)
+        if (tma) { while (!mbar_try_wait(bar, 0)) {} }
+        __syncwarp();
+        staged = true;
+      }
+#pragma unroll 1
+      for (int j = 0; j < 4; ++j) {
+        const bool valid = a0 + 32u * j + lane < k;
+        // a4: screen slot j of every lane against the current tile
+        auto screen = [&]() -> unsigned {
+          const uint32_t wt = tile[ts[0] & 0xFFFF], ws = tile[(uint32_t)ts[0] >> 16];
+          return __ballot_sync(FULL, valid && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0));
+        };
+        unsigned m = screen();
+        while (m != 0u) {
+          const int src = __ffs(m) - 1;
+          const int tsel = __shfl_sync(FULL, ts[0], src);
+          ++n_eval;
+          const bool acc = evaluate(tsel & 0xFFFF, (int)((uint32_t)tsel >> 16), src, u[0], prop[0]);
+          m &= m - 1;                                           // attempt src is done
+          if (acc) { ++n_acc; m = screen() & ~((2u << src) - 1u); }  // later attempts see the new tile
         }
-        return m & valid;
-      };
-      uint32_t alive = screen();
-      while (true) {
-        const unsigned bal = __ballot_sync(FULL, alive != 0u);
-        if (bal == 0u) break;
-        const int src = __ffs(bal) - 1;
-        const uint32_t nib = __shfl_sync(FULL, alive, src);
-        const int j = __ffs(nib) - 1;
-        const int mine = (j == 0) ? prop[0] : (j == 1) ? prop[1] : (j == 2) ? prop[2] : prop[3];
-        const int pr = __shfl_sync(FULL, mine, src);
-        ++n_eval;
-        const bool acc = evaluate(pr & 0xFFFFFF, (pr >> 24) & 31, 4u * (q0 + (uint32_t)src) + (uint32_t)j);
-        if (lane == src) alive &= ~(1u << j);
-        if (acc) {
-          ++n_acc;
-          const uint32_t later = (lane > src) ? 0xFu : (lane == src) ? ((0xFu << (j + 1)) & 0xFu) : 0u;
-          alive = screen() & later;
-        }
+        // rotate the next slot into position 0 (keeps every array index a compile-time constant)
+        ts[0] = ts[1]; ts[1] = ts[2]; ts[2] = ts[3];
+        u[0] = u[1]; u[1] = u[2]; u[2] = u[3];
+        prop[0] = prop[1]; prop[1] = prop[2]; prop[2] = prop[3];
       }
     }
 
@@ -553,25 +543,42 @@ struct Sweep {
   }
 };
 
-// One warp per active subsection.  Dynamic smem: per warp [tile | act tile], then the mbarriers.
+// One warp per active subsection.  Dynamic smem: per warp [id tile | Act tile], then the mbarriers,
+// then the CTA's copies of the small tables (J, per-type parameters, neighbour offsets).
 template <int DIM, bool ACT, bool LIVE, int NSETS>
 __global__ void __launch_bounds__(128) sweep_kernel(const __grid_constant__ CUtensorMap tm_lat,
                                                     const __grid_constant__ SweepParams P) {
   extern __shared__ __align__(128) unsigned char smem[];
+  constexpr int NNB = (DIM == 2) ? 8 : 26;
   const int warp = threadIdx.x >> 5;
   const int nwarps = blockDim.x >> 5;
   const unsigned long long w = (unsigned long long)blockIdx.x * nwarps + warp;
-  uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)nwarps * P.warp_smem_bytes);
-  if (w >= P.n_active) return;
-  unsigned char *mine = smem + (size_t)warp * P.warp_smem_bytes;
-  uint32_t *tile = reinterpret_cast<uint32_t *>(mine);
-  uint8_t *atile = mine + ((P.tile_bytes + 127) & ~127);
+  unsigned char *tabs = smem + (size_t)nwarps * P.warp_smem_bytes;
+  uint64_t *bars = reinterpret_cast<uint64_t *>(tabs);
+  int *sOff = reinterpret_cast<int *>(tabs + 64);
+  int *sAOff = sOff + 32;
+  TypeParams *sT = reinterpret_cast<TypeParams *>(tabs + 64 + 256);
+  int32_t *sJ = reinterpret_cast<int32_t *>(tabs + 64 + 256 + (size_t)(P.nT + 1) * sizeof(TypeParams));
+  for (int i = threadIdx.x; i < P.nT * P.nT; i += blockDim.x) sJ[i] = P.J[i];
+  for (int i = threadIdx.x; i < (P.nT + 1) * 8; i += blockDim.x)   // P.types has nT + 1 rows, the last all zero
+    reinterpret_cast<int32_t *>(sT)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+  if (threadIdx.x < 32) {
+    int dx = 0, dy = 0, dz = 0;
+    if (threadIdx.x < NNB) nb_delta<DIM>(threadIdx.x, dx, dy, dz);
+    sOff[threadIdx.x] = (dz * P.TY + dy) * P.TX + dx;
+    sAOff[threadIdx.x] = (dz * P.TY + dy) * P.AX + dx;
+  }
   if ((threadIdx.x & 31) == 0) {
     mbar_init(&bars[warp], 1);
     fence_mbar_init();
   }
-  __syncwarp();
+  __syncthreads();
+  if (w >= P.n_active) return;
+  unsigned char *mine = smem + (size_t)warp * P.warp_smem_bytes;
+  uint32_t *tile = reinterpret_cast<uint32_t *>(mine);
+  uint8_t *atile = mine + ((P.tile_bytes + 127) & ~127);
   Sweep<DIM, ACT, LIVE, NSETS> sw(P);
+  sw.sJ = sJ; sw.sT = sT; sw.sOff = sOff; sw.sAOff = sAOff;
   sw.run(w, tile, atile, &bars[warp], &tm_lat);
 }
 
@@ -636,6 +643,8 @@ __global__ void act_get_kernel(const uint8_t *act, long long apitch, int X, int 
 
 // recount of the per-cell globals from the lattice: V (L225), A = Moore interfaces with sites not
 // of the same cell (L234; outside-medium counts as foreign), coordinate sums (L288).
+// Lanes of a warp that hold the same cell id (runs along x) are combined with match_any + REDUX so
+// that one lane issues the atomics for the whole group.
 template <int DIM>
 __global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int Y, int Z, int perx, int pery, int perz,
                                unsigned long long *liveVP, unsigned long long *sumx, unsigned long long *sumy,
@@ -645,32 +654,47 @@ __global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int 
   const int per[3] = {perx, pery, perz};
   const int dimv[3] = {X, Y, Z};
   constexpr int NNB = (DIM == 2) ? 8 : 26;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-    const int x = (int)(i % X);
-    const long long r = i / X;
-    const int y = (int)(r % Y), z = (int)(r / Y);
-    const uint32_t me = lat[(long long)x + pitch * r] & ID_MASK;
-    if (me == 0) continue;
-    int foreign = 0;
-    for (int nb = 0; nb < NNB; ++nb) {
-      int dx, dy, dz;
-      nb_delta<DIM>(nb, dx, dy, dz);
-      int g[3] = {x + dx, y + dy, z + dz};
-      bool inside = true;
+  const long long first = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long n_iter = (N + stride - 1) / stride;   // same trip count for every lane of a warp
+  for (long long it = 0; it < n_iter; ++it) {
+    const long long i = first + it * stride;
+    uint32_t me = 0;
+    int x = 0, y = 0, z = 0, foreign = 0;
+    if (i < N) {
+      x = (int)(i % X);
+      const long long r = i / X;
+      y = (int)(r % Y); z = (int)(r / Y);
+      me = lat[(long long)x + pitch * r] & ID_MASK;
+      if (me != 0) {
+        for (int nb = 0; nb < NNB; ++nb) {
+          int dx, dy, dz;
+          nb_delta<DIM>(nb, dx, dy, dz);
+          int g[3] = {x + dx, y + dy, z + dz};
+          bool inside = true;
 #pragma unroll
-      for (int a = 0; a < DIM; ++a) {
-        if (g[a] < 0 || g[a] >= dimv[a]) {
-          if (per[a]) g[a] = (g[a] + dimv[a]) % dimv[a];
-          else inside = false;
+          for (int a = 0; a < DIM; ++a) {
+            if (g[a] < 0 || g[a] >= dimv[a]) {
+              if (per[a]) g[a] = (g[a] + dimv[a]) % dimv[a];
+              else inside = false;
+            }
+          }
+          const uint32_t other = inside ? (lat[(long long)g[0] + pitch * ((long long)g[1] + (long long)Y * g[2])] & ID_MASK) : 0u;
+          foreign += (other != me);
         }
       }
-      const uint32_t other = inside ? (lat[(long long)g[0] + pitch * ((long long)g[1] + (long long)Y * g[2])] & ID_MASK) : 0u;
-      foreign += (other != me);
     }
-    atomicAdd(liveVP + me, (1ull << 32) + (unsigned long long)foreign);
-    atomicAdd(sumx + me, (unsigned long long)x);
-    atomicAdd(sumy + me, (unsigned long long)y);
-    if (DIM == 3) atomicAdd(sumz + me, (unsigned long long)z);
+    const unsigned peers = __match_any_sync(FULL, me);
+    const unsigned cnt = __popc(peers);
+    const unsigned f = __reduce_add_sync(peers, (unsigned)foreign);
+    const unsigned sx = __reduce_add_sync(peers, (unsigned)x);
+    const unsigned sy = __reduce_add_sync(peers, (unsigned)y);
+    const unsigned sz = (DIM == 3) ? __reduce_add_sync(peers, (unsigned)z) : 0u;
+    if (me != 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) {
+      atomicAdd(liveVP + me, ((unsigned long long)cnt << 32) + (unsigned long long)f);
+      atomicAdd(sumx + me, (unsigned long long)sx);
+      atomicAdd(sumy + me, (unsigned long long)sy);
+      if (DIM == 3) atomicAdd(sumz + me, (unsigned long long)sz);
+    }
   }
 }
 __global__ void stats_unpack_kernel(const unsigned long long *liveVP, long long n, uint32_t *V, uint32_t *Pm) {

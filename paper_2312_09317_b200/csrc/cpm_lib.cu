@@ -195,6 +195,8 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   for (int i = 0; i < nT; ++i) {
     if (p->max_act && (p->max_act[i] < 0 || p->max_act[i] > 255)) return CPM_ERR_ARG;
     if (p->lambda_act && p->lambda_act[i] < 0) return CPM_ERR_ARG;
+    // ranges that keep the 32x32->64 products of the dH assembly exact
+    if (p->lambda_P && (p->lambda_P[i] > (1 << 24) || p->lambda_P[i] < -(1 << 24))) return CPM_ERR_ARG;
     if (p->max_act && p->max_act[i] != 0) any_act = true;
   }
 
@@ -259,7 +261,10 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   const size_t smem_cap = 227 * 1024;
   c->wpc = 4;
   while (c->wpc > 1 && (size_t)c->wpc * sp.warp_smem_bytes + 64 > 100 * 1024) c->wpc /= 2;
-  c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + 8 * c->wpc;
+  if (c->wpc > 8) c->wpc = 8;  // 64 B of mbarriers
+  // per CTA: warp tiles, 64 B of mbarriers, neighbour-offset tables (256 B), type records, J
+  const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
+  c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
   // ---- host-built tables ----
@@ -275,14 +280,18 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   std::vector<int32_t> logq(256, 0), expq(1024, 0);
   for (int a = 1; a < 256; ++a) logq[a] = (int32_t)std::llround(65536.0 * std::log2((double)a));
   for (int f = 0; f < 1024; ++f) expq[f] = (int32_t)std::llround(65536.0 * std::exp2((double)f / 1024.0));
-  std::vector<TypeParams> types(nT);
+  // per-type records; row nT is all zero (what medium, id 0, reads: no constraints, reading S3);
+  // lamA is stored as 0 when Max_act is 0 so that one test decides whether a side has an Act bias
+  std::vector<TypeParams> types(nT + 1);
   for (int i = 0; i < nT; ++i) {
     TypeParams t{};
     t.lamV = p->lambda_V ? p->lambda_V[i] : 0; t.tgtV = p->target_V ? p->target_V[i] : 0;
     t.lamP = p->lambda_P ? p->lambda_P[i] : 0; t.tgtP = p->target_P ? p->target_P[i] : 0;
-    t.lamA = p->lambda_act ? p->lambda_act[i] : 0; t.maxA = p->max_act ? p->max_act[i] : 0;
+    t.maxA = p->max_act ? p->max_act[i] : 0;
+    t.lamA = (p->lambda_act && t.maxA != 0) ? p->lambda_act[i] : 0;
     types[i] = t;
   }
+  types[nT] = TypeParams{};
 
   // ---- device state ----
   const long long pitch = roundup(c->dim[0], 4), apitch = roundup(c->dim[0], 16);
@@ -303,12 +312,12 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   alloc((void **)&c->counters, COUNTER_SLOTS * 2 * 8);
   alloc((void **)&c->error_flag, 4); alloc((void **)&c->mcs_dev, 4);
   alloc((void **)&c->J_dev, (size_t)nT * nT * 4); alloc((void **)&c->log_dev, 256 * 4); alloc((void **)&c->exp_dev, 1024 * 4);
-  alloc((void **)&c->types_dev, nT * sizeof(TypeParams)); alloc((void **)&c->thr_dev, c->thr.size() * 4);
+  alloc((void **)&c->types_dev, (nT + 1) * sizeof(TypeParams)); alloc((void **)&c->thr_dev, c->thr.size() * 4);
   if (rc == CPM_OK) {
     cudaError_t e = cudaMemcpyAsync(c->J_dev, p->J, (size_t)nT * nT * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->log_dev, logq.data(), 256 * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->exp_dev, expq.data(), 1024 * 4, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(c->types_dev, types.data(), nT * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->types_dev, types.data(), (nT + 1) * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->thr_dev, c->thr.data(), c->thr.size() * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) rc = fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));

@@ -173,7 +173,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4")
     ap.add_argument("--dims", default=None, help="override the lattice size, e.g. 256x256x256")
-    ap.add_argument("--subsection", type=int, default=0)
+    ap.add_argument("--subsection", type=int, default=0, help="checkerboard subsection edge S; 0 = scheduler's choice")
     ap.add_argument("--mode", type=int, default=0, help="0 deterministic (default), 1 live atomics")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -203,8 +203,7 @@ def main():
     dims = cfg["dims"]
     N = int(np.prod(dims))
     params = dict(cfg["params"])
-    if args.subsection:
-        params["subsection"] = args.subsection
+    params["subsection"] = args.subsection   # 0: the library's scheduler chooses (3D: 4, 2D: 8)
     act_on = params.get("max_act") is not None and any(int(v) != 0 for v in params["max_act"])
 
     # pinned host buffers: the inputs of the end-to-end leg and the result buffer
@@ -295,7 +294,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "kernel": "sweep_kernel", "bytes_per_attempt": bpa,
+                         "traffic": traffic, "kernel": "sweep_thread_kernel" if info0["thread_per_subsection"] else "sweep_kernel", "bytes_per_attempt": bpa,
                          "launches_timed": int(sweep_n), "avg_launch_ms": 1e3 * avg_launch_s, "peak_source": peak_src,
                          "kernel_share_of_step": sweep_ms / ms,
                          "frac_with_survey_model_bytes": survey_bpa * attempts_per_launch / avg_launch_s / 1e9 / peak},

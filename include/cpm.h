@@ -97,8 +97,9 @@ int  cpm_get_schedule(cpm_ctx *ctx, int32_t *S, int32_t *k, int32_t *phase_steps
  * h = 1..Hmax; returns Hmax (>= 0) or a negative error; fills at most cap entries (thr[0] unused). */
 int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);
 /* Introspection: kernels launched by this context so far, and the launch geometry of the sweep
- * kernel: out = {launches, sweep_launches, warps_per_cta, smem_bytes_per_cta, uses_tma}. */
-int  cpm_get_launch_info(cpm_ctx *ctx, uint64_t out[5]);
+ * kernel: out = {launches, sweep_launches, warps_per_cta, smem_bytes_per_cta, uses_tma,
+ * thread_per_subsection (1: one thread per subsection, small power-of-two S; 0: one warp)}. */
+int  cpm_get_launch_info(cpm_ctx *ctx, uint64_t out[6]);
 /* Average device time (ms) of the sweep kernel launches since the last call with reset != 0,
  * measured with CUDA events on the context's stream when timing is enabled. */
 int  cpm_set_kernel_timing(cpm_ctx *ctx, int enabled);

@@ -326,14 +326,14 @@ void run_subsection(oracle_ctx *c, int64_t b, uint32_t p) {
   const uint32_t key[2] = {(uint32_t)c->seed, (uint32_t)(c->seed >> 32)};
   std::map<uint32_t, Delta> loc; /* own deltas of this activation (reading S12) */
 
-  /* Reading S15: attempts are taken in blocks of 128; attempt a of a block uses word
-   * (a>>5)&3 of the Philox call with counter word 0 = 32*(a>>7) + (a&31).  (The paper is silent on
-   * the generator's indexing, L284; any fixed assignment of i.i.d. words to attempts is equivalent.) */
+  /* Reading S15: attempt a uses word a&3 of the Philox call with counter
+   * (a>>2, b, 2p+stream, mcs): one call serves four consecutive attempts.  (The paper is silent on
+   * the generator's indexing, L284.) */
+  uint32_t w4[4] = {0, 0, 0, 0};
   for (int64_t a = 0; a < c->k; ++a) {
-    const uint32_t call = (uint32_t)(32 * (a >> 7) + (a & 31));
-    const int word = (int)((a >> 5) & 3);
-    uint32_t w4[4];
-    {
+    const uint32_t call = (uint32_t)(a >> 2);
+    const int word = (int)(a & 3);
+    if (word == 0) {
       uint32_t ctr[4] = {call, (uint32_t)b, 2 * p + 0, c->mcs};
       philox(ctr, key, w4);
     }
@@ -470,7 +470,7 @@ int oracle_create(const oracle_params *p, oracle_ctx **out) {
    * number of subsections so that same-colour subsections are never adjacent through the wrap */
   int S = p->subsection;
   if (S == 0) {
-    S = (c->d == 2) ? 16 : 8;
+    S = (c->d == 2) ? 8 : 4;   /* a small area per worker, as in the paper's Fig 4 (4x4 per thread) */
     auto divides = [&](int s) { for (int a = 0; a < c->d; ++a) if (c->dim[a] % s) return false; return true; };
     while (S > 2 && !divides(S)) S /= 2;
   }

@@ -240,10 +240,11 @@ class CPM:
         return int(hmax), thr
 
     def get_launch_info(self):
-        out = np.zeros(5, np.uint64)
+        out = np.zeros(6, np.uint64)
         self._chk(self._L.cpm_get_launch_info(self._h, out.ctypes.data))
         return {"launches": int(out[0]), "sweep_launches": int(out[1]), "warps_per_cta": int(out[2]),
-                "smem_bytes_per_cta": int(out[3]), "uses_tma": bool(out[4])}
+                "smem_bytes_per_cta": int(out[3]), "uses_tma": bool(out[4]),
+                "thread_per_subsection": bool(out[5])}
 
     def set_kernel_timing(self, enabled=True):
         self._chk(self._L.cpm_set_kernel_timing(self._h, 1 if enabled else 0))

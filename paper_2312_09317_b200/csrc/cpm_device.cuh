@@ -6,7 +6,7 @@
 //       coordinate at a 16-byte boundary (measured on B200: a 4-byte-aligned start raises
 //       "illegal instruction"), so the tile starts at x0-4 words; the 1-byte Act tile is staged
 //       with plain 32-bit loads while the TMA is in flight;
-//   a3  Philox4x32-10: every lane draws one 128-bit block = 4 proposals -> 128 proposals / batch;
+//   a3  Philox4x32-10: every lane draws one 128-bit block = 4 consecutive proposals -> 128 / batch;
 //   a4  all 128 proposals are screened in parallel against the tile (same cell / frozen);
 //   a5-a9 the surviving ("interesting") proposals are processed strictly in attempt order, one at
 //       a time, with lanes = Moore neighbours: ballot/popc for n_A, n_B, REDUX for the adhesion sum;
@@ -52,6 +52,7 @@ struct SweepParams {
   int tile_bytes, act_tile_bytes, warp_smem_bytes;
   int use_tma;
   const int32_t *J; int nT;
+  const int32_t *D;         // thread kernel: [nT^3] J(a,n) - J(b,n), then [nT] J(t,t)
   const TypeParams *types;
   const uint32_t *thr; long long Hmax; int accept_all;
   const int32_t *logq16;    // [256]
@@ -472,9 +473,8 @@ struct Sweep {
       if (ACT) load_act_tile();
     }
 
-    // a3-a9: k sequential attempts in blocks of 128: lane L draws Philox call 32*block + L (4 words);
-    // attempt a of the block is word (a>>5)&3 of lane a&31, so slot j of all lanes = 32 consecutive
-    // attempts and the slots are handled one after the other (reading S15).
+    // a3-a9: k sequential attempts in blocks of 128: lane L draws Philox call (a0>>2) + L, whose four
+    // words are attempts a0 + 4L + j, j = 0..3 (reading S15); the sequential order is (L, j) lexicographic.
     const uint32_t k = (uint32_t)P.k;
     uint32_t n_eval = 0, n_acc = 0;
     bool staged = false;
@@ -507,27 +507,37 @@ struct Sweep {
         __syncwarp();
         staged = true;
       }
-#pragma unroll 1
-      for (int j = 0; j < 4; ++j) {
-        const bool valid = a0 + 32u * j + lane < k;
-        // a4: screen slot j of every lane against the current tile
-        auto screen = [&]() -> unsigned {
-          const uint32_t wt = tile[ts[0] & 0xFFFF], ws = tile[(uint32_t)ts[0] >> 16];
-          return __ballot_sync(FULL, valid && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0));
-        };
-        unsigned m = screen();
-        while (m != 0u) {
-          const int src = __ffs(m) - 1;
-          const int tsel = __shfl_sync(FULL, ts[0], src);
-          ++n_eval;
-          const bool acc = evaluate(tsel & 0xFFFF, (int)((uint32_t)tsel >> 16), src, u[0], prop[0]);
-          m &= m - 1;                                           // attempt src is done
-          if (acc) { ++n_acc; m = screen() & ~((2u << src) - 1u); }  // later attempts see the new tile
+      // a4: screen all 128 proposals against the current tile; m[j] = lanes whose slot j is interesting
+      auto screen = [&](int tsj, bool valid) -> unsigned {
+        const uint32_t wt = tile[tsj & 0xFFFF], ws = tile[(uint32_t)tsj >> 16];
+        return __ballot_sync(FULL, valid && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0));
+      };
+      unsigned m[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) m[j] = screen(ts[j], a0 + 4u * lane + j < k);
+      while (true) {
+        const unsigned any = m[0] | m[1] | m[2] | m[3];
+        if (any == 0u) break;
+        const int src = __ffs(any) - 1;            // first lane with an interesting slot ...
+        const unsigned bit = 1u << src;
+        const int j = (m[0] & bit) ? 0 : (m[1] & bit) ? 1 : (m[2] & bit) ? 2 : 3;   // ... and its first such slot
+        const int tsv = j == 0 ? ts[0] : j == 1 ? ts[1] : j == 2 ? ts[2] : ts[3];
+        const uint32_t uv = j == 0 ? u[0] : j == 1 ? u[1] : j == 2 ? u[2] : u[3];
+        const int pv = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
+        const int tsel = __shfl_sync(FULL, tsv, src);
+        ++n_eval;
+        const bool acc = evaluate(tsel & 0xFFFF, (int)((uint32_t)tsel >> 16), src, uv, pv);
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) if (jj == j) m[jj] &= ~bit;   // attempt (src, j) is done
+        if (acc) {                                                    // later attempts see the new tile
+          ++n_acc;
+          const unsigned after = ~((2u << src) - 1u);
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) {
+            const unsigned r = screen(ts[jj], a0 + 4u * lane + jj < k);
+            m[jj] = r & (after | (jj > j ? bit : 0u));
+          }
         }
-        // rotate the next slot into position 0 (keeps every array index a compile-time constant)
-        ts[0] = ts[1]; ts[1] = ts[2]; ts[2] = ts[3];
-        u[0] = u[1]; u[1] = u[2]; u[2] = u[3];
-        prop[0] = prop[1]; prop[1] = prop[2]; prop[2] = prop[3];
       }
     }
 

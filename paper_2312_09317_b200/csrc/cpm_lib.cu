@@ -4,6 +4,7 @@
 // usable CUDA device every entry point that needs one returns CPM_ERR_CUDA.
 #include "../../include/cpm.h"
 #include "cpm_device.cuh"
+#include "cpm_thread_kernel.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -18,6 +19,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 typedef void (*SweepFn)(const CUtensorMap, const SweepParams);
+typedef void (*ThreadFn)(const SweepParams);
 
 struct cpm_ctx {
   int d = 0, device = 0;
@@ -39,6 +41,8 @@ struct cpm_ctx {
   size_t cta_smem = 0;
   bool use_tma = true;
   SweepFn fn = nullptr;
+  bool thread_kernel = false;   // one thread per subsection (small power-of-two S), else one warp
+  ThreadFn tfn = nullptr;
   SweepParams sp;        // template of the launch parameters
   CUtensorMap tm_lat;
 
@@ -49,7 +53,7 @@ struct cpm_ctx {
   unsigned long long *counters = nullptr;
   int *error_flag = nullptr;
   uint32_t *mcs_dev = nullptr;
-  int32_t *J_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
+  int32_t *J_dev = nullptr, *D_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
   TypeParams *types_dev = nullptr;
   uint32_t *thr_dev = nullptr;
 
@@ -92,6 +96,25 @@ SweepFn pick_flags(bool act, bool live, int nsets) {
 // pre-generated specialised kernels per extension set
 SweepFn pick_kernel(int d, bool act, bool live, int nsets) {
   return d == 2 ? pick_flags<2>(act, live, nsets) : pick_flags<3>(act, live, nsets);
+}
+
+template <int DIM, int S>
+ThreadFn pick_thread_flags(bool act, bool live) {
+  if (act) return live ? (ThreadFn)sweep_thread_kernel<DIM, S, true, true> : (ThreadFn)sweep_thread_kernel<DIM, S, true, false>;
+  return live ? (ThreadFn)sweep_thread_kernel<DIM, S, false, true> : (ThreadFn)sweep_thread_kernel<DIM, S, false, false>;
+}
+// one thread per subsection: 3D S = 2, 4; 2D S = 2, 4, 8, 16
+ThreadFn pick_thread_kernel(int d, int S, bool act, bool live) {
+  if (d == 3) {
+    if (S == 2) return pick_thread_flags<3, 2>(act, live);
+    if (S == 4) return pick_thread_flags<3, 4>(act, live);
+    return nullptr;
+  }
+  if (S == 2) return pick_thread_flags<2, 2>(act, live);
+  if (S == 4) return pick_thread_flags<2, 4>(act, live);
+  if (S == 8) return pick_thread_flags<2, 8>(act, live);
+  if (S == 16) return pick_thread_flags<2, 16>(act, live);
+  return nullptr;
 }
 
 int grid_for(long long n, int block = 256) {
@@ -158,7 +181,7 @@ int check_device_flag(cpm_ctx *c) {
   int flag = 0;
   CK(cudaMemcpyAsync(&flag, c->error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
-  if (flag & 1) return fail(c, CPM_ERR_UNSUPPORTED, "a subsection touched more distinct cells in one activation than the per-warp delta table holds");
+  if (flag & 1) return fail(c, CPM_ERR_UNSUPPORTED, "a subsection changed more distinct cells in one activation than its own-delta table holds");
   if (flag & 2) return fail(c, CPM_ERR_ARG, "cell id above max_cells in the lattice");
   if (flag & 4) return fail(c, CPM_ERR_ARG, "Act values must be integers in [0,255]");
   return CPM_OK;
@@ -166,7 +189,7 @@ int check_device_flag(cpm_ctx *c) {
 
 void free_all(cpm_ctx *c) {
   cudaFree(c->lat); cudaFree(c->act); cudaFree(c->liveVP); cudaFree(c->snapVP); cudaFree(c->sumx); cudaFree(c->sumy);
-  cudaFree(c->sumz); cudaFree(c->counters); cudaFree(c->error_flag); cudaFree(c->mcs_dev); cudaFree(c->J_dev);
+  cudaFree(c->sumz); cudaFree(c->counters); cudaFree(c->error_flag); cudaFree(c->mcs_dev); cudaFree(c->J_dev); cudaFree(c->D_dev);
   cudaFree(c->log_dev); cudaFree(c->exp_dev); cudaFree(c->types_dev); cudaFree(c->thr_dev);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
 }
@@ -203,7 +226,7 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   // ---- checkerboard scheduler (a1): subsection edge S, attempts per activation k ----
   int S = p->subsection;
   if (S == 0) {
-    S = (d == 2) ? 16 : 8;
+    S = (d == 2) ? 8 : 4;   // small enough for one thread per subsection (the paper's granularity, Fig 4)
     auto divides = [&](int s) { for (int a = 0; a < d; ++a) if (p->dims[a] % s) return false; return true; };
     while (S > 2 && !divides(S)) S /= 2;
   }
@@ -241,6 +264,10 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   c->nsets = (sites <= 512) ? 1 : 4;
   // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
   c->use_tma = getenv("CPM_NO_TMA") == nullptr && (S % 4 == 0);
+  c->tfn = (nT <= 8 && getenv("CPM_WARP_KERNEL") == nullptr)
+               ? pick_thread_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS) : nullptr;
+  c->thread_kernel = c->tfn != nullptr;
+  if (c->thread_kernel) c->use_tma = false;
 
   // ---- tile geometry (a2) ----
   SweepParams &sp = c->sp;
@@ -265,6 +292,14 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   // per CTA: warp tiles, 64 B of mbarriers, neighbour-offset tables (256 B), type records, J
   const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
   c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
+  if (c->thread_kernel) {
+    // one warp per CTA: interleaved (S+2)^d id tiles (+ Act bytes) of 32 lanes, then the small tables
+    size_t words = 1;
+    for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
+    c->wpc = 1;
+    c->cta_smem = words * 128 + (c->act_enabled ? words * 32 : 0) + 128 + (size_t)(nT + 1) * sizeof(TypeParams) +
+                  ((size_t)nT * nT * nT + nT) * 4;
+  }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
   // ---- host-built tables ----
@@ -292,6 +327,12 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     types[i] = t;
   }
   types[nT] = TypeParams{};
+  // adhesion difference table of the thread kernel: D[a][b][n] = J(a,n) - J(b,n), then the diagonal J(t,t)
+  std::vector<int32_t> Dtab((size_t)nT * nT * nT + nT);
+  for (int a = 0; a < nT; ++a)
+    for (int b2 = 0; b2 < nT; ++b2)
+      for (int n = 0; n < nT; ++n) Dtab[((size_t)a * nT + b2) * nT + n] = p->J[a * nT + n] - p->J[b2 * nT + n];
+  for (int t = 0; t < nT; ++t) Dtab[(size_t)nT * nT * nT + t] = p->J[t * nT + t];
 
   // ---- device state ----
   const long long pitch = roundup(c->dim[0], 4), apitch = roundup(c->dim[0], 16);
@@ -311,10 +352,11 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   alloc((void **)&c->sumx, ncell * 8); alloc((void **)&c->sumy, ncell * 8); alloc((void **)&c->sumz, ncell * 8);
   alloc((void **)&c->counters, COUNTER_SLOTS * 2 * 8);
   alloc((void **)&c->error_flag, 4); alloc((void **)&c->mcs_dev, 4);
-  alloc((void **)&c->J_dev, (size_t)nT * nT * 4); alloc((void **)&c->log_dev, 256 * 4); alloc((void **)&c->exp_dev, 1024 * 4);
+  alloc((void **)&c->J_dev, (size_t)nT * nT * 4); alloc((void **)&c->D_dev, Dtab.size() * 4); alloc((void **)&c->log_dev, 256 * 4); alloc((void **)&c->exp_dev, 1024 * 4);
   alloc((void **)&c->types_dev, (nT + 1) * sizeof(TypeParams)); alloc((void **)&c->thr_dev, c->thr.size() * 4);
   if (rc == CPM_OK) {
     cudaError_t e = cudaMemcpyAsync(c->J_dev, p->J, (size_t)nT * nT * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->D_dev, Dtab.data(), Dtab.size() * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->log_dev, logq.data(), 256 * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->exp_dev, expq.data(), 1024 * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->types_dev, types.data(), (nT + 1) * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
@@ -334,7 +376,7 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   sp.mcs_ptr = c->mcs_dev;
   sp.key0 = (uint32_t)c->seed; sp.key1 = (uint32_t)(c->seed >> 32);
   sp.use_tma = c->use_tma ? 1 : 0;
-  sp.J = c->J_dev; sp.nT = nT; sp.types = c->types_dev;
+  sp.J = c->J_dev; sp.D = c->D_dev; sp.nT = nT; sp.types = c->types_dev;
   sp.thr = c->thr_dev; sp.Hmax = c->Hmax; sp.accept_all = accept_all ? 1 : 0;
   sp.logq16 = c->log_dev; sp.expq16 = c->exp_dev;
   sp.snapVP = c->snapVP; sp.liveVP = c->liveVP; sp.sumx = c->sumx; sp.sumy = c->sumy; sp.sumz = c->sumz;
@@ -346,7 +388,8 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     if (rc != CPM_OK) { free_all(c); delete c; return rc; }
   }
   c->fn = pick_kernel(d, c->act_enabled, c->mode == CPM_MODE_LIVE_ATOMICS, c->nsets);
-  cudaError_t e = cudaFuncSetAttribute((const void *)c->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cta_smem);
+  cudaError_t e = cudaFuncSetAttribute(c->thread_kernel ? (const void *)c->tfn : (const void *)c->fn,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cta_smem);
   if (e != cudaSuccess) { free_all(c); delete c; return CPM_ERR_CUDA; }
   *out = c;
   return CPM_OK;
@@ -442,7 +485,8 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
         }
         if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
         sp.n_active = n_active;
-        const unsigned long long grid = (n_active + c->wpc - 1) / c->wpc;
+        const unsigned long long per_cta = c->thread_kernel ? 32ull : (unsigned long long)c->wpc;
+        const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
         if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (c->timing) {
@@ -450,7 +494,8 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
           e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
           CK(cudaEventRecord(e0, c->stream));
         }
-        c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
+        if (c->thread_kernel) c->tfn<<<(unsigned)grid, 32, c->cta_smem, c->stream>>>(sp);
+        else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
         if (c->timing) CK(cudaEventRecord(e1, c->stream));
         c->launches++; c->sweep_launches++;
         // deterministic mode: the next phase-step reads the values as of its own start
@@ -541,10 +586,10 @@ int64_t cpm_get_threshold_table(cpm_ctx *c, uint32_t *thr, uint64_t cap) {
   return (int64_t)c->Hmax;
 }
 
-int cpm_get_launch_info(cpm_ctx *c, uint64_t out[5]) {
+int cpm_get_launch_info(cpm_ctx *c, uint64_t out[6]) {
   if (!c || !out) return CPM_ERR_ARG;
   out[0] = c->launches; out[1] = c->sweep_launches; out[2] = (uint64_t)c->wpc; out[3] = (uint64_t)c->cta_smem;
-  out[4] = c->use_tma ? 1 : 0;
+  out[4] = c->use_tma ? 1 : 0; out[5] = c->thread_kernel ? 1 : 0;
   return CPM_OK;
 }
 

@@ -85,7 +85,39 @@ def test_C1_bit_exact_every_mcs(pk, oracle_mod):
     cfg = ci.make_config("C1")
     g, o = _run(pk, oracle_mod, cfg, 100, 1)
     assert g.get_schedule() == {"S": 16, "k": 256, "phase_steps_per_mcs": 4}
-    assert g.get_launch_info()["uses_tma"]
+    assert g.get_launch_info()["thread_per_subsection"]
+
+
+def test_C1_warp_kernel_bit_exact(pk, oracle_mod, monkeypatch):
+    """The same config through the warp-per-subsection kernel (TMA staging)."""
+    import cpm_inputs as ci
+    monkeypatch.setenv("CPM_WARP_KERNEL", "1")
+    cfg = ci.make_config("C1")
+    g, o = _run(pk, oracle_mod, cfg, 30, 5)
+    info = g.get_launch_info()
+    assert info["uses_tma"] and not info["thread_per_subsection"]
+
+
+@pytest.mark.parametrize("name,dims,act", [("C2", (64, 64, 64), False), ("C3", (64, 64, 64), True),
+                                           ("C4", (80, 80, 80), True), ("C4", (72, 40, 24), True)])
+def test_thread_kernel_S4_bit_exact(pk, oracle_mod, name, dims, act):
+    """The bench's launch configuration: one thread per 4^3 subsection (k = 64), scaled C2/C3/C4."""
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims, subsection=4)
+    g, o = _run(pk, oracle_mod, cfg, 12, 3, act=act)
+    assert g.get_schedule() == {"S": 4, "k": 64, "phase_steps_per_mcs": 8}
+    assert g.get_launch_info()["thread_per_subsection"]
+
+
+def test_default_schedule_is_thread_per_subsection(pk, oracle_mod):
+    """subsection = 0: both sides choose S = 4 (3D) / 8 (2D)."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C4", dims=(40, 40, 40))
+    g, o = _run(pk, oracle_mod, cfg, 4, 2, act=True, subsection=0)
+    assert g.get_schedule()["S"] == 4 and g.get_launch_info()["thread_per_subsection"]
+    cfg = ci.make_config("C5", dims=(64, 48))
+    g, o = _run(pk, oracle_mod, cfg, 4, 2, subsection=0)
+    assert g.get_schedule()["S"] == 8 and g.get_launch_info()["thread_per_subsection"]
 
 
 def test_C2_scaled_bit_exact(pk, oracle_mod):
@@ -132,6 +164,9 @@ def test_C5_scaled_subsection_sweep(pk, oracle_mod, S):
     ((32, 16, 16), 8, 0, (0, 1, 0)),      # mixed boundary, a single subsection pair
     ((8, 8, 8), 8, 0, (0, 0, 0)),         # one subsection: most colours are empty
     ((16, 16, 16), 2, 0, (0, 0, 0)),      # smallest subsection
+    ((32, 24, 16), 4, 0, (1, 1, 1)),      # thread kernel, periodic wrap of halo words and rows
+    ((24, 16, 8), 4, 16, (0, 1, 0)),      # thread kernel, k < S^d, mixed boundary
+    ((24, 16, 8), 2, 0, (1, 0, 1)),       # thread kernel, S = 2, periodic
 ])
 def test_3d_shapes_schedules_boundaries(pk, oracle_mod, dims, S, k, periodic):
     import cpm_inputs as ci
@@ -144,6 +179,7 @@ def test_3d_shapes_schedules_boundaries(pk, oracle_mod, dims, S, k, periodic):
 
 @pytest.mark.parametrize("dims,S,periodic", [
     ((64, 64), 16, (1, 1, 0)), ((40, 24), 8, (0, 0, 0)), ((30, 18), 6, (0, 0, 0)), ((64, 64), 32, (1, 0, 0)),
+    ((24, 16), 4, (1, 1, 0)), ((12, 20), 2, (0, 0, 0)), ((48, 32), 8, (1, 0, 0)),
 ])
 def test_2d_shapes_boundaries(pk, oracle_mod, dims, S, periodic):
     import cpm_inputs as ci
@@ -151,10 +187,11 @@ def test_2d_shapes_boundaries(pk, oracle_mod, dims, S, periodic):
     _run(pk, oracle_mod, cfg, 8, 2, periodic=periodic)
 
 
-def test_negative_J_and_extreme_temperatures(pk, oracle_mod):
+@pytest.mark.parametrize("S", [8, 4])
+def test_negative_J_and_extreme_temperatures(pk, oracle_mod, S):
     """Negative adhesion energies occur in the paper (J_cell,FRC down to -3000, L194-201)."""
     import cpm_inputs as ci
-    cfg = ci.make_config("C4", dims=(40, 40, 40))
+    cfg = ci.make_config("C4", dims=(40, 40, 40), subsection=S)
     J = cfg["params"]["J"].copy(); J[1, 3] = J[3, 1] = -400; J[2, 3] = J[3, 2] = -3000
     for T in (0.0, float("inf"), 3.0):
         _run(pk, oracle_mod, cfg, 3, 1, act=True, J=J, T=T)
@@ -299,15 +336,16 @@ def test_errors_are_reported(pk):
     assert e.value.code == -1
 
 
-def test_cell_table_overflow_is_flagged(pk):
-    """Degenerate input: every voxel its own cell and T = inf, so one 8^3 activation touches far
+@pytest.mark.parametrize("S", [8, 4])
+def test_cell_table_overflow_is_flagged(pk, S):
+    """Degenerate input: every voxel its own cell and T = inf, so one activation changes far
     more than 32 distinct cells -> the library reports CPM_ERR_UNSUPPORTED instead of silently
-    dropping deltas."""
+    dropping deltas (warp kernel S = 8, thread kernel S = 4)."""
     dims = (16, 16, 16)
     n = 16 ** 3
     ids = np.arange(1, n + 1, dtype=np.uint32).reshape(16, 16, 16)
     ct = np.ones(n + 1, np.uint8); ct[0] = 0
-    g = pk.CPM(dims, J=[[0, 1], [1, 1]], lambda_V=[0, 0], target_V=[0, 0], max_cells=n, T=float("inf"), subsection=8)
+    g = pk.CPM(dims, J=[[0, 1], [1, 1]], lambda_V=[0, 0], target_V=[0, 0], max_cells=n, T=float("inf"), subsection=S)
     # volume-1 cells cannot be erased (S13); give them volume 2 by pairing voxels along x
     ids = ((ids - 1) // 2 + 1).astype(np.uint32)
     g.set_lattice(ids, None, ct)

@@ -304,8 +304,8 @@ def test_P8_philox_known_answers(oracle_mod):
 
 
 def test_P8_counter_layout_and_decode(oracle_mod):
-    """ctr = (32*(a>>7) + (a&31), b, 2p+stream, mcs), key = seed (lo, hi); word (a>>5)&3; decode by
-    multiply-shift (readings S15, S16) -- recomputed here with the python Philox."""
+    """ctr = (a>>2, b, 2p+stream, mcs), key = seed (lo, hi); word a&3; decode by multiply-shift
+    (readings S15, S16) -- recomputed here with the python Philox."""
     import cpm_inputs as ci
     c = ci.make_config("C1", dims=(32, 32))
     seed = (0xABCDEF12 << 32) | 0x00C0FFEE
@@ -325,7 +325,7 @@ def test_P8_counter_layout_and_decode(oracle_mod):
             if ((bx & 1) | ((by & 1) << 1)) != pstep:
                 continue
             for a in range(256):
-                call, word = 32 * (a >> 7) + (a & 31), (a >> 5) & 3
+                call, word = a >> 2, a & 3
                 w = H.philox_py([call, b, 2 * pstep, 41], [seed & 0xFFFFFFFF, seed >> 32])[word]
                 prod = w * 256
                 l = prod >> 32

@@ -7,12 +7,16 @@
 //       the warp (word j of lane L at [j][L]): every later shared-memory access of a warp is
 //       bank-conflict free whatever sites the lanes picked; global loads are 128-bit for the interior
 //       of a row plus the two halo words;
-//   a3  Philox4x32-10, one call = four consecutive attempts of this lane's subsection;
-//   a4  each lane screens its own attempts (same cell / frozen) until it finds one that needs a dH,
-//       at most SCREEN_BUDGET per round, then the warp reconverges and
-//   a5-a9 all lanes that found one evaluate it together, each serially over its 26 (8) neighbours:
-//       n_A, n_B by compares, adhesion through the difference table D[tA][tB][tn] = J(tA,tn) - J(tB,tn);
-//       acceptance words (Philox stream 1) are drawn only for uphill moves inside the table range;
+//   a3  Philox4x32-10, one call = four consecutive attempts ("quad") of this lane's subsection;
+//   a4  the warp works in rounds.  Step 1 (converged): every lane without a pending attempt draws its
+//       next quad and screens its four proposals against its tile (same cell / frozen) -> 4-bit mask;
+//   a5-a9 step 2 (converged): every lane with a pending attempt evaluates the first one, serially over
+//       its 26 (8) neighbours: n_A, n_B by compares, adhesion through the difference table
+//       D[tA][tB][tn] = J(tA,tn) - J(tB,tn); after an accepted copy the rest of the quad is re-screened,
+//       so the result is exactly that of k sequential attempts; acceptance words (Philox stream 1)
+//       are drawn only for uphill moves inside the table range;
+//   Act the geometric means (Eq 9) are needed by few lanes at a time, so they are computed by the
+//       WHOLE warp for one lane after the other (lanes = the 27 sites, ballot / REDUX);
 //   a10 dirty interiors are written back with 128-bit stores, own deltas flushed with 64-bit atomics.
 // With Act the tile keeps halo 1; the geometric mean around a source that lies in the halo reads the
 // few voxels of ring 2 straight from global memory (they belong to inactive subsections, so they are
@@ -24,7 +28,7 @@
 namespace cpm {
 
 constexpr int TK_CAP = 32;          // own-delta entries per thread (cells changed in one activation)
-constexpr int SCREEN_BUDGET = 8;    // screened attempts per lane between two evaluation rounds
+constexpr int TK_REG = 8;           // of which the first keys are held in registers
 
 template <int DIM, int S>
 struct TGeom {
@@ -57,13 +61,18 @@ struct ThreadSweep {
   uint32_t *tile;          // this lane's word 0; word j at tile[32 * j]
   uint8_t *atile;          // this lane's Act byte 0; byte j at atile[32 * j]
   const int *sOff;         // neighbour index -> 32 * tile offset
+  const int *sNbr;         // neighbour index -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
   const int32_t *sD;       // [nT][nT][nT] adhesion difference table
   const int32_t *sDiag;    // [nT] J(t,t)
   const TypeParams *sT;    // [nT + 1], row nT all zero (medium)
+  const int32_t *sLog;     // [256] Q16 log2 (Act)
+  int lane;
   int ox, oy, oz;
   uint32_t b;
   uint32_t mcs;
-  // own deltas of this activation (deterministic mode), in local memory
+  // own deltas of this activation (deterministic mode): the first TK_REG keys in registers, the
+  // rest and all values in local memory
+  uint32_t rk[TK_REG];
   uint32_t key[TK_CAP];
   unsigned long long dvp[TK_CAP];
   int dsx[TK_CAP], dsy[TK_CAP], dsz[TK_CAP];
@@ -73,6 +82,10 @@ struct ThreadSweep {
   __device__ ThreadSweep(const SweepParams &p) : P(p) {}
 
   static __device__ __forceinline__ int off32(int dx, int dy, int dz) { return 32 * ((dz * T + dy) * T + dx); }
+  static __device__ __forceinline__ int site32(int l) {   // site index -> 32 * tile offset
+    const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
+    return 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1);
+  }
 
   // ---- boundary rule for one axis (reading S5): false = outside a closed lattice ----
   static __device__ __forceinline__ bool wrap(int &g, int n, int per) {
@@ -83,47 +96,55 @@ struct ThreadSweep {
 
   // ---- a2: stage this lane's tile ----
   __device__ __forceinline__ void load_tile() {
+    int xl = ox - 1, xr = ox + S;
+    const bool okxl = wrap(xl, P.X, P.per[0]);
+    const bool okxr = wrap(xr, P.X, P.per[0]);
+    constexpr int TZ = (DIM == 3) ? T : 1;
 #pragma unroll
-    for (int r = 0; r < G::ROWS; ++r) {
-      const int ty = r % T, tz = r / T;
-      int gy = oy - 1 + ty, gz = (DIM == 3) ? oz - 1 + tz : 0;
-      bool ok = wrap(gy, P.Y, P.per[1]);
-      if (DIM == 3) ok = wrap(gz, P.Z, P.per[2]) && ok;
-      const long long rowi = (long long)gy + (long long)P.Y * gz;
-      const uint32_t *rowp = P.lat + P.pitch * rowi;
-      uint32_t *dst = tile + 32 * (r * T);
-      int xl = ox - 1, xr = ox + S;
-      const bool okl = ok && wrap(xl, P.X, P.per[0]);
-      const bool okr = ok && wrap(xr, P.X, P.per[0]);
-      dst[0] = okl ? __ldg(rowp + xl) : 0u;
-      dst[32 * (S + 1)] = okr ? __ldg(rowp + xr) : 0u;
-      if constexpr (S % 4 == 0) {
+    for (int tz = 0; tz < TZ; ++tz) {
+      int gz = (DIM == 3) ? oz - 1 + tz : 0;
+      bool okz = true;
+      if (DIM == 3 && (tz == 0 || tz == T - 1)) okz = wrap(gz, P.Z, P.per[2]);   // interior planes are inside
+      const long long zrow = (long long)P.Y * gz;
 #pragma unroll
-        for (int q = 0; q < S / 4; ++q) {
-          uint4 v = make_uint4(0u, 0u, 0u, 0u);
-          if (ok) v = __ldg(reinterpret_cast<const uint4 *>(rowp + ox + 4 * q));
-          dst[32 * (1 + 4 * q)] = v.x; dst[32 * (2 + 4 * q)] = v.y; dst[32 * (3 + 4 * q)] = v.z; dst[32 * (4 + 4 * q)] = v.w;
-        }
-      } else {
-        uint2 v = make_uint2(0u, 0u);
-        if (ok) v = __ldg(reinterpret_cast<const uint2 *>(rowp + ox));
-        dst[32] = v.x; dst[64] = v.y;
-      }
-      if constexpr (ACT) {
-        const uint8_t *arow = P.act + P.apitch * rowi;
-        uint8_t *ad = atile + 32 * (r * T);
-        ad[0] = okl ? __ldg(arow + xl) : (uint8_t)0;
-        ad[32 * (S + 1)] = okr ? __ldg(arow + xr) : (uint8_t)0;
+      for (int ty = 0; ty < T; ++ty) {
+        int gy = oy - 1 + ty;
+        bool ok = okz;
+        if (ty == 0 || ty == T - 1) ok = wrap(gy, P.Y, P.per[1]) && ok;
+        const long long rowi = zrow + gy;
+        const uint32_t *rowp = P.lat + P.pitch * rowi;
+        uint32_t *dst = tile + 32 * ((tz * T + ty) * T);
+        const bool okl = ok && okxl, okr = ok && okxr;
+        dst[0] = okl ? __ldg(rowp + xl) : 0u;
+        dst[32 * (S + 1)] = okr ? __ldg(rowp + xr) : 0u;
         if constexpr (S % 4 == 0) {
 #pragma unroll
           for (int q = 0; q < S / 4; ++q) {
-            const uint32_t v = ok ? __ldg(reinterpret_cast<const uint32_t *>(arow + ox + 4 * q)) : 0u;
-            ad[32 * (1 + 4 * q)] = (uint8_t)v; ad[32 * (2 + 4 * q)] = (uint8_t)(v >> 8);
-            ad[32 * (3 + 4 * q)] = (uint8_t)(v >> 16); ad[32 * (4 + 4 * q)] = (uint8_t)(v >> 24);
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (ok) v = __ldg(reinterpret_cast<const uint4 *>(rowp + ox + 4 * q));
+            dst[32 * (1 + 4 * q)] = v.x; dst[32 * (2 + 4 * q)] = v.y; dst[32 * (3 + 4 * q)] = v.z; dst[32 * (4 + 4 * q)] = v.w;
           }
         } else {
-          const uint32_t v = ok ? (uint32_t)__ldg(reinterpret_cast<const unsigned short *>(arow + ox)) : 0u;
-          ad[32] = (uint8_t)v; ad[64] = (uint8_t)(v >> 8);
+          uint2 v = make_uint2(0u, 0u);
+          if (ok) v = __ldg(reinterpret_cast<const uint2 *>(rowp + ox));
+          dst[32] = v.x; dst[64] = v.y;
+        }
+        if constexpr (ACT) {
+          const uint8_t *arow = P.act + P.apitch * rowi;
+          uint8_t *ad = atile + 32 * ((tz * T + ty) * T);
+          ad[0] = okl ? __ldg(arow + xl) : (uint8_t)0;
+          ad[32 * (S + 1)] = okr ? __ldg(arow + xr) : (uint8_t)0;
+          if constexpr (S % 4 == 0) {
+#pragma unroll
+            for (int q = 0; q < S / 4; ++q) {
+              const uint32_t v = ok ? __ldg(reinterpret_cast<const uint32_t *>(arow + ox + 4 * q)) : 0u;
+              ad[32 * (1 + 4 * q)] = (uint8_t)v; ad[32 * (2 + 4 * q)] = (uint8_t)(v >> 8);
+              ad[32 * (3 + 4 * q)] = (uint8_t)(v >> 16); ad[32 * (4 + 4 * q)] = (uint8_t)(v >> 24);
+            }
+          } else {
+            const uint32_t v = ok ? (uint32_t)__ldg(reinterpret_cast<const unsigned short *>(arow + ox)) : 0u;
+            ad[32] = (uint8_t)v; ad[64] = (uint8_t)(v >> 8);
+          }
         }
       }
     }
@@ -160,33 +181,46 @@ struct ThreadSweep {
     }
   }
 
-  // ---- a6: per-cell {V,P} as this attempt sees it ----
+  // ---- a6: own deltas of this activation ----
+  __device__ __forceinline__ int find(uint32_t cell) const {
+    int e = -1;
+#pragma unroll
+    for (int i = 0; i < TK_REG; ++i)
+      if (rk[i] == cell) e = i;
+    if (e < 0 && n_entries > TK_REG)
+      for (int i = TK_REG; i < n_entries; ++i)
+        if (key[i] == cell) { e = i; break; }
+    return e;
+  }
+  // per-cell {V,P} as this attempt sees it: snapshot + own deltas (deterministic) / live value
   __device__ __forceinline__ unsigned long long view(uint32_t cell, unsigned long long base) const {
     if constexpr (LIVE) {
       return base;
     } else {
-      for (int e = 0; e < n_entries; ++e)
-        if (key[e] == cell) return base + dvp[e];
-      return base;
+      if (n_entries == 0) return base;
+      const int e = find(cell);
+      return e >= 0 ? base + dvp[e] : base;
     }
   }
   __device__ __forceinline__ void add_delta(uint32_t cell, int dV, int dP, int x, int y, int z, int sgn) {
     const unsigned long long d = ((unsigned long long)(long long)dV << 32) + (unsigned long long)(long long)dP;
-    if (LIVE) {
+    if constexpr (LIVE) {
       atomicAdd(P.liveVP + cell, d);
       atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
       atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
       if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
-      return;
+    } else {
+      int e = find(cell);
+      if (e < 0) {
+        if (n_entries == TK_CAP) { overflow = true; return; }
+        e = n_entries++;
+#pragma unroll
+        for (int i = 0; i < TK_REG; ++i)
+          if (i == e) rk[i] = cell;
+        key[e] = cell; dvp[e] = 0ull; dsx[e] = 0; dsy[e] = 0; dsz[e] = 0;
+      }
+      dvp[e] += d; dsx[e] += sgn * x; dsy[e] += sgn * y; dsz[e] += sgn * z;
     }
-    int e = 0;
-    while (e < n_entries && key[e] != cell) ++e;
-    if (e == n_entries) {
-      if (n_entries == TK_CAP) { overflow = true; return; }
-      key[e] = cell; dvp[e] = 0ull; dsx[e] = 0; dsy[e] = 0; dsz[e] = 0;
-      ++n_entries;
-    }
-    dvp[e] += d; dsx[e] += sgn * x; dsy[e] += sgn * y; dsz[e] += sgn * z;
   }
   __device__ __forceinline__ void flush_table() {
     if constexpr (!LIVE) {
@@ -201,65 +235,60 @@ struct ThreadSweep {
   }
 
   // ---- Act: fixed-point geometric mean over {x} + same-cell Moore neighbours (Eq 9, reading S8) ----
-  __device__ __forceinline__ int gm_finish(int ssum, int n, bool zero) const {
-    if (zero) return 0;
-    const int m = ssum / n;
-    return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
-  }
-  // centre inside the subsection: the whole neighbourhood is in the tile
-  __device__ __forceinline__ int gm_inner(int c32, uint32_t mC) const {
-    int a = atile[c32];
-    bool zero = (a == 0);
-    int ssum = __ldg(P.logq16 + a), n = 1;
-#pragma unroll
-    for (int nb = 0; nb < NNB; ++nb) {
-      const int o = off32(nbc_dx<DIM>(nb), nbc_dy<DIM>(nb), nbc_dz<DIM>(nb));
-      if ((tile[c32 + o] & CELL_MASK) == mC) {
-        a = atile[c32 + o];
-        zero |= (a == 0);
-        ssum += __ldg(P.logq16 + a);
-        ++n;
-      }
-    }
-    return gm_finish(ssum, n, zero);
-  }
-  // centre in the halo: neighbours outside the tile are read from global memory
-  __device__ int gm_outer(int cx, int cy, int cz, uint32_t mC) const {   // tile coordinates in [0, T)
-    const int c32 = 32 * ((cz * T + cy) * T + cx);
-    int a = atile[c32];
-    bool zero = (a == 0);
-    int ssum = __ldg(P.logq16 + a), n = 1;
-#pragma unroll 1
-    for (int nb = 0; nb < NNB; ++nb) {
-      int dx, dy, dz;
-      nb_delta<DIM>(nb, dx, dy, dz);
-      const int px = cx + dx, py = cy + dy, pz = cz + dz;
-      uint32_t w; int av;
+  // Computed by the whole warp for the subsection of lane L: lane n < NNB takes neighbour n of the
+  // centre c = (cx, cy, cz) (tile coordinates), lane NNB the centre itself.  Sites outside the halo-1
+  // tile (ring 2 around the subsection) are read from global memory.  Warp-uniform arguments.
+  __device__ __forceinline__ int gm_coop(int L, int c, uint32_t mC, int oxL, int oyL, int ozL) const {
+    const bool part = lane <= NNB;
+    const int code = sNbr[part ? lane : NNB];
+    const int px = (c & 255) + (code & 3) - 1, py = ((c >> 8) & 255) + ((code >> 2) & 3) - 1;
+    const int pz = (DIM == 3) ? ((c >> 16) & 255) + ((code >> 4) & 3) - 1 : 0;
+    uint32_t w = 0u;
+    int av = 0;
+    bool have = false;
+    if (part) {
       const bool in = px >= 0 && px < T && py >= 0 && py < T && (DIM == 2 || (pz >= 0 && pz < T));
       if (in) {
-        const int p32 = 32 * ((pz * T + py) * T + px);
-        w = tile[p32]; av = atile[p32];
+        const int idx = 32 * ((pz * T + py) * T + px) + L;
+        w = (tile - lane)[idx]; av = (atile - lane)[idx];
+        have = true;
       } else {
-        int gx = ox - 1 + px, gy = oy - 1 + py, gz = (DIM == 3) ? oz - 1 + pz : 0;
+        int gx = oxL - 1 + px, gy = oyL - 1 + py, gz = (DIM == 3) ? ozL - 1 + pz : 0;
         bool ok = wrap(gx, P.X, P.per[0]);
         ok = wrap(gy, P.Y, P.per[1]) && ok;
         if (DIM == 3) ok = wrap(gz, P.Z, P.per[2]) && ok;
-        if (!ok) continue;   // outside a closed lattice: medium, never the same cell
-        const long long rowi = (long long)gy + (long long)P.Y * gz;
-        w = __ldg(P.lat + P.pitch * rowi + gx);
-        av = __ldg(P.act + P.apitch * rowi + gx);
+        if (ok) {   // outside a closed lattice: medium, never the same cell
+          const long long rowi = (long long)gy + (long long)P.Y * gz;
+          w = __ldg(P.lat + P.pitch * rowi + gx);
+          av = __ldg(P.act + P.apitch * rowi + gx);
+          have = true;
+        }
       }
-      if ((w & CELL_MASK) == mC) { zero |= (av == 0); ssum += __ldg(P.logq16 + av); ++n; }
     }
-    return gm_finish(ssum, n, zero);
+    const bool same = have && (lane == NNB || (w & CELL_MASK) == mC);
+    const unsigned msame = __ballot_sync(FULL, same);
+    const unsigned mzero = __ballot_sync(FULL, same && av == 0);
+    const int ssum = __reduce_add_sync(FULL, same ? sLog[av] : 0);
+    if (mzero) return 0;
+    const int m = ssum / __popc(msame);
+    return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
   }
 
-  // ---- a5-a9: one evaluated copy attempt; l = site index, nb = neighbour index, a = attempt index ----
-  __device__ __forceinline__ bool evaluate(int t32, int s32, int l, int nb, int a) {
-    const uint32_t wA = tile[s32], wB = tile[t32];
+  // ---- a5-a7 for this lane's attempt: census of t, per-cell state, dH without the Act term ----
+  struct Eval {
+    int t32, s32, l, nb, a;
+    uint32_t wA, mA, mB;
+    long long dH;
+    int dPA, dPB;
+    int lamA_a, maxA_a, lamA_b, maxA_b;   // Act parameters of the source / target cell's type
+    bool go;                              // false: refused before Metropolis (reading S13)
+  };
+  __device__ __forceinline__ void census(Eval &e) {
+    const uint32_t wA = tile[e.s32], wB = tile[e.t32];
     const uint32_t A = wA & ID_MASK, B = wB & ID_MASK;
     const uint32_t mA = wA & CELL_MASK, mB = wB & CELL_MASK;
     const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
+    e.wA = wA; e.mA = mA; e.mB = mB;
     // per-cell state: issue the loads first, they are consumed after the census
     unsigned long long baseA = 0ull, baseB = 0ull;
     if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
@@ -270,7 +299,7 @@ struct ThreadSweep {
     int nA = 0, nB = 0, adh = 0;
 #pragma unroll
     for (int n = 0; n < NNB; ++n) {
-      const uint32_t m = tile[t32 + off32(nbc_dx<DIM>(n), nbc_dy<DIM>(n), nbc_dz<DIM>(n))] & CELL_MASK;
+      const uint32_t m = tile[e.t32 + off32(nbc_dx<DIM>(n), nbc_dy<DIM>(n), nbc_dz<DIM>(n))] & CELL_MASK;
       nA += (m == mA);
       nB += (m == mB);
       adh += Drow[m >> 24];
@@ -281,7 +310,7 @@ struct ThreadSweep {
 
     const unsigned long long vpA = (A != 0) ? view(A, baseA) : 0ull;
     const unsigned long long vpB = (B != 0) ? view(B, baseB) : 0ull;
-    if (B != 0 && (uint32_t)(vpB >> 32) <= 1u) return false;   // a cell is never erased (reading S13)
+    e.go = !(B != 0 && (uint32_t)(vpB >> 32) <= 1u);   // a cell is never erased (reading S13)
 
     const int rA = (A != 0) ? tA : P.nT, rB = (B != 0) ? tB : P.nT;   // medium reads the all-zero row (S3)
     const TypeParams pa = sT[rA], pb = sT[rB];
@@ -292,46 +321,42 @@ struct ThreadSweep {
       const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
       dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
     }
-    int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
-    if constexpr (ACT) {
-      if ((pa.lamA | pb.lamA) != 0) {   // lamA is stored as 0 when the type's Max_act is 0
-        long long sideA = 0, sideB = 0;
-        if (pa.lamA != 0) {
-          int dx, dy, dz;
-          nb_delta<DIM>(nb, dx, dy, dz);
-          const int sx = lx + dx, sy = ly + dy, sz = lz + dz;
-          const bool inner = sx >= 0 && sx < S && sy >= 0 && sy < S && (DIM == 2 || (sz >= 0 && sz < S));
-          const int g = inner ? gm_inner(s32, mA) : gm_outer(sx + 1, sy + 1, (DIM == 3) ? sz + 1 : 0, mA);
-          if (g != 0) sideA = ((long long)pa.lamA * g) / pa.maxA;
-        }
-        if (pb.lamA != 0) {
-          const int g = gm_inner(t32, mB);
-          if (g != 0) sideB = ((long long)pb.lamA * g) / pb.maxA;
-        }
-        dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
-      }
-    }
+    e.dH = dH; e.dPA = dPA; e.dPB = dPB;
+    e.lamA_a = pa.lamA; e.maxA_a = pa.maxA; e.lamA_b = pb.lamA; e.maxA_b = pb.maxA;
+  }
 
-    // a8: Metropolis (Eq 2) against the integer threshold table; the word comes from stream 1
+  // ---- a8-a9: Metropolis and commit; returns true if the copy was made ----
+  __device__ __forceinline__ bool decide(const Eval &e) {
+    const long long dH = e.dH;
     if (dH > 0 && !P.accept_all) {
       if (dH > P.Hmax) return false;
-      const uint4 ua = philox4x32_10(make_uint4((uint32_t)a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
-      if (pick(ua, a & 3) >= __ldg(P.thr + dH)) return false;
+      const uint4 ua = philox4x32_10(make_uint4((uint32_t)e.a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
+      if (pick(ua, e.a & 3) >= __ldg(P.thr + dH)) return false;
     }
-
-    // a9: commit
-    tile[t32] = wA;
-    if constexpr (ACT) atile[t32] = (uint8_t)pa.maxA;   // Max_act of the new owner; 0 for medium
+    tile[e.t32] = e.wA;
+    if constexpr (ACT) atile[e.t32] = (uint8_t)e.maxA_a;   // Max_act of the new owner; 0 for medium
     dirty = true;
+    const int l = e.l;
+    const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
     const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
-    if (A != 0) add_delta(A, 1, dPA, gx, gy, gz, +1);
-    if (B != 0) add_delta(B, -1, dPB, gx, gy, gz, -1);
+    const uint32_t A = e.mA & ID_MASK, B = e.mB & ID_MASK;
+    if (A != 0) add_delta(A, 1, e.dPA, gx, gy, gz, +1);
+    if (B != 0) add_delta(B, -1, e.dPB, gx, gy, gz, -1);
     return true;
   }
 
+  // screen one proposal against the current tile (a4): true = it needs a dH
+  __device__ __forceinline__ bool interesting(int prop) const {
+    const int t32 = site32(prop & 255);
+    const uint32_t wt = tile[t32], ws = tile[t32 + sOff[prop >> 8]];
+    return (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
+  }
+
   // ---- the whole activation of this lane's subsection ----
-  __device__ void run(bool active, unsigned long long w, int lane) {
+  __device__ void run(bool active, unsigned long long w) {
     n_entries = 0; dirty = false; overflow = false;
+#pragma unroll
+    for (int i = 0; i < TK_REG; ++i) rk[i] = 0xFFFFFFFFu;
     mcs = *P.mcs_ptr;
     ox = oy = oz = 0; b = 0;
     if (active) {
@@ -345,33 +370,76 @@ struct ThreadSweep {
       load_tile();
     }
     const int k = active ? P.k : 0;
-    int a = 0, rq = -1;
-    uint4 r = make_uint4(0u, 0u, 0u, 0u);
+    const int nq = (k + 3) >> 2;     // quads of this activation
+    int q = 0;                       // next quad to draw
+    unsigned mask = 0u;              // attempts of the current quad (bit j) that still need a dH
+    int prop[4] = {0, 0, 0, 0};      // l | nb << 8 of the current quad
     uint32_t n_eval = 0, n_acc = 0;
     while (true) {
-      bool found = false;
-      int t32 = 0, s32 = 0, l = 0, nb = 0;
-      int budget = SCREEN_BUDGET;
-      while (a < k && budget > 0) {
-        if ((a >> 2) != rq) {
-          rq = a >> 2;
-          r = philox4x32_10(make_uint4((uint32_t)rq, b, 2u * P.p, mcs), P.key0, P.key1);
+      // step 1: lanes without a pending attempt draw and screen their next quad
+      if (mask == 0u && q < nq) {
+        const uint4 r = philox4x32_10(make_uint4((uint32_t)q, b, 2u * P.p, mcs), P.key0, P.key1);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t wd = pick(r, j);
+          const int l = (int)(wd >> (32 - G::LOG2SITES));                          // = (wd * S^d) >> 32
+          const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
+          prop[j] = l | (nb << 8);
+          if (4 * q + j < k && interesting(prop[j])) mask |= 1u << j;
         }
-        const uint32_t wd = pick(r, a & 3);
-        l = (int)(wd >> (32 - G::LOG2SITES));                     // = (wd * S^d) >> 32
-        nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);    // = (u32(wd * S^d) * nNb) >> 32
-        const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
-        t32 = 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1);
-        s32 = t32 + sOff[nb];
-        const uint32_t wt = tile[t32], ws = tile[s32];
-        if ((((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0)) { found = true; break; }
-        ++a; --budget;
+        ++q;
       }
-      if (!__any_sync(FULL, a < k)) break;
-      if (found) {
+      if (!__any_sync(FULL, mask != 0u || q < nq)) break;
+
+      // step 2: lanes with a pending attempt evaluate the first one
+      const bool ev = mask != 0u;
+      Eval e;
+      e.go = false; e.lamA_a = 0; e.lamA_b = 0; e.maxA_a = 0; e.maxA_b = 0; e.mA = 0u; e.mB = 0u; e.l = 0; e.nb = 0;
+      int j = 0;
+      if (ev) {
+        j = __ffs(mask) - 1;
+        const int pj = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
+        e.l = pj & 255; e.nb = pj >> 8;
+        e.t32 = site32(e.l); e.s32 = e.t32 + sOff[e.nb];
+        e.a = 4 * (q - 1) + j;
         ++n_eval;
-        if (evaluate(t32, s32, l, nb, a)) ++n_acc;
-        ++a;
+        census(e);
+      }
+      if constexpr (ACT) {
+        // geometric means for the lanes whose source / target cell has an Act bias, by the whole warp
+        const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
+        const int code = sNbr[e.nb];
+        const int ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
+        const int cs = (lx + (code & 3)) | ((ly + ((code >> 2) & 3)) << 8) | ((DIM == 3 ? lz + ((code >> 4) & 3) : 1) << 16);
+        unsigned needA = __ballot_sync(FULL, ev && e.go && e.lamA_a != 0);
+        unsigned needB = __ballot_sync(FULL, ev && e.go && e.lamA_b != 0);
+        long long sideA = 0, sideB = 0;
+        while (needA | needB) {
+          const bool isA = needA != 0u;
+          const int L = __ffs(isA ? needA : needB) - 1;
+          if (isA) needA &= needA - 1; else needB &= needB - 1;
+          const int c = __shfl_sync(FULL, isA ? cs : ct, L);
+          const uint32_t mC = __shfl_sync(FULL, isA ? e.mA : e.mB, L);
+          const int oxL = __shfl_sync(FULL, ox, L), oyL = __shfl_sync(FULL, oy, L), ozL = __shfl_sync(FULL, oz, L);
+          const int g = gm_coop(L, c, mC, oxL, oyL, ozL);
+          if (lane == L && g != 0) {
+            if (isA) sideA = ((long long)e.lamA_a * g) / e.maxA_a;
+            else sideB = ((long long)e.lamA_b * g) / e.maxA_b;
+          }
+        }
+        if ((e.lamA_a | e.lamA_b) != 0) e.dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
+      }
+      if (ev) {
+        mask &= mask - 1u;                 // attempt j is done
+        if (e.go && decide(e)) {
+          ++n_acc;
+          // later attempts of the quad see the new tile: screen them again
+          unsigned m2 = 0u;
+#pragma unroll
+          for (int jj = 1; jj < 4; ++jj)
+            if (jj > j && 4 * (q - 1) + jj < k && interesting(prop[jj])) m2 |= 1u << jj;
+          mask = m2;
+        }
       }
     }
     if (dirty) store_tile();
@@ -389,7 +457,8 @@ struct ThreadSweep {
 };
 
 // One warp per CTA, one lane per active subsection.  Dynamic smem: [id tiles: WORDS x 32 words]
-// [Act tiles: WORDS x 32 bytes] [neighbour offsets: 32 ints] [type records: nT+1] [D: nT^3, then J(t,t): nT].
+// [Act tiles: WORDS x 32 bytes] [neighbour offsets: 32 ints] [neighbour codes: 32 ints]
+// [type records: nT+1] [D: nT^3, then J(t,t): nT] [Act log table: 256 ints, with Act only].
 template <int DIM, int S, bool ACT, bool LIVE>
 __global__ void __launch_bounds__(32) sweep_thread_kernel(const __grid_constant__ SweepParams P) {
   extern __shared__ __align__(128) unsigned char smem[];
@@ -399,23 +468,28 @@ __global__ void __launch_bounds__(32) sweep_thread_kernel(const __grid_constant_
   uint8_t *atiles = smem + (size_t)G::WORDS * 128;
   unsigned char *tabs = atiles + (ACT ? (size_t)G::WORDS * 32 : 0);
   int *sOff = reinterpret_cast<int *>(tabs);
-  TypeParams *sT = reinterpret_cast<TypeParams *>(tabs + 128);
-  int32_t *sD = reinterpret_cast<int32_t *>(tabs + 128 + (size_t)(P.nT + 1) * sizeof(TypeParams));
+  int *sNbr = sOff + 32;
+  TypeParams *sT = reinterpret_cast<TypeParams *>(tabs + 256);
+  int32_t *sD = reinterpret_cast<int32_t *>(tabs + 256 + (size_t)(P.nT + 1) * sizeof(TypeParams));
+  const int nD = P.nT * P.nT * P.nT + P.nT;
+  int32_t *sLog = sD + nD;
   {
     int dx = 0, dy = 0, dz = 0;
     if (lane < G::NNB) nb_delta<DIM>(lane, dx, dy, dz);
     sOff[lane] = 32 * ((dz * G::T + dy) * G::T + dx);
+    sNbr[lane] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
     for (int i = lane; i < (P.nT + 1) * 8; i += 32)
       reinterpret_cast<int32_t *>(sT)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-    const int nD = P.nT * P.nT * P.nT + P.nT;
     for (int i = lane; i < nD; i += 32) sD[i] = P.D[i];
+    if constexpr (ACT)
+      for (int i = lane; i < 256; i += 32) sLog[i] = P.logq16[i];
   }
   __syncwarp();
   const unsigned long long w = (unsigned long long)blockIdx.x * 32 + lane;
   ThreadSweep<DIM, S, ACT, LIVE> sw(P);
-  sw.tile = tiles + lane; sw.atile = atiles + lane;
-  sw.sOff = sOff; sw.sD = sD; sw.sDiag = sD + P.nT * P.nT * P.nT; sw.sT = sT;
-  sw.run(w < P.n_active, w, lane);
+  sw.tile = tiles + lane; sw.atile = atiles + lane; sw.lane = lane;
+  sw.sOff = sOff; sw.sNbr = sNbr; sw.sD = sD; sw.sDiag = sD + P.nT * P.nT * P.nT; sw.sT = sT; sw.sLog = sLog;
+  sw.run(w < P.n_active, w);
 }
 
 }  // namespace cpm

@@ -297,8 +297,8 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     size_t words = 1;
     for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
     c->wpc = 1;
-    c->cta_smem = words * 128 + (c->act_enabled ? words * 32 : 0) + 256 + (size_t)(nT + 1) * sizeof(TypeParams) +
-                  ((size_t)nT * nT * nT + nT) * 4 + (c->act_enabled ? 1024 : 0);
+    c->cta_smem = words * 128 + (c->act_enabled ? words * 32 + 1024 : 0) + 256 + 9 * sizeof(TypeParams) +
+                  ((size_t)nT * nT * nT + nT) * 4;
   }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 

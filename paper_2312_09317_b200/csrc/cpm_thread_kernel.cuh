@@ -50,6 +50,14 @@ __host__ __device__ constexpr int nbc_dy(int nb) { return ((nb + (nb >= ((DIM ==
 template <int DIM>
 __host__ __device__ constexpr int nbc_dz(int nb) { return (DIM == 3) ? (nb + (nb >= 13 ? 1 : 0)) / 9 - 1 : 0; }
 
+// dynamically indexed part of the own-delta table: kept apart from ThreadSweep so that everything
+// else in there stays in registers
+struct OwnTable {
+  uint32_t key[TK_CAP];
+  unsigned long long dvp[TK_CAP];
+  int dsx[TK_CAP], dsy[TK_CAP], dsz[TK_CAP];
+};
+
 template <int DIM, int S, bool ACT, bool LIVE>
 struct ThreadSweep {
   using G = TGeom<DIM, S>;
@@ -58,14 +66,25 @@ struct ThreadSweep {
   static constexpr uint32_t CELL_MASK = 0x7FFFFFFFu;   // type + id: equal iff same cell
 
   const SweepParams &P;
-  uint32_t *tile;          // this lane's word 0; word j at tile[32 * j]
-  uint8_t *atile;          // this lane's Act byte 0; byte j at atile[32 * j]
-  const int *sOff;         // neighbour index -> 32 * tile offset
-  const int *sNbr;         // neighbour index -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
-  const int32_t *sD;       // [nT][nT][nT] adhesion difference table
-  const int32_t *sDiag;    // [nT] J(t,t)
-  const TypeParams *sT;    // [nT + 1], row nT all zero (medium)
-  const int32_t *sLog;     // [256] Q16 log2 (Act)
+  // Shared-memory layout of the (one-warp) CTA, all offsets compile-time so that every access is a
+  // plain LDS/STS: [id tiles: WORDS x 32 words][Act tiles: WORDS x 32 bytes][neighbour offsets: 32
+  // ints][neighbour codes: 32 ints][Act log table: 256 ints][type records: 9][D: nT^3, then J(t,t): nT]
+  static constexpr int OFF_ACT = G::WORDS * 128;
+  static constexpr int OFF_TAB = OFF_ACT + (ACT ? G::WORDS * 32 : 0);
+  static constexpr int OFF_LOG = OFF_TAB + 256;
+  static constexpr int OFF_TYPES = OFF_LOG + (ACT ? 1024 : 0);
+  static constexpr int OFF_D = OFF_TYPES + 9 * (int)sizeof(TypeParams);
+  static __device__ __forceinline__ unsigned char *sm() { extern __shared__ __align__(128) unsigned char smem[]; return smem; }
+  static __device__ __forceinline__ uint32_t *tl0() { return reinterpret_cast<uint32_t *>(sm()); }            // lane 0's tile
+  static __device__ __forceinline__ uint32_t *tl() { return tl0() + threadIdx.x; }      // this lane's word j at [32 * j]
+  static __device__ __forceinline__ uint8_t *al0() { return sm() + OFF_ACT; }
+  static __device__ __forceinline__ uint8_t *al() { return al0() + threadIdx.x; }       // this lane's Act byte j at [32 * j]
+  static __device__ __forceinline__ int *so() { return reinterpret_cast<int *>(sm() + OFF_TAB); }             // nbr -> 32 * tile offset
+  static __device__ __forceinline__ int *sn() { return so() + 32; }   // nbr -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
+  static __device__ __forceinline__ int32_t *slog() { return reinterpret_cast<int32_t *>(sm() + OFF_LOG); }   // [256] Q16 log2 (Act)
+  static __device__ __forceinline__ TypeParams *st() { return reinterpret_cast<TypeParams *>(sm() + OFF_TYPES); }   // [nT + 1], row nT zero
+  static __device__ __forceinline__ int32_t *sd() { return reinterpret_cast<int32_t *>(sm() + OFF_D); }       // [nT][nT][nT] adhesion differences
+  __device__ __forceinline__ const int32_t *sdiag() const { return sd() + P.nT * P.nT * P.nT; }                // [nT] J(t,t)
   int lane;
   int ox, oy, oz;
   uint32_t b;
@@ -73,13 +92,11 @@ struct ThreadSweep {
   // own deltas of this activation (deterministic mode): the first TK_REG keys in registers, the
   // rest and all values in local memory
   uint32_t rk[TK_REG];
-  uint32_t key[TK_CAP];
-  unsigned long long dvp[TK_CAP];
-  int dsx[TK_CAP], dsy[TK_CAP], dsz[TK_CAP];
+  OwnTable &tb;
   int n_entries;
   bool dirty, overflow;
 
-  __device__ ThreadSweep(const SweepParams &p) : P(p) {}
+  __device__ __forceinline__ ThreadSweep(const SweepParams &p, OwnTable &t) : P(p), tb(t) {}
 
   static __device__ __forceinline__ int off32(int dx, int dy, int dz) { return 32 * ((dz * T + dy) * T + dx); }
   static __device__ __forceinline__ int site32(int l) {   // site index -> 32 * tile offset
@@ -113,7 +130,7 @@ struct ThreadSweep {
         if (ty == 0 || ty == T - 1) ok = wrap(gy, P.Y, P.per[1]) && ok;
         const long long rowi = zrow + gy;
         const uint32_t *rowp = P.lat + P.pitch * rowi;
-        uint32_t *dst = tile + 32 * ((tz * T + ty) * T);
+        uint32_t *dst = tl() + 32 * ((tz * T + ty) * T);
         const bool okl = ok && okxl, okr = ok && okxr;
         dst[0] = okl ? __ldg(rowp + xl) : 0u;
         dst[32 * (S + 1)] = okr ? __ldg(rowp + xr) : 0u;
@@ -131,7 +148,7 @@ struct ThreadSweep {
         }
         if constexpr (ACT) {
           const uint8_t *arow = P.act + P.apitch * rowi;
-          uint8_t *ad = atile + 32 * ((tz * T + ty) * T);
+          uint8_t *ad = al() + 32 * ((tz * T + ty) * T);
           ad[0] = okl ? __ldg(arow + xl) : (uint8_t)0;
           ad[32 * (S + 1)] = okr ? __ldg(arow + xr) : (uint8_t)0;
           if constexpr (S % 4 == 0) {
@@ -158,7 +175,7 @@ struct ThreadSweep {
       const int ly = r % S, lz = r / S;
       const long long rowi = (long long)(oy + ly) + (long long)P.Y * ((DIM == 3) ? oz + lz : 0);
       uint32_t *rowp = P.lat + P.pitch * rowi + ox;
-      const uint32_t *src = tile + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
+      const uint32_t *src = tl() + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
       if constexpr (S % 4 == 0) {
 #pragma unroll
         for (int q = 0; q < S / 4; ++q)
@@ -168,7 +185,7 @@ struct ThreadSweep {
       }
       if constexpr (ACT) {
         uint8_t *arow = P.act + P.apitch * rowi + ox;
-        const uint8_t *as = atile + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
+        const uint8_t *as = al() + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
         if constexpr (S % 4 == 0) {
 #pragma unroll
           for (int q = 0; q < S / 4; ++q)
@@ -189,7 +206,7 @@ struct ThreadSweep {
       if (rk[i] == cell) e = i;
     if (e < 0 && n_entries > TK_REG)
       for (int i = TK_REG; i < n_entries; ++i)
-        if (key[i] == cell) { e = i; break; }
+        if (tb.key[i] == cell) { e = i; break; }
     return e;
   }
   // per-cell {V,P} as this attempt sees it: snapshot + own deltas (deterministic) / live value
@@ -199,7 +216,7 @@ struct ThreadSweep {
     } else {
       if (n_entries == 0) return base;
       const int e = find(cell);
-      return e >= 0 ? base + dvp[e] : base;
+      return e >= 0 ? base + tb.dvp[e] : base;
     }
   }
   __device__ __forceinline__ void add_delta(uint32_t cell, int dV, int dP, int x, int y, int z, int sgn) {
@@ -217,19 +234,19 @@ struct ThreadSweep {
 #pragma unroll
         for (int i = 0; i < TK_REG; ++i)
           if (i == e) rk[i] = cell;
-        key[e] = cell; dvp[e] = 0ull; dsx[e] = 0; dsy[e] = 0; dsz[e] = 0;
+        tb.key[e] = cell; tb.dvp[e] = 0ull; tb.dsx[e] = 0; tb.dsy[e] = 0; tb.dsz[e] = 0;
       }
-      dvp[e] += d; dsx[e] += sgn * x; dsy[e] += sgn * y; dsz[e] += sgn * z;
+      tb.dvp[e] += d; tb.dsx[e] += sgn * x; tb.dsy[e] += sgn * y; tb.dsz[e] += sgn * z;
     }
   }
   __device__ __forceinline__ void flush_table() {
     if constexpr (!LIVE) {
       for (int e = 0; e < n_entries; ++e) {
-        const uint32_t c = key[e];
-        if (dvp[e] != 0ull) atomicAdd(P.liveVP + c, dvp[e]);
-        if (dsx[e] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)dsx[e]);
-        if (dsy[e] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)dsy[e]);
-        if (DIM == 3 && dsz[e] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)dsz[e]);
+        const uint32_t c = tb.key[e];
+        if (tb.dvp[e] != 0ull) atomicAdd(P.liveVP + c, tb.dvp[e]);
+        if (tb.dsx[e] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)tb.dsx[e]);
+        if (tb.dsy[e] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)tb.dsy[e]);
+        if (DIM == 3 && tb.dsz[e] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)tb.dsz[e]);
       }
     }
   }
@@ -240,7 +257,7 @@ struct ThreadSweep {
   // tile (ring 2 around the subsection) are read from global memory.  Warp-uniform arguments.
   __device__ __forceinline__ int gm_coop(int L, int c, uint32_t mC, int oxL, int oyL, int ozL) const {
     const bool part = lane <= NNB;
-    const int code = sNbr[part ? lane : NNB];
+    const int code = sn()[part ? lane : NNB];
     const int px = (c & 255) + (code & 3) - 1, py = ((c >> 8) & 255) + ((code >> 2) & 3) - 1;
     const int pz = (DIM == 3) ? ((c >> 16) & 255) + ((code >> 4) & 3) - 1 : 0;
     uint32_t w = 0u;
@@ -250,7 +267,7 @@ struct ThreadSweep {
       const bool in = px >= 0 && px < T && py >= 0 && py < T && (DIM == 2 || (pz >= 0 && pz < T));
       if (in) {
         const int idx = 32 * ((pz * T + py) * T + px) + L;
-        w = (tile - lane)[idx]; av = (atile - lane)[idx];
+        w = tl0()[idx]; av = al0()[idx];
         have = true;
       } else {
         int gx = oxL - 1 + px, gy = oyL - 1 + py, gz = (DIM == 3) ? ozL - 1 + pz : 0;
@@ -268,7 +285,7 @@ struct ThreadSweep {
     const bool same = have && (lane == NNB || (w & CELL_MASK) == mC);
     const unsigned msame = __ballot_sync(FULL, same);
     const unsigned mzero = __ballot_sync(FULL, same && av == 0);
-    const int ssum = __reduce_add_sync(FULL, same ? sLog[av] : 0);
+    const int ssum = __reduce_add_sync(FULL, same ? slog()[av] : 0);
     if (mzero) return 0;
     const int m = ssum / __popc(msame);
     return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
@@ -284,7 +301,7 @@ struct ThreadSweep {
     bool go;                              // false: refused before Metropolis (reading S13)
   };
   __device__ __forceinline__ void census(Eval &e) {
-    const uint32_t wA = tile[e.s32], wB = tile[e.t32];
+    const uint32_t wA = tl()[e.s32], wB = tl()[e.t32];
     const uint32_t A = wA & ID_MASK, B = wB & ID_MASK;
     const uint32_t mA = wA & CELL_MASK, mB = wB & CELL_MASK;
     const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
@@ -295,17 +312,17 @@ struct ThreadSweep {
     if (B != 0) baseB = LIVE ? __ldcg(P.liveVP + B) : __ldg(P.snapVP + B);
 
     // neighbour census of t: n_A, n_B and sum_n [J(tA,tn) - J(tB,tn)]
-    const int32_t *Drow = sD + (tA * P.nT + tB) * P.nT;
+    const int32_t *Drow = sd() + (tA * P.nT + tB) * P.nT;
     int nA = 0, nB = 0, adh = 0;
 #pragma unroll
     for (int n = 0; n < NNB; ++n) {
-      const uint32_t m = tile[e.t32 + off32(nbc_dx<DIM>(n), nbc_dy<DIM>(n), nbc_dz<DIM>(n))] & CELL_MASK;
+      const uint32_t m = tl()[e.t32 + off32(nbc_dx<DIM>(n), nbc_dy<DIM>(n), nbc_dz<DIM>(n))] & CELL_MASK;
       nA += (m == mA);
       nB += (m == mB);
       adh += Drow[m >> 24];
     }
     // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
-    adh += nB * sDiag[tB] - nA * sDiag[tA];
+    adh += nB * sdiag()[tB] - nA * sdiag()[tA];
     long long dH = adh;
 
     const unsigned long long vpA = (A != 0) ? view(A, baseA) : 0ull;
@@ -313,7 +330,7 @@ struct ThreadSweep {
     e.go = !(B != 0 && (uint32_t)(vpB >> 32) <= 1u);   // a cell is never erased (reading S13)
 
     const int rA = (A != 0) ? tA : P.nT, rB = (B != 0) ? tB : P.nT;   // medium reads the all-zero row (S3)
-    const TypeParams pa = sT[rA], pb = sT[rB];
+    const TypeParams pa = st()[rA], pb = st()[rB];
     const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
     {
       const int dva = (int)(uint32_t)(vpA >> 32) - pa.tgtV, dvb = (int)(uint32_t)(vpB >> 32) - pb.tgtV;
@@ -333,8 +350,8 @@ struct ThreadSweep {
       const uint4 ua = philox4x32_10(make_uint4((uint32_t)e.a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
       if (pick(ua, e.a & 3) >= __ldg(P.thr + dH)) return false;
     }
-    tile[e.t32] = e.wA;
-    if constexpr (ACT) atile[e.t32] = (uint8_t)e.maxA_a;   // Max_act of the new owner; 0 for medium
+    tl()[e.t32] = e.wA;
+    if constexpr (ACT) al()[e.t32] = (uint8_t)e.maxA_a;   // Max_act of the new owner; 0 for medium
     dirty = true;
     const int l = e.l;
     const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
@@ -348,12 +365,12 @@ struct ThreadSweep {
   // screen one proposal against the current tile (a4): true = it needs a dH
   __device__ __forceinline__ bool interesting(int prop) const {
     const int t32 = site32(prop & 255);
-    const uint32_t wt = tile[t32], ws = tile[t32 + sOff[prop >> 8]];
+    const uint32_t wt = tl()[t32], ws = tl()[t32 + so()[prop >> 8]];
     return (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
   }
 
   // ---- the whole activation of this lane's subsection ----
-  __device__ void run(bool active, unsigned long long w) {
+  __device__ __forceinline__ void run(bool active, unsigned long long w) {
     n_entries = 0; dirty = false; overflow = false;
 #pragma unroll
     for (int i = 0; i < TK_REG; ++i) rk[i] = 0xFFFFFFFFu;
@@ -400,7 +417,7 @@ struct ThreadSweep {
         j = __ffs(mask) - 1;
         const int pj = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
         e.l = pj & 255; e.nb = pj >> 8;
-        e.t32 = site32(e.l); e.s32 = e.t32 + sOff[e.nb];
+        e.t32 = site32(e.l); e.s32 = e.t32 + so()[e.nb];
         e.a = 4 * (q - 1) + j;
         ++n_eval;
         census(e);
@@ -408,7 +425,7 @@ struct ThreadSweep {
       if constexpr (ACT) {
         // geometric means for the lanes whose source / target cell has an Act bias, by the whole warp
         const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
-        const int code = sNbr[e.nb];
+        const int code = sn()[e.nb];
         const int ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
         const int cs = (lx + (code & 3)) | ((ly + ((code >> 2) & 3)) << 8) | ((DIM == 3 ? lz + ((code >> 4) & 3) : 1) << 16);
         unsigned needA = __ballot_sync(FULL, ev && e.go && e.lamA_a != 0);
@@ -456,39 +473,29 @@ struct ThreadSweep {
   }
 };
 
-// One warp per CTA, one lane per active subsection.  Dynamic smem: [id tiles: WORDS x 32 words]
-// [Act tiles: WORDS x 32 bytes] [neighbour offsets: 32 ints] [neighbour codes: 32 ints]
-// [type records: nT+1] [D: nT^3, then J(t,t): nT] [Act log table: 256 ints, with Act only].
+// One warp per CTA, one lane per active subsection; dynamic smem laid out as in ThreadSweep.
 template <int DIM, int S, bool ACT, bool LIVE>
 __global__ void __launch_bounds__(32) sweep_thread_kernel(const __grid_constant__ SweepParams P) {
-  extern __shared__ __align__(128) unsigned char smem[];
+  using TS = ThreadSweep<DIM, S, ACT, LIVE>;
   using G = TGeom<DIM, S>;
   const int lane = threadIdx.x;
-  uint32_t *tiles = reinterpret_cast<uint32_t *>(smem);
-  uint8_t *atiles = smem + (size_t)G::WORDS * 128;
-  unsigned char *tabs = atiles + (ACT ? (size_t)G::WORDS * 32 : 0);
-  int *sOff = reinterpret_cast<int *>(tabs);
-  int *sNbr = sOff + 32;
-  TypeParams *sT = reinterpret_cast<TypeParams *>(tabs + 256);
-  int32_t *sD = reinterpret_cast<int32_t *>(tabs + 256 + (size_t)(P.nT + 1) * sizeof(TypeParams));
-  const int nD = P.nT * P.nT * P.nT + P.nT;
-  int32_t *sLog = sD + nD;
   {
     int dx = 0, dy = 0, dz = 0;
     if (lane < G::NNB) nb_delta<DIM>(lane, dx, dy, dz);
-    sOff[lane] = 32 * ((dz * G::T + dy) * G::T + dx);
-    sNbr[lane] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
+    TS::so()[lane] = 32 * ((dz * G::T + dy) * G::T + dx);
+    TS::sn()[lane] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
     for (int i = lane; i < (P.nT + 1) * 8; i += 32)
-      reinterpret_cast<int32_t *>(sT)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-    for (int i = lane; i < nD; i += 32) sD[i] = P.D[i];
+      reinterpret_cast<int32_t *>(TS::st())[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+    const int nD = P.nT * P.nT * P.nT + P.nT;
+    for (int i = lane; i < nD; i += 32) TS::sd()[i] = P.D[i];
     if constexpr (ACT)
-      for (int i = lane; i < 256; i += 32) sLog[i] = P.logq16[i];
+      for (int i = lane; i < 256; i += 32) TS::slog()[i] = P.logq16[i];
   }
   __syncwarp();
   const unsigned long long w = (unsigned long long)blockIdx.x * 32 + lane;
-  ThreadSweep<DIM, S, ACT, LIVE> sw(P);
-  sw.tile = tiles + lane; sw.atile = atiles + lane; sw.lane = lane;
-  sw.sOff = sOff; sw.sNbr = sNbr; sw.sD = sD; sw.sDiag = sD + P.nT * P.nT * P.nT; sw.sT = sT; sw.sLog = sLog;
+  OwnTable tab;
+  TS sw(P, tab);
+  sw.lane = lane;
   sw.run(w < P.n_active, w);
 }
 

@@ -17,7 +17,8 @@
 //       are drawn only for uphill moves inside the table range;
 //   Act the geometric means (Eq 9) are needed by few lanes at a time, so they are computed by the
 //       WHOLE warp for one lane after the other (lanes = the 27 sites, ballot / REDUX);
-//   a10 dirty interiors are written back with 128-bit stores, own deltas flushed with 64-bit atomics.
+//   a10 dirty interiors are written back with 128-bit stores; the integer deltas of every accepted
+//       copy go out at once as 64-bit reductions (RED) on the live per-cell arrays.
 // With Act the tile keeps halo 1; the geometric mean around a source that lies in the halo reads the
 // few voxels of ring 2 straight from global memory (they belong to inactive subsections, so they are
 // stable during the phase-step).
@@ -55,7 +56,6 @@ __host__ __device__ constexpr int nbc_dz(int nb) { return (DIM == 3) ? (nb + (nb
 struct OwnTable {
   uint32_t key[TK_CAP];
   unsigned long long dvp[TK_CAP];
-  int dsx[TK_CAP], dsy[TK_CAP], dsz[TK_CAP];
 };
 
 template <int DIM, int S, bool ACT, bool LIVE>
@@ -89,9 +89,10 @@ struct ThreadSweep {
   int ox, oy, oz;
   uint32_t b;
   uint32_t mcs;
-  // own deltas of this activation (deterministic mode): the first TK_REG keys in registers, the
-  // rest and all values in local memory
+  // own deltas of this activation (deterministic mode): cell -> composite {dV, dP}; the first TK_REG
+  // entries in registers, the rest in local memory
   uint32_t rk[TK_REG];
+  unsigned long long rdv[TK_REG];
   OwnTable &tb;
   int n_entries;
   bool dirty, overflow;
@@ -117,18 +118,28 @@ struct ThreadSweep {
     const bool okxl = wrap(xl, P.X, P.per[0]);
     const bool okxr = wrap(xr, P.X, P.per[0]);
     constexpr int TZ = (DIM == 3) ? T : 1;
+    // row offsets (in rows) of the T tile rows / planes under the boundary rule; only the first and
+    // the last can fall outside the lattice
+    long long yo[T], zo[TZ];
+    bool yok[T], zok[TZ];
+#pragma unroll
+    for (int ty = 0; ty < T; ++ty) {
+      int gy = oy - 1 + ty;
+      yok[ty] = (ty == 0 || ty == T - 1) ? wrap(gy, P.Y, P.per[1]) : true;
+      yo[ty] = gy;
+    }
 #pragma unroll
     for (int tz = 0; tz < TZ; ++tz) {
       int gz = (DIM == 3) ? oz - 1 + tz : 0;
-      bool okz = true;
-      if (DIM == 3 && (tz == 0 || tz == T - 1)) okz = wrap(gz, P.Z, P.per[2]);   // interior planes are inside
-      const long long zrow = (long long)P.Y * gz;
+      zok[tz] = (DIM == 3 && (tz == 0 || tz == T - 1)) ? wrap(gz, P.Z, P.per[2]) : true;
+      zo[tz] = (long long)P.Y * gz;
+    }
+#pragma unroll
+    for (int tz = 0; tz < TZ; ++tz) {
 #pragma unroll
       for (int ty = 0; ty < T; ++ty) {
-        int gy = oy - 1 + ty;
-        bool ok = okz;
-        if (ty == 0 || ty == T - 1) ok = wrap(gy, P.Y, P.per[1]) && ok;
-        const long long rowi = zrow + gy;
+        const bool ok = zok[tz] && yok[ty];
+        const long long rowi = zo[tz] + yo[ty];
         const uint32_t *rowp = P.lat + P.pitch * rowi;
         uint32_t *dst = tl() + 32 * ((tz * T + ty) * T);
         const bool okl = ok && okxl, okr = ok && okxr;
@@ -198,55 +209,47 @@ struct ThreadSweep {
     }
   }
 
-  // ---- a6: own deltas of this activation ----
-  __device__ __forceinline__ int find(uint32_t cell) const {
-    int e = -1;
-#pragma unroll
-    for (int i = 0; i < TK_REG; ++i)
-      if (rk[i] == cell) e = i;
-    if (e < 0 && n_entries > TK_REG)
-      for (int i = TK_REG; i < n_entries; ++i)
-        if (tb.key[i] == cell) { e = i; break; }
-    return e;
-  }
-  // per-cell {V,P} as this attempt sees it: snapshot + own deltas (deterministic) / live value
+  // ---- a6: per-cell {V,P} as this attempt sees it: snapshot + own deltas (deterministic) / live ----
   __device__ __forceinline__ unsigned long long view(uint32_t cell, unsigned long long base) const {
     if constexpr (LIVE) {
       return base;
     } else {
-      if (n_entries == 0) return base;
-      const int e = find(cell);
-      return e >= 0 ? base + tb.dvp[e] : base;
+      unsigned long long d = 0ull;
+#pragma unroll
+      for (int i = 0; i < TK_REG; ++i)
+        if (rk[i] == cell) d = rdv[i];
+      if (n_entries > TK_REG)
+        for (int i = TK_REG; i < n_entries; ++i)
+          if (tb.key[i] == cell) { d = tb.dvp[i]; break; }
+      return base + d;
     }
   }
+  // a9/a10: the integer deltas of an accepted copy go to the live per-cell arrays at once (fire-and-forget
+  // reductions; nobody reads them before the next phase-step in deterministic mode) and, in
+  // deterministic mode, into this lane's own-delta table
   __device__ __forceinline__ void add_delta(uint32_t cell, int dV, int dP, int x, int y, int z, int sgn) {
     const unsigned long long d = ((unsigned long long)(long long)dV << 32) + (unsigned long long)(long long)dP;
-    if constexpr (LIVE) {
-      atomicAdd(P.liveVP + cell, d);
-      atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
-      atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
-      if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
-    } else {
-      int e = find(cell);
-      if (e < 0) {
-        if (n_entries == TK_CAP) { overflow = true; return; }
-        e = n_entries++;
-#pragma unroll
-        for (int i = 0; i < TK_REG; ++i)
-          if (i == e) rk[i] = cell;
-        tb.key[e] = cell; tb.dvp[e] = 0ull; tb.dsx[e] = 0; tb.dsy[e] = 0; tb.dsz[e] = 0;
-      }
-      tb.dvp[e] += d; tb.dsx[e] += sgn * x; tb.dsy[e] += sgn * y; tb.dsz[e] += sgn * z;
-    }
-  }
-  __device__ __forceinline__ void flush_table() {
+    atomicAdd(P.liveVP + cell, d);
+    atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
+    atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
+    if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
     if constexpr (!LIVE) {
-      for (int e = 0; e < n_entries; ++e) {
-        const uint32_t c = tb.key[e];
-        if (tb.dvp[e] != 0ull) atomicAdd(P.liveVP + c, tb.dvp[e]);
-        if (tb.dsx[e] != 0) atomicAdd(P.sumx + c, (unsigned long long)(long long)tb.dsx[e]);
-        if (tb.dsy[e] != 0) atomicAdd(P.sumy + c, (unsigned long long)(long long)tb.dsy[e]);
-        if (DIM == 3 && tb.dsz[e] != 0) atomicAdd(P.sumz + c, (unsigned long long)(long long)tb.dsz[e]);
+      bool hit = false;
+#pragma unroll
+      for (int i = 0; i < TK_REG; ++i)
+        if (rk[i] == cell) { rdv[i] += d; hit = true; }
+      if (!hit) {
+        for (int i = TK_REG; i < n_entries; ++i)
+          if (tb.key[i] == cell) { tb.dvp[i] += d; hit = true; break; }
+        if (!hit) {
+          const int e = n_entries;
+          if (e == TK_CAP) { overflow = true; return; }
+#pragma unroll
+          for (int i = 0; i < TK_REG; ++i)
+            if (i == e) { rk[i] = cell; rdv[i] = d; }
+          if (e >= TK_REG) { tb.key[e] = cell; tb.dvp[e] = d; }
+          n_entries = e + 1;
+        }
       }
     }
   }
@@ -373,7 +376,7 @@ struct ThreadSweep {
   __device__ __forceinline__ void run(bool active, unsigned long long w) {
     n_entries = 0; dirty = false; overflow = false;
 #pragma unroll
-    for (int i = 0; i < TK_REG; ++i) rk[i] = 0xFFFFFFFFu;
+    for (int i = 0; i < TK_REG; ++i) { rk[i] = 0xFFFFFFFFu; rdv[i] = 0ull; }
     mcs = *P.mcs_ptr;
     ox = oy = oz = 0; b = 0;
     if (active) {
@@ -460,7 +463,6 @@ struct ThreadSweep {
       }
     }
     if (dirty) store_tile();
-    flush_table();
     n_eval = __reduce_add_sync(FULL, n_eval);
     n_acc = __reduce_add_sync(FULL, n_acc);
     const bool any_over = __any_sync(FULL, overflow);

@@ -296,9 +296,8 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     // one warp per CTA: interleaved (S+2)^d id tiles (+ Act bytes) of 32 lanes, then the small tables
     size_t words = 1;
     for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
-    c->wpc = 1;
-    c->cta_smem = words * 128 + (c->act_enabled ? words * 32 + 1024 : 0) + 256 + 9 * sizeof(TypeParams) +
-                  ((size_t)nT * nT * nT + nT) * 4;
+    c->wpc = TK_WARPS;
+    c->cta_smem = (size_t)TK_WARPS * words * 128 + 256 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
   }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
@@ -485,7 +484,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
         }
         if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
         sp.n_active = n_active;
-        const unsigned long long per_cta = c->thread_kernel ? 32ull : (unsigned long long)c->wpc;
+        const unsigned long long per_cta = c->thread_kernel ? 32ull * TK_WARPS : (unsigned long long)c->wpc;
         const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
         if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
         cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -494,7 +493,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
           e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
           CK(cudaEventRecord(e0, c->stream));
         }
-        if (c->thread_kernel) c->tfn<<<(unsigned)grid, 32, c->cta_smem, c->stream>>>(sp);
+        if (c->thread_kernel) c->tfn<<<(unsigned)grid, 32 * TK_WARPS, c->cta_smem, c->stream>>>(sp);
         else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
         if (c->timing) CK(cudaEventRecord(e1, c->stream));
         c->launches++; c->sweep_launches++;

@@ -19,9 +19,10 @@
 //       WHOLE warp for one lane after the other (lanes = the 27 sites, ballot / REDUX);
 //   a10 dirty interiors are written back with 128-bit stores; the integer deltas of every accepted
 //       copy go out at once as 64-bit reductions (RED) on the live per-cell arrays.
-// With Act the tile keeps halo 1; the geometric mean around a source that lies in the halo reads the
-// few voxels of ring 2 straight from global memory (they belong to inactive subsections, so they are
-// stable during the phase-step).
+// The Act bytes are not staged: the geometric means read them from global memory (L2) and accepted
+// copies store Max_act there directly.  The id tile keeps halo 1; the geometric mean around a source
+// that lies in the halo reads the few ids of ring 2 from global memory too (they belong to inactive
+// subsections, so they are stable during the phase-step).
 // Nothing here is shared with oracle/.
 #pragma once
 #include "cpm_device.cuh"
@@ -30,6 +31,7 @@ namespace cpm {
 
 constexpr int TK_CAP = 32;          // own-delta entries per thread (cells changed in one activation)
 constexpr int TK_REG = 8;           // of which the first keys are held in registers
+constexpr int TK_WARPS = 2;         // warps per CTA: 4 CTAs of 2 x 27 KB tiles fill the 228 KB of an SM (3D, S = 4)
 
 template <int DIM, int S>
 struct TGeom {
@@ -66,22 +68,21 @@ struct ThreadSweep {
   static constexpr uint32_t CELL_MASK = 0x7FFFFFFFu;   // type + id: equal iff same cell
 
   const SweepParams &P;
-  // Shared-memory layout of the (one-warp) CTA, all offsets compile-time so that every access is a
-  // plain LDS/STS: [id tiles: WORDS x 32 words][Act tiles: WORDS x 32 bytes][neighbour offsets: 32
-  // ints][neighbour codes: 32 ints][Act log table: 256 ints][type records: 9][D: nT^3, then J(t,t): nT]
-  static constexpr int OFF_ACT = G::WORDS * 128;
-  static constexpr int OFF_TAB = OFF_ACT + (ACT ? G::WORDS * 32 : 0);
-  static constexpr int OFF_LOG = OFF_TAB + 256;
-  static constexpr int OFF_TYPES = OFF_LOG + (ACT ? 1024 : 0);
+  // Shared-memory layout of the CTA (TK_WARPS warps), all offsets compile-time so that every access is a
+  // plain LDS/STS: [id tiles: TK_WARPS x WORDS x 32 words][neighbour offsets: 32 ints][neighbour codes: 32
+  // ints][type records: 9][D: nT^3, then J(t,t): nT].  The Act field is NOT staged: it is read by the
+  // geometric means only (a few lanes per round) and written by accepted copies only, straight in
+  // global memory, which leaves room for two more warps per SM.
+  static constexpr int OFF_TAB = TK_WARPS * G::WORDS * 128;
+  static constexpr int OFF_TYPES = OFF_TAB + 256;
   static constexpr int OFF_D = OFF_TYPES + 9 * (int)sizeof(TypeParams);
   static __device__ __forceinline__ unsigned char *sm() { extern __shared__ __align__(128) unsigned char smem[]; return smem; }
-  static __device__ __forceinline__ uint32_t *tl0() { return reinterpret_cast<uint32_t *>(sm()); }            // lane 0's tile
-  static __device__ __forceinline__ uint32_t *tl() { return tl0() + threadIdx.x; }      // this lane's word j at [32 * j]
-  static __device__ __forceinline__ uint8_t *al0() { return sm() + OFF_ACT; }
-  static __device__ __forceinline__ uint8_t *al() { return al0() + threadIdx.x; }       // this lane's Act byte j at [32 * j]
+  static __device__ __forceinline__ uint32_t *tl0() {   // tile of lane 0 of this warp
+    return reinterpret_cast<uint32_t *>(sm()) + (threadIdx.x >> 5) * (G::WORDS * 32);
+  }
+  static __device__ __forceinline__ uint32_t *tl() { return tl0() + (threadIdx.x & 31); }   // this lane's word j at [32 * j]
   static __device__ __forceinline__ int *so() { return reinterpret_cast<int *>(sm() + OFF_TAB); }             // nbr -> 32 * tile offset
   static __device__ __forceinline__ int *sn() { return so() + 32; }   // nbr -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
-  static __device__ __forceinline__ int32_t *slog() { return reinterpret_cast<int32_t *>(sm() + OFF_LOG); }   // [256] Q16 log2 (Act)
   static __device__ __forceinline__ TypeParams *st() { return reinterpret_cast<TypeParams *>(sm() + OFF_TYPES); }   // [nT + 1], row nT zero
   static __device__ __forceinline__ int32_t *sd() { return reinterpret_cast<int32_t *>(sm() + OFF_D); }       // [nT][nT][nT] adhesion differences
   __device__ __forceinline__ const int32_t *sdiag() const { return sd() + P.nT * P.nT * P.nT; }                // [nT] J(t,t)
@@ -157,23 +158,6 @@ struct ThreadSweep {
           if (ok) v = __ldg(reinterpret_cast<const uint2 *>(rowp + ox));
           dst[32] = v.x; dst[64] = v.y;
         }
-        if constexpr (ACT) {
-          const uint8_t *arow = P.act + P.apitch * rowi;
-          uint8_t *ad = al() + 32 * ((tz * T + ty) * T);
-          ad[0] = okl ? __ldg(arow + xl) : (uint8_t)0;
-          ad[32 * (S + 1)] = okr ? __ldg(arow + xr) : (uint8_t)0;
-          if constexpr (S % 4 == 0) {
-#pragma unroll
-            for (int q = 0; q < S / 4; ++q) {
-              const uint32_t v = ok ? __ldg(reinterpret_cast<const uint32_t *>(arow + ox + 4 * q)) : 0u;
-              ad[32 * (1 + 4 * q)] = (uint8_t)v; ad[32 * (2 + 4 * q)] = (uint8_t)(v >> 8);
-              ad[32 * (3 + 4 * q)] = (uint8_t)(v >> 16); ad[32 * (4 + 4 * q)] = (uint8_t)(v >> 24);
-            }
-          } else {
-            const uint32_t v = ok ? (uint32_t)__ldg(reinterpret_cast<const unsigned short *>(arow + ox)) : 0u;
-            ad[32] = (uint8_t)v; ad[64] = (uint8_t)(v >> 8);
-          }
-        }
       }
     }
   }
@@ -193,18 +177,6 @@ struct ThreadSweep {
           *reinterpret_cast<uint4 *>(rowp + 4 * q) = make_uint4(src[32 * (4 * q)], src[32 * (4 * q + 1)], src[32 * (4 * q + 2)], src[32 * (4 * q + 3)]);
       } else {
         *reinterpret_cast<uint2 *>(rowp) = make_uint2(src[0], src[32]);
-      }
-      if constexpr (ACT) {
-        uint8_t *arow = P.act + P.apitch * rowi + ox;
-        const uint8_t *as = al() + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
-        if constexpr (S % 4 == 0) {
-#pragma unroll
-          for (int q = 0; q < S / 4; ++q)
-            *reinterpret_cast<uint32_t *>(arow + 4 * q) = (uint32_t)as[32 * (4 * q)] | ((uint32_t)as[32 * (4 * q + 1)] << 8) |
-                                                         ((uint32_t)as[32 * (4 * q + 2)] << 16) | ((uint32_t)as[32 * (4 * q + 3)] << 24);
-        } else {
-          *reinterpret_cast<unsigned short *>(arow) = (unsigned short)((uint32_t)as[0] | ((uint32_t)as[32] << 8));
-        }
       }
     }
   }
@@ -264,31 +236,26 @@ struct ThreadSweep {
     const int px = (c & 255) + (code & 3) - 1, py = ((c >> 8) & 255) + ((code >> 2) & 3) - 1;
     const int pz = (DIM == 3) ? ((c >> 16) & 255) + ((code >> 4) & 3) - 1 : 0;
     uint32_t w = 0u;
-    int av = 0;
+    int av = 1;
     bool have = false;
+    long long gidx = 0;
     if (part) {
       const bool in = px >= 0 && px < T && py >= 0 && py < T && (DIM == 2 || (pz >= 0 && pz < T));
-      if (in) {
-        const int idx = 32 * ((pz * T + py) * T + px) + L;
-        w = tl0()[idx]; av = al0()[idx];
-        have = true;
-      } else {
-        int gx = oxL - 1 + px, gy = oyL - 1 + py, gz = (DIM == 3) ? ozL - 1 + pz : 0;
-        bool ok = wrap(gx, P.X, P.per[0]);
-        ok = wrap(gy, P.Y, P.per[1]) && ok;
-        if (DIM == 3) ok = wrap(gz, P.Z, P.per[2]) && ok;
-        if (ok) {   // outside a closed lattice: medium, never the same cell
-          const long long rowi = (long long)gy + (long long)P.Y * gz;
-          w = __ldg(P.lat + P.pitch * rowi + gx);
-          av = __ldg(P.act + P.apitch * rowi + gx);
-          have = true;
-        }
-      }
+      int gx = oxL - 1 + px, gy = oyL - 1 + py, gz = (DIM == 3) ? ozL - 1 + pz : 0;
+      bool ok = wrap(gx, P.X, P.per[0]);
+      ok = wrap(gy, P.Y, P.per[1]) && ok;
+      if (DIM == 3) ok = wrap(gz, P.Z, P.per[2]) && ok;
+      const long long rowi = (long long)gy + (long long)P.Y * gz;
+      gidx = P.apitch * rowi + gx;
+      if (in) w = tl0()[32 * ((pz * T + py) * T + px) + L];
+      else if (ok) w = __ldg(P.lat + P.pitch * rowi + gx);
+      have = ok;   // outside a closed lattice: medium, never the same cell
     }
     const bool same = have && (lane == NNB || (w & CELL_MASK) == mC);
+    if (same) av = __ldcg(P.act + gidx);   // L2: sees the Act bytes this warp stored on earlier commits
     const unsigned msame = __ballot_sync(FULL, same);
     const unsigned mzero = __ballot_sync(FULL, same && av == 0);
-    const int ssum = __reduce_add_sync(FULL, same ? slog()[av] : 0);
+    const int ssum = __reduce_add_sync(FULL, same ? __ldg(P.logq16 + av) : 0);
     if (mzero) return 0;
     const int m = ssum / __popc(msame);
     return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
@@ -354,11 +321,12 @@ struct ThreadSweep {
       if (pick(ua, e.a & 3) >= __ldg(P.thr + dH)) return false;
     }
     tl()[e.t32] = e.wA;
-    if constexpr (ACT) al()[e.t32] = (uint8_t)e.maxA_a;   // Max_act of the new owner; 0 for medium
     dirty = true;
     const int l = e.l;
     const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
     const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
+    if constexpr (ACT)   // Max_act of the new owner; 0 for medium
+      P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)e.maxA_a;
     const uint32_t A = e.mA & ID_MASK, B = e.mB & ID_MASK;
     if (A != 0) add_delta(A, 1, e.dPA, gx, gy, gz, +1);
     if (B != 0) add_delta(B, -1, e.dPB, gx, gy, gz, -1);
@@ -426,7 +394,9 @@ struct ThreadSweep {
         census(e);
       }
       if constexpr (ACT) {
-        // geometric means for the lanes whose source / target cell has an Act bias, by the whole warp
+        // geometric means for the lanes whose source / target cell has an Act bias, by the whole warp;
+        // the Act bytes stored by earlier commits of any lane must be visible to all lanes
+        __syncwarp();
         const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
         const int code = sn()[e.nb];
         const int ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
@@ -467,7 +437,7 @@ struct ThreadSweep {
     n_acc = __reduce_add_sync(FULL, n_acc);
     const bool any_over = __any_sync(FULL, overflow);
     if (lane == 0) {
-      const int slot = (int)(blockIdx.x % COUNTER_SLOTS);
+      const int slot = (int)((blockIdx.x * TK_WARPS + (threadIdx.x >> 5)) % COUNTER_SLOTS);
       if (n_eval) atomicAdd(P.counters + 2 * slot, (unsigned long long)n_eval);
       if (n_acc) atomicAdd(P.counters + 2 * slot + 1, (unsigned long long)n_acc);
       if (any_over) atomicOr(P.error_flag, 1);
@@ -475,29 +445,28 @@ struct ThreadSweep {
   }
 };
 
-// One warp per CTA, one lane per active subsection; dynamic smem laid out as in ThreadSweep.
+// TK_WARPS warps per CTA (they share only the small tables), one lane per active subsection; dynamic
+// smem laid out as in ThreadSweep.
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(32) sweep_thread_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(32 * TK_WARPS) sweep_thread_kernel(const __grid_constant__ SweepParams P) {
   using TS = ThreadSweep<DIM, S, ACT, LIVE>;
   using G = TGeom<DIM, S>;
-  const int lane = threadIdx.x;
-  {
+  const int tid = threadIdx.x;
+  if (tid < 32) {
     int dx = 0, dy = 0, dz = 0;
-    if (lane < G::NNB) nb_delta<DIM>(lane, dx, dy, dz);
-    TS::so()[lane] = 32 * ((dz * G::T + dy) * G::T + dx);
-    TS::sn()[lane] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
-    for (int i = lane; i < (P.nT + 1) * 8; i += 32)
-      reinterpret_cast<int32_t *>(TS::st())[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-    const int nD = P.nT * P.nT * P.nT + P.nT;
-    for (int i = lane; i < nD; i += 32) TS::sd()[i] = P.D[i];
-    if constexpr (ACT)
-      for (int i = lane; i < 256; i += 32) TS::slog()[i] = P.logq16[i];
+    if (tid < G::NNB) nb_delta<DIM>(tid, dx, dy, dz);
+    TS::so()[tid] = 32 * ((dz * G::T + dy) * G::T + dx);
+    TS::sn()[tid] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
   }
-  __syncwarp();
-  const unsigned long long w = (unsigned long long)blockIdx.x * 32 + lane;
+  for (int i = tid; i < (P.nT + 1) * 8; i += 32 * TK_WARPS)
+    reinterpret_cast<int32_t *>(TS::st())[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+  const int nD = P.nT * P.nT * P.nT + P.nT;
+  for (int i = tid; i < nD; i += 32 * TK_WARPS) TS::sd()[i] = P.D[i];
+  __syncthreads();
+  const unsigned long long w = (unsigned long long)blockIdx.x * (32 * TK_WARPS) + tid;
   OwnTable tab;
   TS sw(P, tab);
-  sw.lane = lane;
+  sw.lane = tid & 31;
   sw.run(w < P.n_active, w);
 }
 

@@ -31,6 +31,7 @@ namespace cpm {
 
 constexpr int TK_CAP = 32;          // own-delta entries per thread (cells changed in one activation)
 constexpr int TK_REG = 8;           // of which the first keys are held in registers
+constexpr int GM_BATCH = 2;          // Act geometric means computed per batch (their global loads overlap)
 constexpr int TK_WARPS = 2;         // warps per CTA: 4 CTAs of 2 x 27 KB tiles fill the 228 KB of an SM (3D, S = 4)
 
 template <int DIM, int S>
@@ -230,7 +231,8 @@ struct ThreadSweep {
   // Computed by the whole warp for the subsection of lane L: lane n < NNB takes neighbour n of the
   // centre c = (cx, cy, cz) (tile coordinates), lane NNB the centre itself.  Sites outside the halo-1
   // tile (ring 2 around the subsection) are read from global memory.  Warp-uniform arguments.
-  __device__ __forceinline__ int gm_coop(int L, int c, uint32_t mC, int oxL, int oyL, int ozL) const {
+  // gm_site: this lane's site of the neighbourhood -> (same cell?, Act value); gm_value: the reduction.
+  __device__ __forceinline__ bool gm_site(int L, int c, uint32_t mC, int oxL, int oyL, int ozL, int &av_out) const {
     const bool part = lane <= NNB;
     const int code = sn()[part ? lane : NNB];
     const int px = (c & 255) + (code & 3) - 1, py = ((c >> 8) & 255) + ((code >> 2) & 3) - 1;
@@ -253,6 +255,10 @@ struct ThreadSweep {
     }
     const bool same = have && (lane == NNB || (w & CELL_MASK) == mC);
     if (same) av = __ldcg(P.act + gidx);   // L2: sees the Act bytes this warp stored on earlier commits
+    av_out = av;
+    return same;
+  }
+  __device__ __forceinline__ int gm_value(bool same, int av) const {
     const unsigned msame = __ballot_sync(FULL, same);
     const unsigned mzero = __ballot_sync(FULL, same && av == 0);
     const int ssum = __reduce_add_sync(FULL, same ? __ldg(P.logq16 + av) : 0);
@@ -405,16 +411,31 @@ struct ThreadSweep {
         unsigned needB = __ballot_sync(FULL, ev && e.go && e.lamA_b != 0);
         long long sideA = 0, sideB = 0;
         while (needA | needB) {
-          const bool isA = needA != 0u;
-          const int L = __ffs(isA ? needA : needB) - 1;
-          if (isA) needA &= needA - 1; else needB &= needB - 1;
-          const int c = __shfl_sync(FULL, isA ? cs : ct, L);
-          const uint32_t mC = __shfl_sync(FULL, isA ? e.mA : e.mB, L);
-          const int oxL = __shfl_sync(FULL, ox, L), oyL = __shfl_sync(FULL, oy, L), ozL = __shfl_sync(FULL, oz, L);
-          const int g = gm_coop(L, c, mC, oxL, oyL, ozL);
-          if (lane == L && g != 0) {
-            if (isA) sideA = ((long long)e.lamA_a * g) / e.maxA_a;
-            else sideB = ((long long)e.lamA_b * g) / e.maxA_b;
+          // up to GM_BATCH neighbourhoods at a time: all their global Act loads are in flight together
+          int Ls[GM_BATCH], av[GM_BATCH];
+          bool isAs[GM_BATCH], same[GM_BATCH];
+#pragma unroll
+          for (int i = 0; i < GM_BATCH; ++i) {
+            Ls[i] = -1; isAs[i] = false; same[i] = false; av[i] = 1;
+            if (needA | needB) {
+              isAs[i] = needA != 0u;
+              Ls[i] = __ffs(isAs[i] ? needA : needB) - 1;
+              if (isAs[i]) needA &= needA - 1; else needB &= needB - 1;
+              const int c = __shfl_sync(FULL, isAs[i] ? cs : ct, Ls[i]);
+              const uint32_t mC = __shfl_sync(FULL, isAs[i] ? e.mA : e.mB, Ls[i]);
+              const int oxL = __shfl_sync(FULL, ox, Ls[i]), oyL = __shfl_sync(FULL, oy, Ls[i]), ozL = __shfl_sync(FULL, oz, Ls[i]);
+              same[i] = gm_site(Ls[i], c, mC, oxL, oyL, ozL, av[i]);
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < GM_BATCH; ++i) {
+            if (Ls[i] >= 0) {
+              const int g = gm_value(same[i], av[i]);
+              if (lane == Ls[i] && g != 0) {
+                if (isAs[i]) sideA = ((long long)e.lamA_a * g) / e.maxA_a;
+                else sideB = ((long long)e.lamA_b * g) / e.maxA_b;
+              }
+            }
           }
         }
         if ((e.lamA_a | e.lamA_b) != 0) e.dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)

@@ -30,7 +30,7 @@
 namespace cpm {
 
 constexpr int TK_CAP = 32;          // own-delta entries per thread (cells changed in one activation)
-constexpr int TK_REG = 8;           // of which the first keys are held in registers
+constexpr int TK_REG = 4;           // of which the first keys are held in registers
 constexpr int GM_BATCH = 2;          // Act geometric means computed per batch (their global loads overlap)
 constexpr int TK_WARPS = 2;         // warps per CTA: 4 CTAs of 2 x 27 KB tiles fill the 228 KB of an SM (3D, S = 4)
 

@@ -293,11 +293,11 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
   c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
   if (c->thread_kernel) {
-    // one warp per CTA: interleaved (S+2)^d id tiles (+ Act bytes) of 32 lanes, then the small tables
+    // TK_WARPS warps per CTA, each with the interleaved (S+2)^d id tiles of its TK_CH subsections, then the small tables
     size_t words = 1;
     for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
     c->wpc = TK_WARPS;
-    c->cta_smem = (size_t)TK_WARPS * words * 128 + 256 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
+    c->cta_smem = (size_t)TK_WARPS * words * TK_CH * 4 + 256 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
   }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
@@ -484,7 +484,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
         }
         if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
         sp.n_active = n_active;
-        const unsigned long long per_cta = c->thread_kernel ? 32ull * TK_WARPS : (unsigned long long)c->wpc;
+        const unsigned long long per_cta = c->thread_kernel ? (unsigned long long)(TK_CH * TK_WARPS) : (unsigned long long)c->wpc;
         const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
         if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
         cudaEvent_t e0 = nullptr, e1 = nullptr;

@@ -1,38 +1,45 @@
-// cpm_thread_kernel.cuh -- sm_100a sweep kernel with one THREAD per active checkerboard subsection
-// (the paper's own granularity: "a 4x4 area per thread", Fig 4; thread = local simulation, L47).
+// cpm_thread_kernel.cuh -- sm_100a sweep kernel with one lane PAIR per active checkerboard subsection
+// (the paper's own granularity: "a 4x4 area per thread", Fig 4; one local simulation per
+// worker, L47).
 //
 // Used for small power-of-two subsections (3D S = 2, 4; 2D S = 2..16).  Same algorithm, same RNG
-// counters and same results as the warp-per-subsection kernel of cpm_device.cuh:
-//   a2  every lane stages its own (S+2)^d tile into shared memory, INTERLEAVED across the 32 lanes of
-//       the warp (word j of lane L at [j][L]): every later shared-memory access of a warp is
-//       bank-conflict free whatever sites the lanes picked; global loads are 128-bit for the interior
-//       of a row plus the two halo words;
-//   a3  Philox4x32-10, one call = four consecutive attempts ("quad") of this lane's subsection;
-//   a4  the warp works in rounds.  Step 1 (converged): every lane without a pending attempt draws its
-//       next quad and screens its four proposals against its tile (same cell / frozen) -> 4-bit mask;
-//   a5-a9 step 2 (converged): every lane with a pending attempt evaluates the first one, serially over
-//       its 26 (8) neighbours: n_A, n_B by compares, adhesion through the difference table
-//       D[tA][tB][tn] = J(tA,tn) - J(tB,tn); after an accepted copy the rest of the quad is re-screened,
-//       so the result is exactly that of k sequential attempts; acceptance words (Philox stream 1)
-//       are drawn only for uphill moves inside the table range;
-//   Act the geometric means (Eq 9) are needed by few lanes at a time, so they are computed by the
-//       WHOLE warp for one lane after the other (lanes = the 27 sites, ballot / REDUX);
+// counters and same results as the warp-per-subsection kernel of cpm_device.cuh.
+// The attempts of a subsection are a sequential chain, so the time of a phase-step is set by how many
+// chains an SM holds (shared memory) and by the latency of one link; two lanes per chain halve the
+// work on that critical path and leave room for twice as many warps:
+//   a2  the pair stages the (S+2)^d tile of its subsection (rows split by parity), INTERLEAVED across
+//       the 16 subsections of the warp (word j of subsection c at [j][c]); global loads are 128-bit for
+//       the interior of a row plus the two halo words;
+//   a3  Philox4x32-10, one call = four consecutive attempts; each lane of the pair draws one call, so a
+//       draw covers eight consecutive attempts ("oct");
+//   a4  the warp works in rounds.  Step 1 (converged): every pair without a pending attempt draws its
+//       next oct and screens the eight proposals against its tile (same cell / frozen) -> 8-bit mask;
+//   a5-a9 step 2 (converged): every pair with a pending attempt evaluates the first one: each lane
+//       visits 13 (4) of the 26 (8) neighbours -- n_A, n_B by compares, adhesion through the difference
+//       table D[tA][tB][tn] = J(tA,tn) - J(tB,tn) -- and a shuffle adds the halves; dH, Metropolis and
+//       the own-delta table are computed by both lanes alike, memory is written by the even lane; after
+//       an accepted copy the rest of the oct is re-screened, so the result is exactly that of k
+//       sequential attempts; acceptance words (Philox stream 1) are drawn only for uphill moves inside
+//       the table range;
+//   Act the geometric means (Eq 9) are needed by few pairs at a time, so they are computed by the
+//       WHOLE warp for one pair after the other (lanes = the 27 sites, ballot / REDUX).  The Act bytes
+//       are not staged: the geometric means read them from global memory (L2) and accepted copies
+//       store Max_act there directly.  The id tile keeps halo 1; the few ids of ring 2 around a source
+//       that lies in the halo are read from global memory too (they belong to inactive subsections, so
+//       they are stable during the phase-step);
 //   a10 dirty interiors are written back with 128-bit stores; the integer deltas of every accepted
 //       copy go out at once as 64-bit reductions (RED) on the live per-cell arrays.
-// The Act bytes are not staged: the geometric means read them from global memory (L2) and accepted
-// copies store Max_act there directly.  The id tile keeps halo 1; the geometric mean around a source
-// that lies in the halo reads the few ids of ring 2 from global memory too (they belong to inactive
-// subsections, so they are stable during the phase-step).
 // Nothing here is shared with oracle/.
 #pragma once
 #include "cpm_device.cuh"
 
 namespace cpm {
 
-constexpr int TK_CAP = 32;          // own-delta entries per thread (cells changed in one activation)
-constexpr int TK_REG = 4;           // of which the first keys are held in registers
-constexpr int GM_BATCH = 2;          // Act geometric means computed per batch (their global loads overlap)
-constexpr int TK_WARPS = 2;         // warps per CTA: 4 CTAs of 2 x 27 KB tiles fill the 228 KB of an SM (3D, S = 4)
+constexpr int TK_CAP = 32;     // own-delta entries per subsection (cells changed in one activation)
+constexpr int TK_REG = 4;      // of which the first are held in registers
+constexpr int GM_BATCH = 2;    // Act geometric means computed per batch (their global loads overlap)
+constexpr int TK_CH = 16;      // subsections (chains) per warp: one lane pair each
+constexpr int TK_WARPS = 4;    // warps per CTA: 4 CTAs of 4 x 13.5 KB tiles fill the 228 KB of an SM (3D, S = 4)
 
 template <int DIM, int S>
 struct TGeom {
@@ -46,14 +53,6 @@ struct TGeom {
   static_assert(S == 2 || S == 4 || S == 8 || S == 16, "power-of-two subsection edge");
 };
 
-// compile-time neighbour offsets, same enumeration as nb_delta
-template <int DIM>
-__host__ __device__ constexpr int nbc_dx(int nb) { return (nb + (nb >= ((DIM == 2) ? 4 : 13) ? 1 : 0)) % 3 - 1; }
-template <int DIM>
-__host__ __device__ constexpr int nbc_dy(int nb) { return ((nb + (nb >= ((DIM == 2) ? 4 : 13) ? 1 : 0)) / 3) % 3 - 1; }
-template <int DIM>
-__host__ __device__ constexpr int nbc_dz(int nb) { return (DIM == 3) ? (nb + (nb >= 13 ? 1 : 0)) / 9 - 1 : 0; }
-
 // dynamically indexed part of the own-delta table: kept apart from ThreadSweep so that everything
 // else in there stays in registers
 struct OwnTable {
@@ -66,33 +65,34 @@ struct ThreadSweep {
   using G = TGeom<DIM, S>;
   static constexpr int T = G::T;
   static constexpr int NNB = G::NNB;
+  static constexpr int HNB = NNB / 2;                  // neighbours per lane of the pair
+  static constexpr int CH = TK_CH;
   static constexpr uint32_t CELL_MASK = 0x7FFFFFFFu;   // type + id: equal iff same cell
 
   const SweepParams &P;
   // Shared-memory layout of the CTA (TK_WARPS warps), all offsets compile-time so that every access is a
-  // plain LDS/STS: [id tiles: TK_WARPS x WORDS x 32 words][neighbour offsets: 32 ints][neighbour codes: 32
-  // ints][type records: 9][D: nT^3, then J(t,t): nT].  The Act field is NOT staged: it is read by the
-  // geometric means only (a few lanes per round) and written by accepted copies only, straight in
-  // global memory, which leaves room for two more warps per SM.
-  static constexpr int OFF_TAB = TK_WARPS * G::WORDS * 128;
+  // plain LDS/STS: [id tiles: TK_WARPS x WORDS x CH words][neighbour offsets: 32 ints][neighbour codes: 32
+  // ints][type records: 9][D: nT^3, then J(t,t): nT]
+  static constexpr int OFF_TAB = TK_WARPS * G::WORDS * CH * 4;
   static constexpr int OFF_TYPES = OFF_TAB + 256;
   static constexpr int OFF_D = OFF_TYPES + 9 * (int)sizeof(TypeParams);
   static __device__ __forceinline__ unsigned char *sm() { extern __shared__ __align__(128) unsigned char smem[]; return smem; }
-  static __device__ __forceinline__ uint32_t *tl0() {   // tile of lane 0 of this warp
-    return reinterpret_cast<uint32_t *>(sm()) + (threadIdx.x >> 5) * (G::WORDS * 32);
+  static __device__ __forceinline__ uint32_t *tl0() {   // tile of subsection 0 of this warp
+    return reinterpret_cast<uint32_t *>(sm()) + (threadIdx.x >> 5) * (G::WORDS * CH);
   }
-  static __device__ __forceinline__ uint32_t *tl() { return tl0() + (threadIdx.x & 31); }   // this lane's word j at [32 * j]
-  static __device__ __forceinline__ int *so() { return reinterpret_cast<int *>(sm() + OFF_TAB); }             // nbr -> 32 * tile offset
+  static __device__ __forceinline__ uint32_t *tl() { return tl0() + ((threadIdx.x & 31) >> 1); }   // this pair's word j at [CH * j]
+  static __device__ __forceinline__ int *so() { return reinterpret_cast<int *>(sm() + OFF_TAB); }             // nbr -> CH * tile offset
   static __device__ __forceinline__ int *sn() { return so() + 32; }   // nbr -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
   static __device__ __forceinline__ TypeParams *st() { return reinterpret_cast<TypeParams *>(sm() + OFF_TYPES); }   // [nT + 1], row nT zero
   static __device__ __forceinline__ int32_t *sd() { return reinterpret_cast<int32_t *>(sm() + OFF_D); }       // [nT][nT][nT] adhesion differences
   __device__ __forceinline__ const int32_t *sdiag() const { return sd() + P.nT * P.nT * P.nT; }                // [nT] J(t,t)
-  int lane;
+  int lane, half;          // half = lane & 1: which lane of the pair
+  int noff[HNB];           // CH * tile offsets of this lane's neighbours: n = 2 i + half
   int ox, oy, oz;
   uint32_t b;
   uint32_t mcs;
   // own deltas of this activation (deterministic mode): cell -> composite {dV, dP}; the first TK_REG
-  // entries in registers, the rest in local memory
+  // entries in registers, the rest in local memory; both lanes of the pair keep the same copy
   uint32_t rk[TK_REG];
   unsigned long long rdv[TK_REG];
   OwnTable &tb;
@@ -101,10 +101,9 @@ struct ThreadSweep {
 
   __device__ __forceinline__ ThreadSweep(const SweepParams &p, OwnTable &t) : P(p), tb(t) {}
 
-  static __device__ __forceinline__ int off32(int dx, int dy, int dz) { return 32 * ((dz * T + dy) * T + dx); }
-  static __device__ __forceinline__ int site32(int l) {   // site index -> 32 * tile offset
+  static __device__ __forceinline__ int siteoff(int l) {   // site index -> CH * tile offset
     const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
-    return 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1);
+    return CH * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1);
   }
 
   // ---- boundary rule for one axis (reading S5): false = outside a closed lattice ----
@@ -114,70 +113,56 @@ struct ThreadSweep {
     return true;
   }
 
-  // ---- a2: stage this lane's tile ----
+  // ---- a2: stage this pair's tile; this lane takes the rows r = 2 i + half ----
   __device__ __forceinline__ void load_tile() {
     int xl = ox - 1, xr = ox + S;
     const bool okxl = wrap(xl, P.X, P.per[0]);
     const bool okxr = wrap(xr, P.X, P.per[0]);
-    constexpr int TZ = (DIM == 3) ? T : 1;
-    // row offsets (in rows) of the T tile rows / planes under the boundary rule; only the first and
-    // the last can fall outside the lattice
-    long long yo[T], zo[TZ];
-    bool yok[T], zok[TZ];
+    const int hrow = half * (CH * T);
 #pragma unroll
-    for (int ty = 0; ty < T; ++ty) {
-      int gy = oy - 1 + ty;
-      yok[ty] = (ty == 0 || ty == T - 1) ? wrap(gy, P.Y, P.per[1]) : true;
-      yo[ty] = gy;
-    }
+    for (int i = 0; i < G::ROWS / 2; ++i) {
+      // T is even: row 2 i + half lies in plane (2 i) / T at y = (2 i) % T + half
+      const int ty0 = (2 * i) % T, tz = (2 * i) / T;
+      int gy = oy - 1 + ty0 + half, gz = (DIM == 3) ? oz - 1 + tz : 0;
+      bool ok = true;
+      if (ty0 == 0 || ty0 == T - 2) ok = wrap(gy, P.Y, P.per[1]);        // only the outermost rows can be outside
+      if (DIM == 3 && (tz == 0 || tz == T - 1)) ok = wrap(gz, P.Z, P.per[2]) && ok;
+      const long long rowi = (long long)gy + (long long)P.Y * gz;
+      const uint32_t *rowp = P.lat + P.pitch * rowi;
+      uint32_t *dst = tl() + CH * T * (2 * i) + hrow;
+      const bool okl = ok && okxl, okr = ok && okxr;
+      dst[0] = okl ? __ldg(rowp + xl) : 0u;
+      dst[CH * (S + 1)] = okr ? __ldg(rowp + xr) : 0u;
+      if constexpr (S % 4 == 0) {
 #pragma unroll
-    for (int tz = 0; tz < TZ; ++tz) {
-      int gz = (DIM == 3) ? oz - 1 + tz : 0;
-      zok[tz] = (DIM == 3 && (tz == 0 || tz == T - 1)) ? wrap(gz, P.Z, P.per[2]) : true;
-      zo[tz] = (long long)P.Y * gz;
-    }
-#pragma unroll
-    for (int tz = 0; tz < TZ; ++tz) {
-#pragma unroll
-      for (int ty = 0; ty < T; ++ty) {
-        const bool ok = zok[tz] && yok[ty];
-        const long long rowi = zo[tz] + yo[ty];
-        const uint32_t *rowp = P.lat + P.pitch * rowi;
-        uint32_t *dst = tl() + 32 * ((tz * T + ty) * T);
-        const bool okl = ok && okxl, okr = ok && okxr;
-        dst[0] = okl ? __ldg(rowp + xl) : 0u;
-        dst[32 * (S + 1)] = okr ? __ldg(rowp + xr) : 0u;
-        if constexpr (S % 4 == 0) {
-#pragma unroll
-          for (int q = 0; q < S / 4; ++q) {
-            uint4 v = make_uint4(0u, 0u, 0u, 0u);
-            if (ok) v = __ldg(reinterpret_cast<const uint4 *>(rowp + ox + 4 * q));
-            dst[32 * (1 + 4 * q)] = v.x; dst[32 * (2 + 4 * q)] = v.y; dst[32 * (3 + 4 * q)] = v.z; dst[32 * (4 + 4 * q)] = v.w;
-          }
-        } else {
-          uint2 v = make_uint2(0u, 0u);
-          if (ok) v = __ldg(reinterpret_cast<const uint2 *>(rowp + ox));
-          dst[32] = v.x; dst[64] = v.y;
+        for (int q = 0; q < S / 4; ++q) {
+          uint4 v = make_uint4(0u, 0u, 0u, 0u);
+          if (ok) v = __ldg(reinterpret_cast<const uint4 *>(rowp + ox + 4 * q));
+          dst[CH * (1 + 4 * q)] = v.x; dst[CH * (2 + 4 * q)] = v.y; dst[CH * (3 + 4 * q)] = v.z; dst[CH * (4 + 4 * q)] = v.w;
         }
+      } else {
+        uint2 v = make_uint2(0u, 0u);
+        if (ok) v = __ldg(reinterpret_cast<const uint2 *>(rowp + ox));
+        dst[CH] = v.x; dst[2 * CH] = v.y;
       }
     }
   }
 
-  // ---- a10: write the interior back ----
+  // ---- a10: write the interior back; this lane takes the interior rows r = 2 i + half ----
   __device__ __forceinline__ void store_tile() {
     constexpr int NR = (DIM == 3) ? S * S : S;
 #pragma unroll
-    for (int r = 0; r < NR; ++r) {
-      const int ly = r % S, lz = r / S;
-      const long long rowi = (long long)(oy + ly) + (long long)P.Y * ((DIM == 3) ? oz + lz : 0);
+    for (int i = 0; i < NR / 2; ++i) {
+      const int ly0 = (2 * i) % S, lz = (2 * i) / S;   // S is even
+      const long long rowi = (long long)(oy + ly0 + half) + (long long)P.Y * ((DIM == 3) ? oz + lz : 0);
       uint32_t *rowp = P.lat + P.pitch * rowi + ox;
-      const uint32_t *src = tl() + 32 * ((((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + 1);
+      const uint32_t *src = tl() + CH * ((((DIM == 3) ? (lz + 1) * T : 0) + ly0 + 1) * T + 1) + half * (CH * T);
       if constexpr (S % 4 == 0) {
 #pragma unroll
         for (int q = 0; q < S / 4; ++q)
-          *reinterpret_cast<uint4 *>(rowp + 4 * q) = make_uint4(src[32 * (4 * q)], src[32 * (4 * q + 1)], src[32 * (4 * q + 2)], src[32 * (4 * q + 3)]);
+          *reinterpret_cast<uint4 *>(rowp + 4 * q) = make_uint4(src[CH * (4 * q)], src[CH * (4 * q + 1)], src[CH * (4 * q + 2)], src[CH * (4 * q + 3)]);
       } else {
-        *reinterpret_cast<uint2 *>(rowp) = make_uint2(src[0], src[32]);
+        *reinterpret_cast<uint2 *>(rowp) = make_uint2(src[0], src[CH]);
       }
     }
   }
@@ -198,14 +183,16 @@ struct ThreadSweep {
     }
   }
   // a9/a10: the integer deltas of an accepted copy go to the live per-cell arrays at once (fire-and-forget
-  // reductions; nobody reads them before the next phase-step in deterministic mode) and, in
-  // deterministic mode, into this lane's own-delta table
+  // reductions by the even lane; nobody reads them before the next phase-step in deterministic mode)
+  // and, in deterministic mode, into the own-delta table (both lanes)
   __device__ __forceinline__ void add_delta(uint32_t cell, int dV, int dP, int x, int y, int z, int sgn) {
     const unsigned long long d = ((unsigned long long)(long long)dV << 32) + (unsigned long long)(long long)dP;
-    atomicAdd(P.liveVP + cell, d);
-    atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
-    atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
-    if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
+    if (half == 0) {
+      atomicAdd(P.liveVP + cell, d);
+      atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * x));
+      atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * y));
+      if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * z));
+    }
     if constexpr (!LIVE) {
       bool hit = false;
 #pragma unroll
@@ -228,15 +215,15 @@ struct ThreadSweep {
   }
 
   // ---- Act: fixed-point geometric mean over {x} + same-cell Moore neighbours (Eq 9, reading S8) ----
-  // Computed by the whole warp for the subsection of lane L: lane n < NNB takes neighbour n of the
-  // centre c = (cx, cy, cz) (tile coordinates), lane NNB the centre itself.  Sites outside the halo-1
-  // tile (ring 2 around the subsection) are read from global memory.  Warp-uniform arguments.
-  // gm_site: this lane's site of the neighbourhood -> (same cell?, Act value); gm_value: the reduction.
-  __device__ __forceinline__ bool gm_site(int L, int c, uint32_t mC, int oxL, int oyL, int ozL, int &av_out) const {
+  // Computed by the whole warp for subsection c of the warp: lane n < NNB takes neighbour n of the
+  // centre (cx, cy, cz) (tile coordinates packed in ctr), lane NNB the centre itself.  Ids outside the
+  // halo-1 tile (ring 2 around the subsection) and all Act bytes are read from global memory.
+  // Warp-uniform arguments.  gm_site: this lane's site -> (same cell?, Act value); gm_value: the reduction.
+  __device__ __forceinline__ bool gm_site(int c, int ctr, uint32_t mC, int oxL, int oyL, int ozL, int &av_out) const {
     const bool part = lane <= NNB;
     const int code = sn()[part ? lane : NNB];
-    const int px = (c & 255) + (code & 3) - 1, py = ((c >> 8) & 255) + ((code >> 2) & 3) - 1;
-    const int pz = (DIM == 3) ? ((c >> 16) & 255) + ((code >> 4) & 3) - 1 : 0;
+    const int px = (ctr & 255) + (code & 3) - 1, py = ((ctr >> 8) & 255) + ((code >> 2) & 3) - 1;
+    const int pz = (DIM == 3) ? ((ctr >> 16) & 255) + ((code >> 4) & 3) - 1 : 0;
     uint32_t w = 0u;
     int av = 1;
     bool have = false;
@@ -249,7 +236,7 @@ struct ThreadSweep {
       if (DIM == 3) ok = wrap(gz, P.Z, P.per[2]) && ok;
       const long long rowi = (long long)gy + (long long)P.Y * gz;
       gidx = P.apitch * rowi + gx;
-      if (in) w = tl0()[32 * ((pz * T + py) * T + px) + L];
+      if (in) w = tl0()[CH * ((pz * T + py) * T + px) + c];
       else if (ok) w = __ldg(P.lat + P.pitch * rowi + gx);
       have = ok;   // outside a closed lattice: medium, never the same cell
     }
@@ -267,17 +254,17 @@ struct ThreadSweep {
     return __ldg(P.expq16 + ((m >> 6) & 1023)) << (m >> 16);
   }
 
-  // ---- a5-a7 for this lane's attempt: census of t, per-cell state, dH without the Act term ----
+  // ---- a5-a7 for this pair's attempt: census of t, per-cell state, dH without the Act term ----
   struct Eval {
-    int t32, s32, l, nb, a;
+    int toff, soff, l, nb, a;
     uint32_t wA, mA, mB;
     long long dH;
     int dPA, dPB;
     int lamA_a, maxA_a, lamA_b, maxA_b;   // Act parameters of the source / target cell's type
     bool go;                              // false: refused before Metropolis (reading S13)
   };
-  __device__ __forceinline__ void census(Eval &e) {
-    const uint32_t wA = tl()[e.s32], wB = tl()[e.t32];
+  __device__ __forceinline__ void census(Eval &e, unsigned evmask) {
+    const uint32_t wA = tl()[e.soff], wB = tl()[e.toff];
     const uint32_t A = wA & ID_MASK, B = wB & ID_MASK;
     const uint32_t mA = wA & CELL_MASK, mB = wB & CELL_MASK;
     const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
@@ -287,16 +274,19 @@ struct ThreadSweep {
     if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
     if (B != 0) baseB = LIVE ? __ldcg(P.liveVP + B) : __ldg(P.snapVP + B);
 
-    // neighbour census of t: n_A, n_B and sum_n [J(tA,tn) - J(tB,tn)]
+    // neighbour census of t, this lane's half: n_A, n_B and sum_n [J(tA,tn) - J(tB,tn)]
     const int32_t *Drow = sd() + (tA * P.nT + tB) * P.nT;
-    int nA = 0, nB = 0, adh = 0;
+    int nAB = 0, adh = 0;   // n_A in the low half-word, n_B in the high one
 #pragma unroll
-    for (int n = 0; n < NNB; ++n) {
-      const uint32_t m = tl()[e.t32 + off32(nbc_dx<DIM>(n), nbc_dy<DIM>(n), nbc_dz<DIM>(n))] & CELL_MASK;
-      nA += (m == mA);
-      nB += (m == mB);
+    for (int i = 0; i < HNB; ++i) {
+      const uint32_t m = tl()[e.toff + noff[i]] & CELL_MASK;
+      nAB += (m == mA) ? 1 : 0;
+      nAB += (m == mB) ? 0x10000 : 0;
       adh += Drow[m >> 24];
     }
+    nAB += __shfl_xor_sync(evmask, nAB, 1);   // the other lane's half of the neighbourhood
+    adh += __shfl_xor_sync(evmask, adh, 1);
+    const int nA = nAB & 0xFFFF, nB = nAB >> 16;
     // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
     adh += nB * sdiag()[tB] - nA * sdiag()[tA];
     long long dH = adh;
@@ -318,7 +308,7 @@ struct ThreadSweep {
     e.lamA_a = pa.lamA; e.maxA_a = pa.maxA; e.lamA_b = pb.lamA; e.maxA_b = pb.maxA;
   }
 
-  // ---- a8-a9: Metropolis and commit; returns true if the copy was made ----
+  // ---- a8-a9: Metropolis and commit (both lanes alike; the even lane writes memory) ----
   __device__ __forceinline__ bool decide(const Eval &e) {
     const long long dH = e.dH;
     if (dH > 0 && !P.accept_all) {
@@ -326,13 +316,13 @@ struct ThreadSweep {
       const uint4 ua = philox4x32_10(make_uint4((uint32_t)e.a >> 2, b, 2u * P.p + 1u, mcs), P.key0, P.key1);
       if (pick(ua, e.a & 3) >= __ldg(P.thr + dH)) return false;
     }
-    tl()[e.t32] = e.wA;
+    if (half == 0) tl()[e.toff] = e.wA;
     dirty = true;
     const int l = e.l;
     const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
     const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
     if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-      P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)e.maxA_a;
+      if (half == 0) P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)e.maxA_a;
     const uint32_t A = e.mA & ID_MASK, B = e.mB & ID_MASK;
     if (A != 0) add_delta(A, 1, e.dPA, gx, gy, gz, +1);
     if (B != 0) add_delta(B, -1, e.dPB, gx, gy, gz, -1);
@@ -341,16 +331,19 @@ struct ThreadSweep {
 
   // screen one proposal against the current tile (a4): true = it needs a dH
   __device__ __forceinline__ bool interesting(int prop) const {
-    const int t32 = site32(prop & 255);
-    const uint32_t wt = tl()[t32], ws = tl()[t32 + so()[prop >> 8]];
+    const int toff = siteoff(prop & 255);
+    const uint32_t wt = tl()[toff], ws = tl()[toff + so()[prop >> 8]];
     return (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
   }
 
-  // ---- the whole activation of this lane's subsection ----
+  // ---- the whole activation of this pair's subsection ----
   __device__ __forceinline__ void run(bool active, unsigned long long w) {
     n_entries = 0; dirty = false; overflow = false;
 #pragma unroll
     for (int i = 0; i < TK_REG; ++i) { rk[i] = 0xFFFFFFFFu; rdv[i] = 0ull; }
+#pragma unroll
+    for (int i = 0; i < HNB; ++i) noff[i] = so()[2 * i + half];
+    const unsigned pairmask = 3u << (lane & ~1);
     mcs = *P.mcs_ptr;
     ox = oy = oz = 0; b = 0;
     if (active) {
@@ -364,51 +357,60 @@ struct ThreadSweep {
       load_tile();
     }
     const int k = active ? P.k : 0;
-    const int nq = (k + 3) >> 2;     // quads of this activation
-    int q = 0;                       // next quad to draw
-    unsigned mask = 0u;              // attempts of the current quad (bit j) that still need a dH
-    int prop[4] = {0, 0, 0, 0};      // l | nb << 8 of the current quad
+    const int noct = (k + 7) >> 3;   // octs of this activation
+    int oq = 0;                      // next oct to draw
+    unsigned mask8 = 0u;             // attempts of the current oct (bit jj) that still need a dH
+    int prop[4] = {0, 0, 0, 0};      // l | nb << 8 of this lane's four attempts 4 half + j of the oct
     uint32_t n_eval = 0, n_acc = 0;
     while (true) {
-      // step 1: lanes without a pending attempt draw and screen their next quad
-      if (mask == 0u && q < nq) {
-        const uint4 r = philox4x32_10(make_uint4((uint32_t)q, b, 2u * P.p, mcs), P.key0, P.key1);
+      __syncwarp();   // tile words written by the other lane of the pair (staging, commits) are visible
+      // step 1: pairs without a pending attempt draw and screen their next oct
+      unsigned my = 0u;
+      const bool draw = mask8 == 0u && oq < noct;
+      if (draw) {
+        const uint4 r = philox4x32_10(make_uint4((uint32_t)(2 * oq + half), b, 2u * P.p, mcs), P.key0, P.key1);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           const uint32_t wd = pick(r, j);
           const int l = (int)(wd >> (32 - G::LOG2SITES));                          // = (wd * S^d) >> 32
           const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
           prop[j] = l | (nb << 8);
-          if (4 * q + j < k && interesting(prop[j])) mask |= 1u << j;
+          if (8 * oq + 4 * half + j < k && interesting(prop[j])) my |= 1u << j;
         }
-        ++q;
+        ++oq;
       }
-      if (!__any_sync(FULL, mask != 0u || q < nq)) break;
+      {
+        const unsigned other = __shfl_xor_sync(FULL, my, 1);
+        if (draw) mask8 = half ? (other | (my << 4)) : (my | (other << 4));
+      }
+      const bool ev = mask8 != 0u;
+      const unsigned evmask = __ballot_sync(FULL, ev);
+      if (evmask == 0u && !__any_sync(FULL, oq < noct)) break;
 
-      // step 2: lanes with a pending attempt evaluate the first one
-      const bool ev = mask != 0u;
+      // step 2: pairs with a pending attempt evaluate the first one
       Eval e;
       e.go = false; e.lamA_a = 0; e.lamA_b = 0; e.maxA_a = 0; e.maxA_b = 0; e.mA = 0u; e.mB = 0u; e.l = 0; e.nb = 0;
-      int j = 0;
+      int jj = 0;
       if (ev) {
-        j = __ffs(mask) - 1;
-        const int pj = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
+        jj = __ffs(mask8) - 1;
+        const int j = jj & 3;
+        const int cand = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
+        const int pj = __shfl_sync(evmask, cand, (lane & ~1) | (jj >> 2));   // the attempt lives in lane jj / 4 of the pair
         e.l = pj & 255; e.nb = pj >> 8;
-        e.t32 = site32(e.l); e.s32 = e.t32 + so()[e.nb];
-        e.a = 4 * (q - 1) + j;
-        ++n_eval;
-        census(e);
+        e.toff = siteoff(e.l); e.soff = e.toff + so()[e.nb];
+        e.a = 8 * (oq - 1) + jj;
+        if (half == 0) ++n_eval;
+        census(e, evmask);
       }
       if constexpr (ACT) {
-        // geometric means for the lanes whose source / target cell has an Act bias, by the whole warp;
-        // the Act bytes stored by earlier commits of any lane must be visible to all lanes
-        __syncwarp();
+        // geometric means for the pairs whose source / target cell has an Act bias, by the whole warp
+        // (the Act bytes stored by earlier commits are visible after the __syncwarp above)
         const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
         const int code = sn()[e.nb];
         const int ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
         const int cs = (lx + (code & 3)) | ((ly + ((code >> 2) & 3)) << 8) | ((DIM == 3 ? lz + ((code >> 4) & 3) : 1) << 16);
-        unsigned needA = __ballot_sync(FULL, ev && e.go && e.lamA_a != 0);
-        unsigned needB = __ballot_sync(FULL, ev && e.go && e.lamA_b != 0);
+        unsigned needA = __ballot_sync(FULL, ev && half == 0 && e.go && e.lamA_a != 0);
+        unsigned needB = __ballot_sync(FULL, ev && half == 0 && e.go && e.lamA_b != 0);
         long long sideA = 0, sideB = 0;
         while (needA | needB) {
           // up to GM_BATCH neighbourhoods at a time: all their global Act loads are in flight together
@@ -421,17 +423,17 @@ struct ThreadSweep {
               isAs[i] = needA != 0u;
               Ls[i] = __ffs(isAs[i] ? needA : needB) - 1;
               if (isAs[i]) needA &= needA - 1; else needB &= needB - 1;
-              const int c = __shfl_sync(FULL, isAs[i] ? cs : ct, Ls[i]);
+              const int ctr = __shfl_sync(FULL, isAs[i] ? cs : ct, Ls[i]);
               const uint32_t mC = __shfl_sync(FULL, isAs[i] ? e.mA : e.mB, Ls[i]);
               const int oxL = __shfl_sync(FULL, ox, Ls[i]), oyL = __shfl_sync(FULL, oy, Ls[i]), ozL = __shfl_sync(FULL, oz, Ls[i]);
-              same[i] = gm_site(Ls[i], c, mC, oxL, oyL, ozL, av[i]);
+              same[i] = gm_site(Ls[i] >> 1, ctr, mC, oxL, oyL, ozL, av[i]);
             }
           }
 #pragma unroll
           for (int i = 0; i < GM_BATCH; ++i) {
             if (Ls[i] >= 0) {
               const int g = gm_value(same[i], av[i]);
-              if (lane == Ls[i] && g != 0) {
+              if ((lane >> 1) == (Ls[i] >> 1) && g != 0) {   // both lanes of the pair
                 if (isAs[i]) sideA = ((long long)e.lamA_a * g) / e.maxA_a;
                 else sideB = ((long long)e.lamA_b * g) / e.maxA_b;
               }
@@ -441,18 +443,21 @@ struct ThreadSweep {
         if ((e.lamA_a | e.lamA_b) != 0) e.dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
       }
       if (ev) {
-        mask &= mask - 1u;                 // attempt j is done
+        mask8 &= mask8 - 1u;               // attempt jj is done
         if (e.go && decide(e)) {
-          ++n_acc;
-          // later attempts of the quad see the new tile: screen them again
+          if (half == 0) ++n_acc;
+          // later attempts of the oct see the new tile: screen them again
+          __syncwarp(pairmask);
           unsigned m2 = 0u;
 #pragma unroll
-          for (int jj = 1; jj < 4; ++jj)
-            if (jj > j && 4 * (q - 1) + jj < k && interesting(prop[jj])) m2 |= 1u << jj;
-          mask = m2;
+          for (int j = 0; j < 4; ++j)
+            if (4 * half + j > jj && 8 * (oq - 1) + 4 * half + j < k && interesting(prop[j])) m2 |= 1u << j;
+          const unsigned o2 = __shfl_xor_sync(pairmask, m2, 1);
+          mask8 = half ? (o2 | (m2 << 4)) : (m2 | (o2 << 4));
         }
       }
     }
+    __syncwarp();
     if (dirty) store_tile();
     n_eval = __reduce_add_sync(FULL, n_eval);
     n_acc = __reduce_add_sync(FULL, n_acc);
@@ -466,8 +471,8 @@ struct ThreadSweep {
   }
 };
 
-// TK_WARPS warps per CTA (they share only the small tables), one lane per active subsection; dynamic
-// smem laid out as in ThreadSweep.
+// TK_WARPS warps per CTA (they share only the small tables), one lane pair per active subsection;
+// dynamic smem laid out as in ThreadSweep.
 template <int DIM, int S, bool ACT, bool LIVE>
 __global__ void __launch_bounds__(32 * TK_WARPS) sweep_thread_kernel(const __grid_constant__ SweepParams P) {
   using TS = ThreadSweep<DIM, S, ACT, LIVE>;
@@ -476,7 +481,7 @@ __global__ void __launch_bounds__(32 * TK_WARPS) sweep_thread_kernel(const __gri
   if (tid < 32) {
     int dx = 0, dy = 0, dz = 0;
     if (tid < G::NNB) nb_delta<DIM>(tid, dx, dy, dz);
-    TS::so()[tid] = 32 * ((dz * G::T + dy) * G::T + dx);
+    TS::so()[tid] = TK_CH * ((dz * G::T + dy) * G::T + dx);
     TS::sn()[tid] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
   }
   for (int i = tid; i < (P.nT + 1) * 8; i += 32 * TK_WARPS)
@@ -484,10 +489,11 @@ __global__ void __launch_bounds__(32 * TK_WARPS) sweep_thread_kernel(const __gri
   const int nD = P.nT * P.nT * P.nT + P.nT;
   for (int i = tid; i < nD; i += 32 * TK_WARPS) TS::sd()[i] = P.D[i];
   __syncthreads();
-  const unsigned long long w = (unsigned long long)blockIdx.x * (32 * TK_WARPS) + tid;
+  const unsigned long long w = (unsigned long long)blockIdx.x * (TK_CH * TK_WARPS) + (tid >> 5) * TK_CH + ((tid & 31) >> 1);
   OwnTable tab;
   TS sw(P, tab);
   sw.lane = tid & 31;
+  sw.half = tid & 1;
   sw.run(w < P.n_active, w);
 }
 

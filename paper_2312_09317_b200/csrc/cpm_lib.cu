@@ -297,7 +297,7 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     size_t words = 1;
     for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
     c->wpc = TK_WARPS;
-    c->cta_smem = (size_t)TK_WARPS * words * TK_CH * 4 + 256 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
+    c->cta_smem = (size_t)TK_WARPS * words * TK_CH * 4 + 256 + 512 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
   }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 

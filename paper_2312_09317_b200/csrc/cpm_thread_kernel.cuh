@@ -72,9 +72,10 @@ struct ThreadSweep {
   const SweepParams &P;
   // Shared-memory layout of the CTA (TK_WARPS warps), all offsets compile-time so that every access is a
   // plain LDS/STS: [id tiles: TK_WARPS x WORDS x CH words][neighbour offsets: 32 ints][neighbour codes: 32
-  // ints][type records: 9][D: nT^3, then J(t,t): nT]
+  // ints][site offsets: 256 shorts][type records: 9][D: nT^3, then J(t,t): nT]
   static constexpr int OFF_TAB = TK_WARPS * G::WORDS * CH * 4;
-  static constexpr int OFF_TYPES = OFF_TAB + 256;
+  static constexpr int OFF_SITE = OFF_TAB + 256;
+  static constexpr int OFF_TYPES = OFF_SITE + 512;
   static constexpr int OFF_D = OFF_TYPES + 9 * (int)sizeof(TypeParams);
   static __device__ __forceinline__ unsigned char *sm() { extern __shared__ __align__(128) unsigned char smem[]; return smem; }
   static __device__ __forceinline__ uint32_t *tl0() {   // tile of subsection 0 of this warp
@@ -83,6 +84,7 @@ struct ThreadSweep {
   static __device__ __forceinline__ uint32_t *tl() { return tl0() + ((threadIdx.x & 31) >> 1); }   // this pair's word j at [CH * j]
   static __device__ __forceinline__ int *so() { return reinterpret_cast<int *>(sm() + OFF_TAB); }             // nbr -> CH * tile offset
   static __device__ __forceinline__ int *sn() { return so() + 32; }   // nbr -> (dx+1) | (dy+1) << 2 | (dz+1) << 4; entry NNB = centre
+  static __device__ __forceinline__ unsigned short *ssite() { return reinterpret_cast<unsigned short *>(sm() + OFF_SITE); }   // site -> CH * tile offset
   static __device__ __forceinline__ TypeParams *st() { return reinterpret_cast<TypeParams *>(sm() + OFF_TYPES); }   // [nT + 1], row nT zero
   static __device__ __forceinline__ int32_t *sd() { return reinterpret_cast<int32_t *>(sm() + OFF_D); }       // [nT][nT][nT] adhesion differences
   __device__ __forceinline__ const int32_t *sdiag() const { return sd() + P.nT * P.nT * P.nT; }                // [nT] J(t,t)
@@ -330,9 +332,11 @@ struct ThreadSweep {
   }
 
   // screen one proposal against the current tile (a4): true = it needs a dH
+  // a proposal is kept as toff | nb << 13 | l << 18 (toff = CH * tile offset of the target site)
+  static __device__ __forceinline__ int pack_prop(int l, int nb) { return (int)ssite()[l] | (nb << 13) | (l << 18); }
   __device__ __forceinline__ bool interesting(int prop) const {
-    const int toff = siteoff(prop & 255);
-    const uint32_t wt = tl()[toff], ws = tl()[toff + so()[prop >> 8]];
+    const int toff = prop & 0x1FFF;
+    const uint32_t wt = tl()[toff], ws = tl()[toff + so()[(prop >> 13) & 31]];
     return (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
   }
 
@@ -360,7 +364,7 @@ struct ThreadSweep {
     const int noct = (k + 7) >> 3;   // octs of this activation
     int oq = 0;                      // next oct to draw
     unsigned mask8 = 0u;             // attempts of the current oct (bit jj) that still need a dH
-    int prop[4] = {0, 0, 0, 0};      // l | nb << 8 of this lane's four attempts 4 half + j of the oct
+    int prop[4] = {0, 0, 0, 0};      // this lane's four attempts 4 half + j of the oct (pack_prop)
     uint32_t n_eval = 0, n_acc = 0;
     while (true) {
       __syncwarp();   // tile words written by the other lane of the pair (staging, commits) are visible
@@ -374,7 +378,7 @@ struct ThreadSweep {
           const uint32_t wd = pick(r, j);
           const int l = (int)(wd >> (32 - G::LOG2SITES));                          // = (wd * S^d) >> 32
           const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
-          prop[j] = l | (nb << 8);
+          prop[j] = pack_prop(l, nb);
           if (8 * oq + 4 * half + j < k && interesting(prop[j])) my |= 1u << j;
         }
         ++oq;
@@ -396,8 +400,8 @@ struct ThreadSweep {
         const int j = jj & 3;
         const int cand = j == 0 ? prop[0] : j == 1 ? prop[1] : j == 2 ? prop[2] : prop[3];
         const int pj = __shfl_sync(evmask, cand, (lane & ~1) | (jj >> 2));   // the attempt lives in lane jj / 4 of the pair
-        e.l = pj & 255; e.nb = pj >> 8;
-        e.toff = siteoff(e.l); e.soff = e.toff + so()[e.nb];
+        e.l = pj >> 18; e.nb = (pj >> 13) & 31;
+        e.toff = pj & 0x1FFF; e.soff = e.toff + so()[e.nb];
         e.a = 8 * (oq - 1) + jj;
         if (half == 0) ++n_eval;
         census(e, evmask);
@@ -405,13 +409,16 @@ struct ThreadSweep {
       if constexpr (ACT) {
         // geometric means for the pairs whose source / target cell has an Act bias, by the whole warp
         // (the Act bytes stored by earlier commits are visible after the __syncwarp above)
-        const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
-        const int code = sn()[e.nb];
-        const int ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
-        const int cs = (lx + (code & 3)) | ((ly + ((code >> 2) & 3)) << 8) | ((DIM == 3 ? lz + ((code >> 4) & 3) : 1) << 16);
         unsigned needA = __ballot_sync(FULL, ev && half == 0 && e.go && e.lamA_a != 0);
         unsigned needB = __ballot_sync(FULL, ev && half == 0 && e.go && e.lamA_b != 0);
         long long sideA = 0, sideB = 0;
+        int ct = 0, cs = 0;   // tile coordinates of the target / the source site, packed
+        if (needA | needB) {
+          const int lx = e.l & (S - 1), ly = (e.l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (e.l >> (2 * G::LOG2S)) : 0;
+          const int code = sn()[e.nb];
+          ct = (lx + 1) | ((ly + 1) << 8) | ((lz + 1) << 16);
+          cs = (lx + (code & 3)) | ((ly + ((code >> 2) & 3)) << 8) | ((DIM == 3 ? lz + ((code >> 4) & 3) : 1) << 16);
+        }
         while (needA | needB) {
           // up to GM_BATCH neighbourhoods at a time: all their global Act loads are in flight together
           int Ls[GM_BATCH], av[GM_BATCH];
@@ -484,6 +491,7 @@ __global__ void __launch_bounds__(32 * TK_WARPS) sweep_thread_kernel(const __gri
     TS::so()[tid] = TK_CH * ((dz * G::T + dy) * G::T + dx);
     TS::sn()[tid] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
   }
+  for (int i = tid; i < G::SITES; i += 32 * TK_WARPS) TS::ssite()[i] = (unsigned short)TS::siteoff(i);
   for (int i = tid; i < (P.nT + 1) * 8; i += 32 * TK_WARPS)
     reinterpret_cast<int32_t *>(TS::st())[i] = reinterpret_cast<const int32_t *>(P.types)[i];
   const int nD = P.nT * P.nT * P.nT + P.nT;

@@ -116,6 +116,20 @@ def build_workload(name, dims, rank):
     return cfg
 
 
+def reduce_over_ranks(times, counts, world, device):
+    """Replicas only: the job's time is the MAX over ranks of each device time,
+    its launch count the SUM; no data-path collective.  Identity for one rank."""
+    if world <= 1:
+        return [float(v) for v in times], [int(v) for v in counts]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(counts), dtype=torch.int64, device=device)
+    dist.all_reduce(c)
+    return [float(v) for v in t.tolist()], [int(v) for v in c.tolist()]
+
+
 def oracle_rate(cfg, sample_dims, n_mcs, warm=0):
     """Attempts/s of the oracle, as it stands, on a corner crop of the workload (one host core)."""
     import cpm_inputs as ci
@@ -255,13 +269,7 @@ def main():
     h2d = ids_h.numel() * 4 + (frozen_h.numel() if frozen_h is not None else 0) + ctype_h.numel()
     d2h = out_h.numel() * 4
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s, sweep_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s, sweep_ms = (float(v) for v in t.tolist())
-        ln = torch.tensor([launches], dtype=torch.int64, device="cuda")
-        dist.all_reduce(ln)
-        launches = int(ln.item())
+    (ms, e2e_s, sweep_ms), (launches,) = reduce_over_ranks([ms, e2e_s, sweep_ms], [launches], world, "cuda")
 
     if rank == 0:
         value = world * N * args.steps / (ms * 1e-3)

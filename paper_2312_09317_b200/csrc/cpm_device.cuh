@@ -103,6 +103,14 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 }
 __device__ __forceinline__ uint32_t pick(const uint4 &v, int j) { return j == 0 ? v.x : j == 1 ? v.y : j == 2 ? v.z : v.w; }
 
+// floor(lamA * g / maxA) of the Act term (reading S8) without a 64-bit division: lamA >= 0,
+// 0 < maxA <= 255 and g < 2^24 (EXP entry < 2^17, shifted by at most 7), so with lamA = q maxA + r
+// the result is q g + floor(r g / maxA) and r g < 2^32
+__device__ __forceinline__ long long act_side(int lamA, int maxA, int g) {
+  const unsigned q = (unsigned)lamA / (unsigned)maxA, r = (unsigned)lamA - q * (unsigned)maxA;
+  return (long long)((unsigned long long)q * (unsigned)g) + (long long)((r * (unsigned)g) / (unsigned)maxA);
+}
+
 // neighbour index (0..nNb-1, centre skipped) -> (dx,dy,dz); order: (dz,dy,dx) lexicographic, dx fastest
 template <int DIM>
 __device__ __forceinline__ void nb_delta(int nb, int &dx, int &dy, int &dz) {
@@ -291,11 +299,11 @@ struct Sweep {
         long long sideA = 0, sideB = 0;
         if (pa.lamA != 0) {
           const int g = gm_q16(spos, atpos + sAOff[(pr >> 24) & 31], A);
-          if (g != 0) sideA = ((long long)pa.lamA * g) / pa.maxA;
+          if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g);
         }
         if (pb.lamA != 0) {
           const int g = gm_q16(tpos, atpos, B);
-          if (g != 0) sideB = ((long long)pb.lamA * g) / pb.maxA;
+          if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g);
         }
         dH -= (sideA - sideB + 32768) >> 16;  // copies FROM active areas are favoured (L259)
       }

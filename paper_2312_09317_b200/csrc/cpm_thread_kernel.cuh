@@ -441,8 +441,8 @@ struct ThreadSweep {
             if (Ls[i] >= 0) {
               const int g = gm_value(same[i], av[i]);
               if ((lane >> 1) == (Ls[i] >> 1) && g != 0) {   // both lanes of the pair
-                if (isAs[i]) sideA = ((long long)e.lamA_a * g) / e.maxA_a;
-                else sideB = ((long long)e.lamA_b * g) / e.maxA_b;
+                if (isAs[i]) sideA = act_side(e.lamA_a, e.maxA_a, g);
+                else sideB = act_side(e.lamA_b, e.maxA_b, g);
               }
             }
           }

@@ -281,10 +281,15 @@ def main():
         achieved = bpa * attempts_per_launch / avg_launch_s / 1e9
         survey_bpa = SURVEY_BYTES_ACT if act_on else SURVEY_BYTES_NOACT
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic_per_launch.json")
+        # dram bytes per sweep launch from the committed ncu --set full capture (profiles/traffic_per_launch.csv)
+        tpath = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get("%s_%s" % (args.config, "x".join(map(str, dims))))
+                key = "%s_%s" % (args.config, "x".join(map(str, dims)))
+                for row in open(tpath).read().splitlines()[1:]:
+                    f = row.split(",")
+                    if f[0] == key and int(f[1]) == sched["S"]:
+                        traffic = int(f[2])
             except Exception:
                 traffic = None
         line = {

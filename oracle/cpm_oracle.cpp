@@ -24,7 +24,9 @@
  * tallies == recount (P2), T->0 / T->inf limits (P3), acceptance frequency vs Eq 2 (P4),
  * conservation (P5), order independence inside a phase-step (P6), proposal statistics (P7),
  * Philox known answers (P8), resume (P10), fixed-point GM vs pow() (P11), threshold table
- * (P12), DETERMINISTIC == LIVE when no cell is shared (P13).
+ * (P12), DETERMINISTIC == LIVE when no cell is shared (P13); round 2: P13b (cells straddling
+ * subsection borders, lambda_P != 0: pins the per-phase-step snapshot refresh and the own dP view),
+ * P11b (each side of the Act bias uses its own cell's type), Act decay after the last phase-step.
  * Parity unpinned: nothing in this file (the LIVE-mode *GPU* ensemble is only statistical).
  */
 #include "cpm_oracle.h"

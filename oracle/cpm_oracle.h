@@ -34,7 +34,7 @@ typedef struct {
   const int32_t *lambda_V, *target_V, *lambda_P, *target_P, *lambda_act, *max_act; /* [n_types] or NULL */
   double   T;              /* 0 = no uphill move; +inf = accept every evaluated move */
   uint64_t seed;
-  int32_t  subsection;     /* S; 0 = default (16 in 2D, 8 in 3D, halved until it divides dims) */
+  int32_t  subsection;     /* S; 0 = default (8 in 2D, 4 in 3D, halved while it does not divide dims; R4) */
   int32_t  attempts_per_activation; /* k; 0 = S^d */
   int32_t  mode;
   uint32_t max_cells;      /* cell IDs are 0..max_cells */

@@ -507,3 +507,173 @@ def test_argument_validation(oracle_mod):
         o.set_lattice(np.full((8, 8), 2, np.uint32), None, np.array([0, 1], np.uint8))  # id > max_cells
     with pytest.raises(ob.OracleError):
         o.step(1)                                             # no lattice yet
+
+
+# ------------------------------------------------ pins added in round 2 --
+def _straddling_case(nd, S, n_per_axis, edge, lamP, act):
+    """Cells of extent `edge` <= S-2 on pitch S, offset by S/2 + 1 so that every cell STRADDLES a
+    subsection border (it is touched by subsections of different colours, i.e. in different
+    phase-steps, but never by two subsections of the same phase-step)."""
+    dims = (S * n_per_axis,) * nd
+    ids = np.zeros(tuple(reversed(dims)), np.uint32)
+    off = S // 2 + 1
+    n = 0
+    rng = range(n_per_axis - 1)
+    for idx in np.ndindex(*([n_per_axis - 1] * nd)):       # idx = (z, y, x) / (y, x)
+        n += 1
+        sl = tuple(slice(off + S * i, off + S * i + edge) for i in idx)
+        ids[sl] = n
+    ct = np.ones(n + 1, np.uint8); ct[0] = 0
+    ct[2::2] = 2
+    J = np.array([[0, 8, 11], [8, 14, 19], [11, 19, 9]], np.int32)
+    vol = edge ** nd
+    per = int(H.recount(ids, n, nd)[1][1])      # Moore-interface count of one seed block
+    kw = dict(J=J, lambda_V=[0, 3, 2], target_V=[0, vol, vol + 3], lambda_P=[0, lamP, lamP],
+              target_P=[0, per, per - 6], T=20.0, seed=4242, subsection=S, max_cells=n)
+    if act:
+        kw.update(lambda_act=[0, 150, 60], max_act=[0, 30, 9])
+    return dims, ids, ct, kw
+
+
+def _no_cell_shared_within_a_phase_step(lat, max_cells, S):
+    """SURVEY P13's precondition, checked exactly: a subsection TOUCHES a cell that has a voxel inside it
+    or in its 1-voxel halo; no cell may be touched by two subsections of the same colour (= of the same
+    phase-step)."""
+    nd = lat.ndim
+    dims = lat.shape[::-1]
+    for cell in range(1, max_cells + 1):
+        idx = np.nonzero(lat == cell)            # (z, y, x) / (y, x)
+        if len(idx[0]) == 0:
+            continue
+        coords = np.stack(idx[::-1], 1)          # columns x, y(, z)
+        touched = set()
+        for shift in np.ndindex(*([3] * nd)):
+            c = coords + (np.array(shift) - 1)
+            ok = np.ones(len(c), bool)
+            for a in range(nd):
+                ok &= (c[:, a] >= 0) & (c[:, a] < dims[a])
+            for b in np.unique(c[ok] // S, axis=0):
+                touched.add(tuple(int(v) for v in b))
+        colours = [tuple(v & 1 for v in b) for b in touched]
+        if len(set(colours)) != len(colours):
+            return False
+    return True
+
+
+@pytest.mark.parametrize("nd,S,n_ax,edge,act", [(2, 16, 5, 10, False), (2, 16, 4, 9, True), (3, 8, 4, 4, True)])
+def test_P13b_deterministic_equals_live_with_cells_straddling_borders(oracle_mod, nd, S, n_ax, edge, act):
+    """Reading S12 under SURVEY P13's ACTUAL precondition (no cell touched by two subsections of the
+    SAME phase-step; sufficient: extent <= S-2), with cells that straddle subsection borders and
+    lambda_P != 0.  A straddling cell is changed by one subsection in one phase-step and read by its
+    neighbour subsection in a later phase-step of the same MCS, so the two modes agree bit for bit
+    only if (i) the snapshot is refreshed at EVERY phase-step (reads may be stale
+    only within a step) and (ii) the worker's own deltas carry dP as well as dV."""
+    dims, ids, ct, kw = _straddling_case(nd, S, n_ax, edge, lamP=1, act=act)
+    n = kw["max_cells"]
+    od = oracle_mod.Oracle(dims, mode=0, **kw)
+    ol = oracle_mod.Oracle(dims, mode=1, **kw)
+    for o in (od, ol):
+        o.set_lattice(ids, None, ct)
+    # the set-up really straddles: every cell has voxels in at least two subsections
+    for cell in range(1, n + 1):
+        idx = np.nonzero(ids == cell)
+        assert any(ax.min() // S != ax.max() // S for ax in idx)
+    agreed = 0
+    multi = 0
+    for m in range(12):
+        if not _no_cell_shared_within_a_phase_step(od.get_lattice(), n, S):
+            break
+        before = od.get_cell_stats()["perimeter"].astype(np.int64)
+        od.step(1); ol.step(1)
+        np.testing.assert_array_equal(od.get_lattice(), ol.get_lattice(), err_msg="MCS %d" % m)
+        sd, sl = od.get_cell_stats(), ol.get_cell_stats()
+        for k in sd:
+            np.testing.assert_array_equal(sd[k], sl[k], err_msg="%s MCS %d" % (k, m))
+        if act:
+            np.testing.assert_array_equal(od.get_act(), ol.get_act())
+        assert od.get_counters() == ol.get_counters()
+        multi += int((sd["perimeter"].astype(np.int64) != before).sum())
+        agreed += 1
+    assert agreed >= 4, agreed
+    assert multi >= 4 * n // 2          # perimeters really move, so a stale P would be seen
+    c = od.get_counters()
+    assert c["accepted"] > 20 * agreed
+
+
+def test_P11b_act_bias_uses_each_sides_own_type(oracle_mod):
+    """Eq 8-9 with reading S8(iii): the source side uses lambda_act/Max_act of
+    the SOURCE cell's type, the target side those of the TARGET cell's type.  Two motile types with
+    different (lambda_act, Max_act); expected dH_act recomputed here in double from Eq 8-9."""
+    ob = oracle_mod
+    J = np.array([[0, 5, 6], [5, 9, 7], [6, 7, 4]], np.int32)
+    lam, mx = [0, 200, 96], [0, 40, 12]
+    o = ob.Oracle((8, 8), J=J, lambda_V=[0, 1, 1], target_V=[0, 9, 9], lambda_act=lam, max_act=mx,
+                  max_cells=2, subsection=8, T=20.0)
+    ids = np.zeros((8, 8), np.uint32); ids[2:5, 1:4] = 1; ids[2:5, 4:7] = 2
+    ct = np.array([0, 1, 2], np.uint8)
+    o.set_lattice(ids, None, ct)
+    rng = np.random.default_rng(5)
+    act = np.zeros((8, 8), np.float32)
+    act[ids == 1] = rng.integers(20, 41, int((ids == 1).sum()))
+    act[ids == 2] = rng.integers(3, 13, int((ids == 2).sum()))
+    o.set_act(act)
+    offs = H.moore_offsets(2); nb_of = {o_: i for i, o_ in enumerate(offs)}
+
+    def gm(x, y):            # Eq 9 over {site} + same-cell Moore neighbours (reading S8(ii)), in double
+        vals = [float(act[y, x])]
+        for dx, dy, _ in offs:
+            xx, yy = x + dx, y + dy
+            if 0 <= xx < 8 and 0 <= yy < 8 and ids[yy, xx] == ids[y, x]:
+                vals.append(float(act[yy, xx]))
+        return float(np.exp(np.mean(np.log(vals))))
+
+    checked = 0
+    for (tx, ty), (dx, dy) in [((4, 3), (-1, 0)), ((3, 3), (1, 0)), ((4, 2), (-1, 1)), ((3, 4), (1, -1)), ((4, 4), (-1, 0))]:
+        sx, sy = tx + dx, ty + dy
+        tA, tB = int(ct[ids[sy, sx]]), int(ct[ids[ty, tx]])
+        assert tA != tB and tA and tB
+        st, dH, dA = o.probe(tx + 8 * ty, nb_of[(dx, dy, 0)])
+        assert st == 1
+        exact = lam[tA] / mx[tA] * gm(sx, sy) - lam[tB] / mx[tB] * gm(tx, ty)
+        wrong = lam[tA] / mx[tA] * gm(sx, sy) - lam[tA] / mx[tA] * gm(tx, ty)   # target side with the source's type
+        tol = 0.5 + 7.2e-4 * (lam[tA] / mx[tA] * gm(sx, sy) + lam[tB] / mx[tB] * gm(tx, ty)) + 1e-3
+        assert abs(dA - exact) <= tol, (dA, exact)
+        assert abs(dA - wrong) > 5 * tol      # the cases tell the two readings apart
+        checked += 1
+    assert checked == 5
+
+
+def test_act_decay_runs_after_the_last_phase_step(oracle_mod):
+    """PAPER.md L255 / reading S9: a copied-into site gets Act = Max_act of its new owner, and the field
+    decays by 1 once per MCS AFTER the last phase-step.  So after one MCS every site that received its
+    last accepted copy in that MCS holds Max_act(new owner) - 1 (0 for medium), and untouched sites hold
+    their start value - 1.  (Decay before the phase loop would leave Max_act itself.)"""
+    ob = oracle_mod
+    J = np.array([[0, 5, 6], [5, 9, 7], [6, 7, 4]], np.int32)
+    mx = [0, 40, 17]
+    o = ob.Oracle((16, 16), J=J, lambda_V=[0, 1, 1], target_V=[0, 30, 30], lambda_act=[0, 100, 50], max_act=mx,
+                  max_cells=4, subsection=4, T=float("inf"), seed=3)
+    ids = np.zeros((16, 16), np.uint32)
+    ids[2:8, 2:8] = 1; ids[2:8, 8:14] = 2; ids[8:14, 2:8] = 3; ids[8:14, 8:14] = 4
+    ct = np.array([0, 1, 2, 2, 1], np.uint8)
+    o.set_lattice(ids, None, ct)
+    act0 = np.zeros((16, 16), np.float32); act0[ids > 0] = 7.0
+    o.set_act(act0)
+    buf, cnt = o.trace(16 * 16)
+    o.step(1)
+    o.stop_trace()
+    assert int(cnt[0]) == 256
+    lat, act = o.get_lattice(), o.get_act()
+    last_owner = {}
+    for site, nb, status, dH, acc, u in buf[: int(cnt[0])]:
+        if acc:
+            last_owner[int(site)] = True
+    assert len(last_owner) >= 20
+    for y in range(16):
+        for x in range(16):
+            if (x + 16 * y) in last_owner:
+                owner = int(lat[y, x])
+                want = max(mx[ct[owner]] - 1, 0) if owner else 0
+            else:
+                want = max(float(act0[y, x]) - 1, 0)
+            assert act[y, x] == want, (x, y, act[y, x], want)

@@ -307,7 +307,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "kernel": "sweep_thread_kernel" if info0["thread_per_subsection"] else "sweep_kernel", "bytes_per_attempt": bpa,
+                         "traffic": traffic, "kernel": "sweep_pool_kernel" if info0["pooled"] else "sweep_kernel", "bytes_per_attempt": bpa,
                          "launches_timed": int(sweep_n), "avg_launch_ms": 1e3 * avg_launch_s, "peak_source": peak_src,
                          "kernel_share_of_step": sweep_ms / ms,
                          "frac_with_survey_model_bytes": survey_bpa * attempts_per_launch / avg_launch_s / 1e9 / peak},

@@ -32,6 +32,10 @@ enum { CPM_OK = 0, CPM_ERR_ARG = -1, CPM_ERR_DIMS = -2, CPM_ERR_UNSUPPORTED = -3
        CPM_ERR_CUDA = -4, CPM_ERR_OOM = -5, CPM_ERR_STATE = -6 };
 enum { CPM_MOORE = 0 }; /* the only neighbourhood the paper uses (L225): 8 / 26 neighbours */
 enum {
+  CPM_FLAG_WARP_KERNEL = 1, /* use the warp-per-subsection kernel even where the pooled kernel applies */
+  CPM_FLAG_NO_TMA = 2       /* warp-per-subsection kernel: stage tiles with plain loads instead of TMA */
+};
+enum {
   CPM_MODE_DETERMINISTIC = 0, /* per-cell state read from a phase-start snapshot + the worker's own
                                  deltas; integer atomic deltas applied after (bit-exact, schedule-free) */
   CPM_MODE_LIVE_ATOMICS = 1   /* paper-faithful: live reads (possibly stale, L53), immediate atomics (L51) */
@@ -57,6 +61,7 @@ typedef struct {
   uint32_t max_cells;             /* cell ids are 0..max_cells; < 2^24 */
   int32_t  device;                /* CUDA device ordinal */
   void    *stream;                /* cudaStream_t (e.g. torch's current stream); NULL = default stream */
+  uint32_t flags;                 /* CPM_FLAG_*; 0 = the library chooses (debug / A-B switches for tests) */
 } cpm_params;
 
 /* Validate parameters, build the type tables, the Metropolis threshold table (Eq 2) and the
@@ -98,7 +103,8 @@ int  cpm_get_schedule(cpm_ctx *ctx, int32_t *S, int32_t *k, int32_t *phase_steps
 int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);
 /* Introspection: kernels launched by this context so far, and the launch geometry of the sweep
  * kernel: out = {launches, sweep_launches, warps_per_cta, smem_bytes_per_cta, uses_tma,
- * thread_per_subsection (1: one thread per subsection, small power-of-two S; 0: one warp)}. */
+ * pooled (1: pooled kernel on the tiled lattice layout -- one warp per group of 32 subsections,
+ * small power-of-two S; 0: one warp per subsection on the row-major layout)}. */
 int  cpm_get_launch_info(cpm_ctx *ctx, uint64_t out[6]);
 /* Average device time (ms) of the sweep kernel launches since the last call with reset != 0,
  * measured with CUDA events on the context's stream when timing is enabled. */

@@ -12,6 +12,7 @@ import numpy as np
 from . import build as _build
 
 MODE_DETERMINISTIC, MODE_LIVE_ATOMICS = 0, 1
+FLAG_WARP_KERNEL, FLAG_NO_TMA = 1, 2
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "cpm.h")
 
@@ -34,6 +35,7 @@ class _Params(C.Structure):
         ("subsection", C.c_int32), ("attempts_per_activation", C.c_int32),
         ("mode", C.c_int32), ("max_cells", C.c_uint32),
         ("device", C.c_int32), ("stream", C.c_void_p),
+        ("flags", C.c_uint32),
     ]
 
 
@@ -114,7 +116,7 @@ class CPM:
     def __init__(self, dims, J, lambda_V=None, target_V=None, lambda_P=None, target_P=None,
                  lambda_act=None, max_act=None, T=20.0, seed=1, subsection=0,
                  attempts_per_activation=0, mode=MODE_DETERMINISTIC, max_cells=0,
-                 periodic=(0, 0, 0), device=None, stream=None):
+                 periodic=(0, 0, 0), device=None, stream=None, flags=0):
         import torch  # device memory + streams only
         L = load_library()
         if not torch.cuda.is_available():
@@ -158,6 +160,7 @@ class CPM:
         p.max_cells = self.max_cells
         p.device = self.device
         p.stream = C.c_void_p(int(stream))
+        p.flags = int(flags)
         h = C.c_void_p()
         rc = L.cpm_create(C.byref(p), C.byref(h))
         if rc != 0:
@@ -244,7 +247,7 @@ class CPM:
         self._chk(self._L.cpm_get_launch_info(self._h, out.ctypes.data))
         return {"launches": int(out[0]), "sweep_launches": int(out[1]), "warps_per_cta": int(out[2]),
                 "smem_bytes_per_cta": int(out[3]), "uses_tma": bool(out[4]),
-                "thread_per_subsection": bool(out[5])}
+                "pooled": bool(out[5])}
 
     def set_kernel_timing(self, enabled=True):
         self._chk(self._L.cpm_set_kernel_timing(self._h, 1 if enabled else 0))

@@ -30,8 +30,19 @@ struct __align__(16) TypeParams {  // per cell type, Tables 1-3 of the paper
   int32_t lamA, maxA, pad0, pad1;
 };
 
+// Tiled lattice layout of the pooled kernel (cpm_pool_kernel.cuh): every subsection owns a tile of (S+2)^d
+// words (its sites + a halo replicated from its neighbours); the tiles of 32 same-colour subsections
+// (consecutive in the active-subsection order w) are interleaved: word j of subsection w of colour col at
+// base[col] + (((w >> 5) * TW + j) << 5) + (w & 31).
+struct TileLayout {
+  uint32_t *tiles;
+  unsigned long long base[8];   // word offset of the first group of each colour
+  int nact[8][3];               // subsections of that colour per axis
+  int S, TW;
+};
+
 struct SweepParams {
-  uint32_t *lat;            // pitched lattice words
+  uint32_t *lat;            // pitched lattice words (warp kernel; null with the tiled layout)
   uint8_t *act;             // pitched Act bytes (may be null)
   long long pitch;          // words per lattice row
   long long apitch;         // bytes per Act row
@@ -62,6 +73,12 @@ struct SweepParams {
   unsigned long long *sumx, *sumy, *sumz;
   unsigned long long *counters;      // [COUNTER_SLOTS][2] evaluated, accepted
   int *error_flag;
+  // pooled kernel
+  TileLayout tl;
+  unsigned long long grp_base;       // word offset of this colour's first group
+  uint32_t *ovf_keys;                // spill slots of the own-delta tables: [ovf_cap][PK_SPILL]
+  unsigned long long *ovf_dvp;
+  int *ovf_count; int ovf_cap;
 };
 
 // ------------------------------------------------------------------ PTX wrappers ----------

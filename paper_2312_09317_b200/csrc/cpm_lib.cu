@@ -4,11 +4,12 @@
 // usable CUDA device every entry point that needs one returns CPM_ERR_CUDA.
 #include "../../include/cpm.h"
 #include "cpm_device.cuh"
-#include "cpm_thread_kernel.cuh"
+#include "cpm_pool_kernel.cuh"
 
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <new>
 #include <string>
 #include <vector>
 
@@ -41,10 +42,13 @@ struct cpm_ctx {
   size_t cta_smem = 0;
   bool use_tma = true;
   SweepFn fn = nullptr;
-  bool thread_kernel = false;   // one thread per subsection (small power-of-two S), else one warp
+  bool pooled = false;          // pooled kernel on the tiled layout (small power-of-two S), else one warp per subsection
   ThreadFn tfn = nullptr;
+  unsigned long long n_act_col[8] = {0}, grp_col[8] = {0};   // active subsections / groups of 32 per colour
+  size_t tile_words = 0;
   SweepParams sp;        // template of the launch parameters
   CUtensorMap tm_lat;
+  uint32_t *tl_tiles() const { return sp.tl.tiles; }
 
   // device state
   uint32_t *lat = nullptr;
@@ -56,6 +60,12 @@ struct cpm_ctx {
   int32_t *J_dev = nullptr, *D_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
   TypeParams *types_dev = nullptr;
   uint32_t *thr_dev = nullptr;
+  uint32_t *ovf_keys = nullptr;
+  unsigned long long *ovf_dvp = nullptr;
+  int *ovf_count = nullptr;
+  // staging buffers for host-pointer I/O, kept between calls
+  void *stage_a = nullptr, *stage_b = nullptr, *stage_c = nullptr;
+  size_t stage_a_cap = 0, stage_b_cap = 0, stage_c_cap = 0;
 
   std::vector<uint32_t> thr;
   long long Hmax = 0;
@@ -99,21 +109,22 @@ SweepFn pick_kernel(int d, bool act, bool live, int nsets) {
 }
 
 template <int DIM, int S>
-ThreadFn pick_thread_flags(bool act, bool live) {
-  if (act) return live ? (ThreadFn)sweep_thread_kernel<DIM, S, true, true> : (ThreadFn)sweep_thread_kernel<DIM, S, true, false>;
-  return live ? (ThreadFn)sweep_thread_kernel<DIM, S, false, true> : (ThreadFn)sweep_thread_kernel<DIM, S, false, false>;
+ThreadFn pick_pool_flags(bool act, bool live, int nT, size_t *smem) {
+  *smem = PSmem<DIM, S>::bytes(nT);
+  if (act) return live ? (ThreadFn)sweep_pool_kernel<DIM, S, true, true> : (ThreadFn)sweep_pool_kernel<DIM, S, true, false>;
+  return live ? (ThreadFn)sweep_pool_kernel<DIM, S, false, true> : (ThreadFn)sweep_pool_kernel<DIM, S, false, false>;
 }
-// one thread per subsection: 3D S = 2, 4; 2D S = 2, 4, 8, 16
-ThreadFn pick_thread_kernel(int d, int S, bool act, bool live) {
+// pooled kernel: 3D S = 2, 4; 2D S = 2, 4, 8, 16
+ThreadFn pick_pool_kernel(int d, int S, bool act, bool live, int nT, size_t *smem) {
   if (d == 3) {
-    if (S == 2) return pick_thread_flags<3, 2>(act, live);
-    if (S == 4) return pick_thread_flags<3, 4>(act, live);
+    if (S == 2) return pick_pool_flags<3, 2>(act, live, nT, smem);
+    if (S == 4) return pick_pool_flags<3, 4>(act, live, nT, smem);
     return nullptr;
   }
-  if (S == 2) return pick_thread_flags<2, 2>(act, live);
-  if (S == 4) return pick_thread_flags<2, 4>(act, live);
-  if (S == 8) return pick_thread_flags<2, 8>(act, live);
-  if (S == 16) return pick_thread_flags<2, 16>(act, live);
+  if (S == 2) return pick_pool_flags<2, 2>(act, live, nT, smem);
+  if (S == 4) return pick_pool_flags<2, 4>(act, live, nT, smem);
+  if (S == 8) return pick_pool_flags<2, 8>(act, live, nT, smem);
+  if (S == 16) return pick_pool_flags<2, 16>(act, live, nT, smem);
   return nullptr;
 }
 
@@ -127,35 +138,38 @@ int grid_for(long long n, int block = 256) {
 
 int roundup(int v, int m) { return (v + m - 1) / m * m; }
 
-// a device pointer to n elements of T holding the caller's data: the caller's own pointer when it
-// is already on the device, otherwise a temporary copy
-template <class T>
-struct Staged {
-  T *p = nullptr;
-  bool owned = false;
-  ~Staged() { if (owned && p) cudaFree(p); }
-};
-template <class T>
-cudaError_t stage_in(Staged<T> &s, const T *src, size_t n, int on_device, cudaStream_t st) {
-  if (!src) return cudaSuccess;
-  if (on_device) { s.p = const_cast<T *>(src); return cudaSuccess; }
-  cudaError_t e = cudaMalloc(&s.p, n * sizeof(T));
-  if (e != cudaSuccess) return e;
-  s.owned = true;
-  return cudaMemcpyAsync(s.p, src, n * sizeof(T), cudaMemcpyHostToDevice, st);
-}
-template <class T>
-cudaError_t stage_out_begin(Staged<T> &s, T *dst, size_t n, int on_device) {
-  if (!dst) return cudaSuccess;
-  if (on_device) { s.p = dst; return cudaSuccess; }
-  cudaError_t e = cudaMalloc(&s.p, n * sizeof(T));
-  if (e == cudaSuccess) s.owned = true;
+// a device pointer to n elements of T holding the caller's data: the caller's own pointer when it is
+// already on the device, otherwise one of the context's staging buffers (kept between calls)
+cudaError_t stage_reserve(void **buf, size_t *cap, size_t bytes) {
+  if (*cap >= bytes) return cudaSuccess;
+  if (*buf) { cudaFree(*buf); *buf = nullptr; *cap = 0; }
+  cudaError_t e = cudaMalloc(buf, bytes);
+  if (e == cudaSuccess) *cap = bytes;
   return e;
 }
 template <class T>
-cudaError_t stage_out_end(Staged<T> &s, T *dst, size_t n, int on_device, cudaStream_t st) {
+cudaError_t stage_in(T **out, void **buf, size_t *cap, const T *src, size_t n, int on_device, cudaStream_t st) {
+  *out = nullptr;
+  if (!src) return cudaSuccess;
+  if (on_device) { *out = const_cast<T *>(src); return cudaSuccess; }
+  cudaError_t e = stage_reserve(buf, cap, n * sizeof(T));
+  if (e != cudaSuccess) return e;
+  *out = reinterpret_cast<T *>(*buf);
+  return cudaMemcpyAsync(*buf, src, n * sizeof(T), cudaMemcpyHostToDevice, st);
+}
+template <class T>
+cudaError_t stage_out_begin(T **out, void **buf, size_t *cap, T *dst, size_t n, int on_device) {
+  *out = nullptr;
+  if (!dst) return cudaSuccess;
+  if (on_device) { *out = dst; return cudaSuccess; }
+  cudaError_t e = stage_reserve(buf, cap, n * sizeof(T));
+  if (e == cudaSuccess) *out = reinterpret_cast<T *>(*buf);
+  return e;
+}
+template <class T>
+cudaError_t stage_out_end(T *staged, T *dst, size_t n, int on_device, cudaStream_t st) {
   if (!dst || on_device) return cudaSuccess;
-  return cudaMemcpyAsync(dst, s.p, n * sizeof(T), cudaMemcpyDeviceToHost, st);
+  return cudaMemcpyAsync(dst, staged, n * sizeof(T), cudaMemcpyDeviceToHost, st);
 }
 
 int make_tensor_map(cpm_ctx *c, CUtensorMap *tm, CUtensorMapDataType dt, int elem, void *base, long long pitch_elems,
@@ -191,6 +205,8 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->lat); cudaFree(c->act); cudaFree(c->liveVP); cudaFree(c->snapVP); cudaFree(c->sumx); cudaFree(c->sumy);
   cudaFree(c->sumz); cudaFree(c->counters); cudaFree(c->error_flag); cudaFree(c->mcs_dev); cudaFree(c->J_dev); cudaFree(c->D_dev);
   cudaFree(c->log_dev); cudaFree(c->exp_dev); cudaFree(c->types_dev); cudaFree(c->thr_dev);
+  cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
+  cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
 }
 
@@ -198,13 +214,21 @@ void free_all(cpm_ctx *c) {
 
 extern "C" {
 
-int cpm_create(const cpm_params *p, cpm_ctx **out) {
+// every entry point catches allocation failures of the host containers: nothing throws through the C ABI
+#define CPM_GUARD_BEGIN try {
+#define CPM_GUARD_END(ctx)                                                     \
+  } catch (const std::bad_alloc &) { return fail(ctx, CPM_ERR_OOM, "host allocation failed"); } \
+  catch (...) { return fail(ctx, CPM_ERR_STATE, "unexpected host exception"); }
+
+static int create_impl(const cpm_params *p, cpm_ctx **out) {
   if (!p || !out) return CPM_ERR_ARG;
   *out = nullptr;
   if (p->ndim != 2 && p->ndim != 3) return CPM_ERR_DIMS;
   if (p->neighbourhood != CPM_MOORE) return CPM_ERR_UNSUPPORTED;
   if (p->n_types < 1 || p->n_types > 127 || !p->J) return CPM_ERR_ARG;
   if (!(p->T >= 0)) return CPM_ERR_ARG;
+  // the Metropolis table has floor(T 32 ln 2) + 1 entries: a finite T above 2^20 is outside this build
+  if (!std::isinf(p->T) && p->T > 1048576.0) return CPM_ERR_UNSUPPORTED;
   if (p->mode != CPM_MODE_DETERMINISTIC && p->mode != CPM_MODE_LIVE_ATOMICS) return CPM_ERR_ARG;
   if (p->max_cells >= (1u << 24)) return CPM_ERR_UNSUPPORTED;
   const int d = p->ndim, nT = p->n_types;
@@ -218,15 +242,16 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   for (int i = 0; i < nT; ++i) {
     if (p->max_act && (p->max_act[i] < 0 || p->max_act[i] > 255)) return CPM_ERR_ARG;
     if (p->lambda_act && p->lambda_act[i] < 0) return CPM_ERR_ARG;
-    // ranges that keep the 32x32->64 products of the dH assembly exact
+    // ranges that keep the 32x32->64 products and the int32 sums of the dH assembly exact
     if (p->lambda_P && (p->lambda_P[i] > (1 << 24) || p->lambda_P[i] < -(1 << 24))) return CPM_ERR_ARG;
+    if (p->lambda_V && (p->lambda_V[i] > (1 << 30) || p->lambda_V[i] < -(1 << 30))) return CPM_ERR_ARG;
     if (p->max_act && p->max_act[i] != 0) any_act = true;
   }
 
   // ---- checkerboard scheduler (a1): subsection edge S, attempts per activation k ----
   int S = p->subsection;
   if (S == 0) {
-    S = (d == 2) ? 8 : 4;   // small enough for one thread per subsection (the paper's granularity, Fig 4)
+    S = (d == 2) ? 8 : 4;   // small subsections: many independent chains per warp (R4)
     auto divides = [&](int s) { for (int a = 0; a < d; ++a) if (p->dims[a] % s) return false; return true; };
     while (S > 2 && !divides(S)) S /= 2;
   }
@@ -263,11 +288,12 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   c->act_enabled = any_act;
   c->nsets = (sites <= 512) ? 1 : 4;
   // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
-  c->use_tma = getenv("CPM_NO_TMA") == nullptr && (S % 4 == 0);
-  c->tfn = (nT <= 8 && getenv("CPM_WARP_KERNEL") == nullptr)
-               ? pick_thread_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS) : nullptr;
-  c->thread_kernel = c->tfn != nullptr;
-  if (c->thread_kernel) c->use_tma = false;
+  c->use_tma = !(p->flags & CPM_FLAG_NO_TMA) && (S % 4 == 0);
+  size_t pool_smem = 0;
+  c->tfn = (nT <= 8 && !(p->flags & CPM_FLAG_WARP_KERNEL))
+               ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, nT, &pool_smem) : nullptr;
+  c->pooled = c->tfn != nullptr;
+  if (c->pooled) c->use_tma = true;   // one bulk copy per group of 32 tiles
 
   // ---- tile geometry (a2) ----
   SweepParams &sp = c->sp;
@@ -281,7 +307,7 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   sp.tile_bytes = sp.TX * sp.TY * sp.TZ * 4;
   sp.act_tile_bytes = c->act_enabled ? sp.AX * sp.TY * sp.TZ : 0;
   sp.warp_smem_bytes = roundup(sp.tile_bytes, 128) + roundup(sp.act_tile_bytes, 128);
-  if ((long long)sp.TX * sp.TY * sp.TZ > 65535 || sp.TX > 256 || sp.TY > 256 || sp.AX > 256) {
+  if (!c->pooled && ((long long)sp.TX * sp.TY * sp.TZ > 65535 || sp.TX > 256 || sp.TY > 256 || sp.AX > 256)) {
     delete c;
     return CPM_ERR_UNSUPPORTED;
   }
@@ -292,13 +318,7 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   // per CTA: warp tiles, 64 B of mbarriers, neighbour-offset tables (256 B), type records, J
   const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
   c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
-  if (c->thread_kernel) {
-    // TK_WARPS warps per CTA, each with the interleaved (S+2)^d id tiles of its TK_CH subsections, then the small tables
-    size_t words = 1;
-    for (int a = 0; a < d; ++a) words *= (size_t)(S + 2);
-    c->wpc = TK_WARPS;
-    c->cta_smem = (size_t)TK_WARPS * words * TK_CH * 4 + 256 + 512 + 9 * sizeof(TypeParams) + ((size_t)nT * nT * nT + nT) * 4;
-  }
+  if (c->pooled) { c->wpc = 1; c->cta_smem = pool_smem; }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
   // ---- host-built tables ----
@@ -326,12 +346,30 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     types[i] = t;
   }
   types[nT] = TypeParams{};
-  // adhesion difference table of the thread kernel: D[a][b][n] = J(a,n) - J(b,n), then the diagonal J(t,t)
+  // adhesion difference table of the pooled kernel: D[a][b][n] = J(a,n) - J(b,n), then the diagonal J(t,t)
   std::vector<int32_t> Dtab((size_t)nT * nT * nT + nT);
   for (int a = 0; a < nT; ++a)
     for (int b2 = 0; b2 < nT; ++b2)
       for (int n = 0; n < nT; ++n) Dtab[((size_t)a * nT + b2) * nT + n] = p->J[a * nT + n] - p->J[b2 * nT + n];
   for (int t = 0; t < nT; ++t) Dtab[(size_t)nT * nT * nT + t] = p->J[t * nT + t];
+
+  // ---- tiled layout of the pooled kernel: per colour, groups of 32 tiles of (S+2)^d words ----
+  TileLayout &tl = sp.tl;
+  tl.S = S; tl.TW = 1;
+  for (int a = 0; a < d; ++a) tl.TW *= S + 2;
+  c->tile_words = 0;
+  for (int col = 0; col < 8; ++col) {
+    unsigned long long na = 1;
+    for (int a = 0; a < 3; ++a) {
+      const int bit = (col >> a) & 1;
+      tl.nact[col][a] = (a < d) ? (c->nsub[a] - bit + 1) / 2 : (bit ? 0 : 1);
+      na *= (unsigned long long)tl.nact[col][a];
+    }
+    c->n_act_col[col] = na;
+    c->grp_col[col] = (na + 31ull) / 32ull;
+    tl.base[col] = c->tile_words;
+    c->tile_words += (size_t)(c->grp_col[col] * (unsigned long long)tl.TW * 32ull);
+  }
 
   // ---- device state ----
   const long long pitch = roundup(c->dim[0], 4), apitch = roundup(c->dim[0], 16);
@@ -344,7 +382,18 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
     if (e != cudaSuccess) rc = fail(c, e == cudaErrorMemoryAllocation ? CPM_ERR_OOM : CPM_ERR_CUDA, cudaGetErrorString(e));
     else if (cudaMemsetAsync(*ptr, 0, bytes, c->stream) != cudaSuccess) rc = CPM_ERR_CUDA;
   };
-  alloc((void **)&c->lat, (size_t)pitch * rows * 4);
+  sp.ovf_cap = 0;
+  if (c->pooled) {
+    alloc((void **)&tl.tiles, c->tile_words * 4);
+    if (c->mode == CPM_MODE_DETERMINISTIC) {
+      sp.ovf_cap = 65536;   // spill slots for chains that change more than PK_DCAP distinct cells in one activation
+      alloc((void **)&c->ovf_keys, (size_t)sp.ovf_cap * PK_SPILL * 4);
+      alloc((void **)&c->ovf_dvp, (size_t)sp.ovf_cap * PK_SPILL * 8);
+    }
+    alloc((void **)&c->ovf_count, 4);
+  } else {
+    alloc((void **)&c->lat, (size_t)pitch * rows * 4);
+  }
   if (c->act_enabled) alloc((void **)&c->act, (size_t)apitch * rows);
   alloc((void **)&c->liveVP, ncell * 8);
   if (c->mode == CPM_MODE_DETERMINISTIC) alloc((void **)&c->snapVP, ncell * 8);
@@ -380,18 +429,25 @@ int cpm_create(const cpm_params *p, cpm_ctx **out) {
   sp.logq16 = c->log_dev; sp.expq16 = c->exp_dev;
   sp.snapVP = c->snapVP; sp.liveVP = c->liveVP; sp.sumx = c->sumx; sp.sumy = c->sumy; sp.sumz = c->sumz;
   sp.counters = c->counters; sp.error_flag = c->error_flag;
+  sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
 
   memset(&c->tm_lat, 0, sizeof(CUtensorMap));
-  if (c->use_tma) {
+  if (c->use_tma && !c->pooled) {
     rc = make_tensor_map(c, &c->tm_lat, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, c->lat, pitch, sp.TX);
     if (rc != CPM_OK) { free_all(c); delete c; return rc; }
   }
   c->fn = pick_kernel(d, c->act_enabled, c->mode == CPM_MODE_LIVE_ATOMICS, c->nsets);
-  cudaError_t e = cudaFuncSetAttribute(c->thread_kernel ? (const void *)c->tfn : (const void *)c->fn,
+  cudaError_t e = cudaFuncSetAttribute(c->pooled ? (const void *)c->tfn : (const void *)c->fn,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->cta_smem);
   if (e != cudaSuccess) { free_all(c); delete c; return CPM_ERR_CUDA; }
   *out = c;
   return CPM_OK;
+}
+
+int cpm_create(const cpm_params *p, cpm_ctx **out) {
+  CPM_GUARD_BEGIN
+  return create_impl(p, out);
+  CPM_GUARD_END(nullptr)
 }
 
 int cpm_destroy(cpm_ctx *c) {
@@ -406,54 +462,83 @@ int cpm_destroy(cpm_ctx *c) {
 int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, const uint8_t *cell_type, int on_device) {
   if (!c) return CPM_ERR_ARG;
   if (!ids || !cell_type) return fail(c, CPM_ERR_ARG, "ids and cell_type are required");
+  CPM_GUARD_BEGIN
   CK(cudaSetDevice(c->device));
   const size_t ncell = (size_t)c->max_cells + 1;
-  Staged<uint32_t> sid; Staged<uint8_t> sfz, sct;
-  CK(stage_in(sid, ids, (size_t)c->N, on_device, c->stream));
-  CK(stage_in(sfz, frozen, (size_t)c->N, on_device, c->stream));
   // the type table is validated on the host
   std::vector<uint8_t> ct(ncell);
   if (on_device) { CK(cudaMemcpyAsync(ct.data(), cell_type, ncell, cudaMemcpyDeviceToHost, c->stream)); CK(cudaStreamSynchronize(c->stream)); }
   else memcpy(ct.data(), cell_type, ncell);
   if (ct[0] != 0) return fail(c, CPM_ERR_ARG, "cell 0 must have type 0 (medium)");
   for (size_t i = 0; i < ncell; ++i) if (ct[i] >= c->nT) return fail(c, CPM_ERR_ARG, "cell type out of range");
-  CK(stage_in(sct, cell_type, ncell, on_device, c->stream));
+  const uint32_t *sid; const uint8_t *sfz, *sct;
+  CK(stage_in(const_cast<uint32_t **>(&sid), &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device, c->stream));
+  CK(stage_in(const_cast<uint8_t **>(&sfz), &c->stage_b, &c->stage_b_cap, frozen, (size_t)c->N, on_device, c->stream));
+  CK(stage_in(const_cast<uint8_t **>(&sct), &c->stage_c, &c->stage_c_cap, cell_type, ncell, on_device, c->stream));
 
   CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
-  pack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(sid.p, sfz.p, sct.p, c->max_cells, c->lat, c->sp.pitch, c->dim[0],
-                                                      c->dim[1], c->dim[2], c->error_flag);
-  c->launches++;
   if (c->act) CK(cudaMemsetAsync(c->act, 0, (size_t)c->sp.apitch * c->dim[1] * c->dim[2], c->stream));
   CK(cudaMemsetAsync(c->liveVP, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumx, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumy, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumz, 0, ncell * 8, c->stream));
-  if (c->d == 2)
-    recount_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
-                                                              c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
-  else
-    recount_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
-                                                              c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
-  c->launches++;
+  if (c->pooled) {
+    const TileLayout &tl = c->sp.tl;
+    for (int col = 0; col < (1 << c->d); ++col) {
+      if (c->n_act_col[col] == 0) continue;
+      const long long words = (long long)(c->grp_col[col] * (unsigned long long)tl.TW * 32ull);
+      if (c->d == 2)
+        tile_pack_kernel<2><<<grid_for(words), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
+                                                                     c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
+      else
+        tile_pack_kernel<3><<<grid_for(words), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
+                                                                     c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
+      c->launches++;
+    }
+    for (int col = 0; col < (1 << c->d); ++col) {
+      if (c->n_act_col[col] == 0) continue;
+      const long long thr = (long long)c->grp_col[col] * 32;
+      if (c->d == 2)
+        tile_recount_kernel<2><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz);
+      else
+        tile_recount_kernel<3><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz);
+      c->launches++;
+    }
+  } else {
+    pack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, c->lat, c->sp.pitch, c->dim[0],
+                                                        c->dim[1], c->dim[2], c->error_flag);
+    c->launches++;
+    if (c->d == 2)
+      recount_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
+                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+    else
+      recount_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
+                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+    c->launches++;
+  }
   if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
   CK(cudaGetLastError());
   int rc = check_device_flag(c);
   if (rc != CPM_OK) return rc;
   c->have_lattice = true;
   return CPM_OK;
+  CPM_GUARD_END(c)
 }
 
 int cpm_set_act(cpm_ctx *c, const float *act, int on_device) {
   if (!c || !act) return fail(c, CPM_ERR_ARG, "null argument");
   if (!c->act_enabled) return fail(c, CPM_ERR_UNSUPPORTED, "the Act field needs at least one type with max_act > 0");
   CK(cudaSetDevice(c->device));
-  Staged<float> s;
-  CK(stage_in(s, act, (size_t)c->N, on_device, c->stream));
-  CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
-  act_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s.p, c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], c->error_flag);
+  int rc = check_device_flag(c);   // a pending error of an earlier cpm_step is reported, not discarded
+  if (rc != CPM_OK) return rc;
+  const float *s;
+  CK(stage_in(const_cast<float **>(&s), &c->stage_a, &c->stage_a_cap, act, (size_t)c->N, on_device, c->stream));
+  act_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s, c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], c->error_flag);
   c->launches++;
   CK(cudaGetLastError());
-  return check_device_flag(c);
+  rc = check_device_flag(c);
+  if (rc != CPM_OK) CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));   // bad input: reported once, state stays usable
+  return rc;
 }
 
 int cpm_set_mcs(cpm_ctx *c, uint32_t mcs) {
@@ -468,6 +553,7 @@ int cpm_set_mcs(cpm_ctx *c, uint32_t mcs) {
 int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
   if (!c) return CPM_ERR_ARG;
   if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CPM_GUARD_BEGIN
   CK(cudaSetDevice(c->device));
   const int ncol = 1 << c->d;
   const size_t ncell = (size_t)c->max_cells + 1;
@@ -484,16 +570,18 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
         }
         if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
         sp.n_active = n_active;
-        const unsigned long long per_cta = c->thread_kernel ? (unsigned long long)(TK_CH * TK_WARPS) : (unsigned long long)c->wpc;
+        sp.grp_base = sp.tl.base[col];
+        const unsigned long long per_cta = c->pooled ? 32ull : (unsigned long long)c->wpc;
         const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
         if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
+        if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, c->stream));
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (c->timing) {
           while (c->ev_pool.size() < c->ev_used + 2) { cudaEvent_t e; CK(cudaEventCreate(&e)); c->ev_pool.push_back(e); }
           e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
           CK(cudaEventRecord(e0, c->stream));
         }
-        if (c->thread_kernel) c->tfn<<<(unsigned)grid, 32 * TK_WARPS, c->cta_smem, c->stream>>>(sp);
+        if (c->pooled) c->tfn<<<(unsigned)grid, 32, c->cta_smem, c->stream>>>(sp);
         else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
         if (c->timing) CK(cudaEventRecord(e1, c->stream));
         c->launches++; c->sweep_launches++;
@@ -511,14 +599,20 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
   }
   CK(cudaGetLastError());
   return CPM_OK;
+  CPM_GUARD_END(c)
 }
 
 int cpm_get_lattice(cpm_ctx *c, uint32_t *ids, int on_device) {
   if (!c || !ids) return fail(c, CPM_ERR_ARG, "null argument");
   CK(cudaSetDevice(c->device));
-  Staged<uint32_t> s;
-  CK(stage_out_begin(s, ids, (size_t)c->N, on_device));
-  unpack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], s.p);
+  uint32_t *s;
+  CK(stage_out_begin(&s, &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device));
+  if (c->pooled) {
+    if (c->d == 2) tile_unpack_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s);
+    else tile_unpack_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s);
+  } else {
+    unpack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], s);
+  }
   c->launches++;
   CK(cudaGetLastError());
   CK(stage_out_end(s, ids, (size_t)c->N, on_device, c->stream));
@@ -528,9 +622,9 @@ int cpm_get_lattice(cpm_ctx *c, uint32_t *ids, int on_device) {
 int cpm_get_act(cpm_ctx *c, float *act, int on_device) {
   if (!c || !act) return fail(c, CPM_ERR_ARG, "null argument");
   CK(cudaSetDevice(c->device));
-  Staged<float> s;
-  CK(stage_out_begin(s, act, (size_t)c->N, on_device));
-  act_get_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], s.p);
+  float *s;
+  CK(stage_out_begin(&s, &c->stage_a, &c->stage_a_cap, act, (size_t)c->N, on_device));
+  act_get_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], s);
   c->launches++;
   CK(cudaGetLastError());
   CK(stage_out_end(s, act, (size_t)c->N, on_device, c->stream));
@@ -542,11 +636,11 @@ int cpm_get_cell_stats(cpm_ctx *c, uint32_t *volume, uint32_t *perimeter, uint64
   if (!c) return CPM_ERR_ARG;
   CK(cudaSetDevice(c->device));
   const size_t n = (size_t)c->max_cells + 1;
-  Staged<uint32_t> sv, spm;
-  CK(stage_out_begin(sv, volume, n, on_device));
-  CK(stage_out_begin(spm, perimeter, n, on_device));
+  uint32_t *sv, *spm;
+  CK(stage_out_begin(&sv, &c->stage_b, &c->stage_b_cap, volume, n, on_device));
+  CK(stage_out_begin(&spm, &c->stage_c, &c->stage_c_cap, perimeter, n, on_device));
   if (volume || perimeter) {
-    stats_unpack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->liveVP, (long long)n, sv.p, spm.p);
+    stats_unpack_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->liveVP, (long long)n, sv, spm);
     c->launches++;
     CK(cudaGetLastError());
   }
@@ -562,8 +656,8 @@ int cpm_get_cell_stats(cpm_ctx *c, uint32_t *volume, uint32_t *perimeter, uint64
 int cpm_get_counters(cpm_ctx *c, uint64_t out[4]) {
   if (!c || !out) return fail(c, CPM_ERR_ARG, "null argument");
   CK(cudaSetDevice(c->device));
-  std::vector<unsigned long long> h(COUNTER_SLOTS * 2);
-  CK(cudaMemcpyAsync(h.data(), c->counters, h.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+  unsigned long long h[COUNTER_SLOTS * 2];
+  CK(cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   uint64_t ev = 0, ac = 0;
   for (int i = 0; i < COUNTER_SLOTS; ++i) { ev += h[2 * i]; ac += h[2 * i + 1]; }
@@ -588,7 +682,7 @@ int64_t cpm_get_threshold_table(cpm_ctx *c, uint32_t *thr, uint64_t cap) {
 int cpm_get_launch_info(cpm_ctx *c, uint64_t out[6]) {
   if (!c || !out) return CPM_ERR_ARG;
   out[0] = c->launches; out[1] = c->sweep_launches; out[2] = (uint64_t)c->wpc; out[3] = (uint64_t)c->cta_smem;
-  out[4] = c->use_tma ? 1 : 0; out[5] = c->thread_kernel ? 1 : 0;
+  out[4] = c->use_tma ? 1 : 0; out[5] = c->pooled ? 1 : 0;
   return CPM_OK;
 }
 

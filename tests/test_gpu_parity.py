@@ -19,9 +19,9 @@ def pk():
     return m
 
 
-def _pair(pk, ob, cfg, mode=0, **over):
+def _pair(pk, ob, cfg, mode=0, flags=0, **over):
     p = dict(cfg["params"]); p.update(over)
-    g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], mode=mode, **p)
+    g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], mode=mode, flags=flags, **p)
     o = ob.Oracle(cfg["dims"], max_cells=cfg["max_cells"], mode=mode, **p)
     g.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
     o.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
@@ -85,39 +85,38 @@ def test_C1_bit_exact_every_mcs(pk, oracle_mod):
     cfg = ci.make_config("C1")
     g, o = _run(pk, oracle_mod, cfg, 100, 1)
     assert g.get_schedule() == {"S": 16, "k": 256, "phase_steps_per_mcs": 4}
-    assert g.get_launch_info()["thread_per_subsection"]
+    assert g.get_launch_info()["pooled"], g.get_launch_info()
 
 
-def test_C1_warp_kernel_bit_exact(pk, oracle_mod, monkeypatch):
-    """The same config through the warp-per-subsection kernel (TMA staging)."""
+def test_C1_warp_kernel_bit_exact(pk, oracle_mod):
+    """The same config through the warp-per-subsection kernel (TMA tile staging)."""
     import cpm_inputs as ci
-    monkeypatch.setenv("CPM_WARP_KERNEL", "1")
     cfg = ci.make_config("C1")
-    g, o = _run(pk, oracle_mod, cfg, 30, 5)
+    g, o = _run(pk, oracle_mod, cfg, 30, 5, flags=pk.FLAG_WARP_KERNEL)
     info = g.get_launch_info()
-    assert info["uses_tma"] and not info["thread_per_subsection"]
+    assert info["uses_tma"] and not info["pooled"]
 
 
 @pytest.mark.parametrize("name,dims,act", [("C2", (64, 64, 64), False), ("C3", (64, 64, 64), True),
                                            ("C4", (80, 80, 80), True), ("C4", (72, 40, 24), True)])
-def test_thread_kernel_S4_bit_exact(pk, oracle_mod, name, dims, act):
-    """The bench's launch configuration: one thread per 4^3 subsection (k = 64), scaled C2/C3/C4."""
+def test_pooled_kernel_S4_bit_exact(pk, oracle_mod, name, dims, act):
+    """The bench launch configuration: 4^3 subsections (k = 64) in the pooled kernel, scaled C2/C3/C4."""
     import cpm_inputs as ci
     cfg = ci.make_config(name, dims=dims, subsection=4)
     g, o = _run(pk, oracle_mod, cfg, 12, 3, act=act)
     assert g.get_schedule() == {"S": 4, "k": 64, "phase_steps_per_mcs": 8}
-    assert g.get_launch_info()["thread_per_subsection"]
+    assert g.get_launch_info()["pooled"]
 
 
-def test_default_schedule_is_thread_per_subsection(pk, oracle_mod):
+def test_default_schedule_runs_the_pooled_kernel(pk, oracle_mod):
     """subsection = 0: both sides choose S = 4 (3D) / 8 (2D)."""
     import cpm_inputs as ci
     cfg = ci.make_config("C4", dims=(40, 40, 40))
     g, o = _run(pk, oracle_mod, cfg, 4, 2, act=True, subsection=0)
-    assert g.get_schedule()["S"] == 4 and g.get_launch_info()["thread_per_subsection"]
+    assert g.get_schedule()["S"] == 4 and g.get_launch_info()["pooled"]
     cfg = ci.make_config("C5", dims=(64, 48))
     g, o = _run(pk, oracle_mod, cfg, 4, 2, subsection=0)
-    assert g.get_schedule()["S"] == 8 and g.get_launch_info()["thread_per_subsection"]
+    assert g.get_schedule()["S"] == 8 and g.get_launch_info()["pooled"]
 
 
 def test_C2_scaled_bit_exact(pk, oracle_mod):
@@ -215,7 +214,7 @@ def test_resume_is_exact_on_device(pk, oracle_mod):
         np.testing.assert_array_equal(g2.get_cell_stats()[k], v)
 
 
-def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod, monkeypatch):
+def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     """Inputs/outputs as device tensors (on_device=1); and the non-TMA staging path."""
     import torch
     import cpm_inputs as ci
@@ -230,9 +229,8 @@ def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod, monkeypatc
     out = torch.empty(gd.N, dtype=torch.int32, device="cuda")
     gd.get_lattice(out)
     np.testing.assert_array_equal(out.cpu().numpy().astype(np.uint32).reshape(o.shape), o.get_lattice())
-    monkeypatch.setenv("CPM_NO_TMA", "1")
-    gm = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], **cfg["params"])
-    assert not gm.get_launch_info()["uses_tma"]
+    gm = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], flags=pk.FLAG_NO_TMA, **cfg["params"])
+    assert not gm.get_launch_info()["uses_tma"] and not gm.get_launch_info()["pooled"]
     gm.set_lattice(cfg["ids"], None, cfg["cell_type"])
     gm.step(3)
     np.testing.assert_array_equal(gm.get_lattice(), o.get_lattice())
@@ -363,7 +361,7 @@ def test_C4_256_cubed_scheduler_choice_bit_exact(pk, oracle_mod):
     cfg = ci.make_config("C4", dims=(256, 256, 256))
     g, o = _run(pk, oracle_mod, cfg, 3, 1, act=True, subsection=0)
     assert g.get_schedule() == {"S": 4, "k": 64, "phase_steps_per_mcs": 8}
-    assert g.get_launch_info()["thread_per_subsection"]
+    assert g.get_launch_info()["pooled"]
 
 
 def test_C4_full_size_properties(pk):
@@ -386,7 +384,7 @@ def test_C4_full_size_properties(pk):
         return g, g.get_lattice()
 
     g, lat = run()
-    assert g.get_launch_info()["thread_per_subsection"] and g.get_schedule()["S"] == 4
+    assert g.get_launch_info()["pooled"] and g.get_schedule()["S"] == 4
     st = g.get_cell_stats()
     c = g.get_counters()
     assert c["attempts"] == 2 * 1024 ** 3 and 0 < c["accepted"] < c["evaluated"] < c["attempts"]

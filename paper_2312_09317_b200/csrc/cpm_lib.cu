@@ -318,7 +318,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   // per CTA: warp tiles, 64 B of mbarriers, neighbour-offset tables (256 B), type records, J
   const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
   c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
-  if (c->pooled) { c->wpc = 1; c->cta_smem = pool_smem; }
+  if (c->pooled) { c->wpc = PK_WARPS; c->cta_smem = pool_smem; }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
   // ---- host-built tables ----
@@ -581,7 +581,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
           e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
           CK(cudaEventRecord(e0, c->stream));
         }
-        if (c->pooled) c->tfn<<<(unsigned)grid, 32, c->cta_smem, c->stream>>>(sp);
+        if (c->pooled) c->tfn<<<(unsigned)grid, PK_THREADS, c->cta_smem, c->stream>>>(sp);
         else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
         if (c->timing) CK(cudaEventRecord(e1, c->stream));
         c->launches++; c->sweep_launches++;

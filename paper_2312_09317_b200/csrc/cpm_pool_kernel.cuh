@@ -1,5 +1,5 @@
 // cpm_pool_kernel.cuh -- sm_100a sweep kernel for small power-of-two subsections (3D S = 2, 4; 2D S = 2..16):
-// one WARP owns a GROUP of 32 active checkerboard subsections ("chains") and evaluates their copy
+// one CTA of four warps owns a GROUP of 32 active checkerboard subsections ("chains") and evaluates their copy
 // attempts SPECULATIVELY IN PARALLEL, pooled over the 32 chains, while keeping the exact sequential
 // semantics of every chain (the attempts of one subsection are applied in order).
 //
@@ -9,22 +9,25 @@
 // contiguous block of TW * 128 bytes, so
 //   a2  ONE bulk asynchronous copy (TMA, cp.async.bulk -> SASS UBLKCP) stages the tiles of all 32 chains,
 //       already in the bank-conflict-free order the kernel wants (bank = chain); completion on an mbarrier
-//       while the warp draws its first random numbers;
+//       while the CTA draws its first random numbers;
 //   a10 there is no tile write-back: an accepted copy stores its word to the home tile and to the (at most
 //       2^d - 1) halo replicas in the neighbouring subsections' tiles, which are inactive in this phase-step.
-// Per chunk of 16 attempts per chain (512 attempts per warp):
-//   a3  every lane draws 4 Philox4x32-10 blocks for ITS chain (counter (a>>2, b, 2p, mcs), reading S15) and
-//       decodes 16 proposals;
-//   a4  the owner lane screens them against its tile (same cell / frozen); ballot + popc compact the
-//       surviving attempts of all chains into one queue, ordered by (attempt, chain);
-//   a5-a8 the queue is evaluated 32 items at a time, one lane per item whatever chain it belongs to: neighbour
-//       census from the chain's tile column, per-cell state (snapshot + the chain's own deltas / live),
-//       dH in int64, Act geometric means pooled again over the lanes that need one, Metropolis;
-//   a9  for every chain the FIRST accepted attempt in sequence order is committed (shared-memory atomicMin);
-//       everything evaluated before it was evaluated on the true state and is final, the attempts after it
-//       are screened and evaluated again in the next round on the new state.  Rounds per chunk = 1 + the
-//       largest number of accepted copies any chain has in the chunk, so the result equals k sequential
-//       attempts per subsection exactly;
+// Per chunk of 16 attempts per chain (512 attempts per CTA), thread (warp w, lane c) owns attempts 4w..4w+3 of
+// chain c:
+//   a3  one Philox4x32-10 block per thread (counter (a>>2, b, 2p, mcs), reading S15) -> 4 proposals;
+//   a4  the owner thread screens them against its chain's tile (same cell / frozen); ballot + popc + one
+//       shared-memory atomic per warp compact the surviving attempts of all chains into one queue;
+//   a5-a7 the queue is evaluated one item per thread whatever chain it belongs to: neighbour census from the
+//       chain's tile column, per-cell state (snapshot + the chain's own deltas / live), dH in int64;
+//   Act the geometric means (Eq 9) the items need are requested through a second queue and computed one per
+//       thread (a request is dropped when the centre's own Act value is 0: any zero makes the mean 0);
+//   a8  Metropolis; an accepted item enters a shared-memory atomicMin on its chain's slot, keyed by the attempt
+//       index, so the FIRST accepted attempt of every chain wins;
+//   a9  nothing is committed before every item of the round is decided: all of them saw the state at the start
+//       of the round, what lies before a chain's winner is final, the winner is committed, and the attempts
+//       after it are screened and evaluated again in the next round on the new state.  Rounds per chunk =
+//       1 + the largest number of accepted copies any chain has in the chunk, so the result equals k
+//       sequential attempts per subsection exactly;
 //   a10 the integer deltas of a committed copy go to the live per-cell arrays at once as 64-bit reductions.
 // Nothing here is shared with oracle/.
 #pragma once
@@ -32,11 +35,13 @@
 
 namespace cpm {
 
-constexpr int PK_CHUNK = 16;                 // attempts per chain between two pooled evaluations
+constexpr int PK_WARPS = 4;                  // warps per CTA = per group of 32 chains
+constexpr int PK_THREADS = 32 * PK_WARPS;
+constexpr int PK_CHUNK = 16;                 // attempts per chain between two pooled evaluations (4 per thread)
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 4;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
-constexpr int PK_GMQ = 64;                   // geometric means requested by one batch of 32 items (2 per item)
+constexpr int PK_NOWIN = PK_CHUNK << 10;     // "no accepted attempt": winner slots hold a << 10 | nA << 5 | nB
 constexpr uint32_t CELL_MASK31 = 0x7FFFFFFFu;   // type + id: equal iff same cell
 
 template <int DIM, int S>
@@ -55,27 +60,37 @@ struct PGeom {
   static __host__ __device__ constexpr int dy(int n) { return (idx27(n) / 3) % 3 - 1; }
   static __host__ __device__ constexpr int dz(int n) { return DIM == 3 ? idx27(n) / 9 - 1 : 0; }
   static __host__ __device__ constexpr int noff(int n) { return (dz(n) * T + dy(n)) * T + dx(n); }   // in tile words
+  // neighbours with offset d (-1 / +1) along axis ax, as a bit mask over n
+  static __host__ __device__ constexpr uint32_t face(int ax, int d) {
+    uint32_t m = 0;
+    for (int n = 0; n < NNB; ++n) if ((ax == 0 ? dx(n) : ax == 1 ? dy(n) : dz(n)) == d) m |= 1u << n;
+    return m;
+  }
 };
 
-// shared-memory carve-up of one CTA (= one warp); D (nT^3 + nT words) comes last
+// shared-memory carve-up of one CTA; D (nT^3 + nT words) comes last
 template <int DIM, int S>
 struct PSmem {
   using G = PGeom<DIM, S>;
   static constexpr int TILE = 0;                                   // uint32 [TW][32]
   static constexpr int PROP = TILE + G::TW * 128;                  // uint16 [16][32]   toff | nb << 9
   static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint16 [16 * 32]  chain | a << 5
-  static constexpr int DKEY = QUEUE + PK_CHUNK * 64;               // uint32 [DCAP][32]
+  static constexpr int GMQ = QUEUE + PK_CHUNK * 64;                // uint2 [2 * PK_THREADS] geometric-mean requests
+  static constexpr int GMOUT = GMQ + 2 * PK_THREADS * 8;           // int [PK_THREADS][2] results
+  static constexpr int DKEY = GMOUT + PK_THREADS * 8;              // uint32 [DCAP][32]
   static constexpr int DDVP = DKEY + PK_DCAP * 128;                // uint64 [DCAP][32]
   static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] entries of the chain's own-delta table
   static constexpr int DSLOT = DN + 128;                           // int [32] spill slot of the chain or -1
-  static constexpr int FIRST = DSLOT + 128;                        // int [32] first accepted attempt of the round
-  static constexpr int BSUB = FIRST + 128;                         // uint32 [32] subsection index b of the chain
+  static constexpr int FIRST = DSLOT + 128;                        // int [32] winner of the round: a << 10 | nA << 5 | nB
+  static constexpr int POS = FIRST + 128;                          // int [32] attempts < pos of the chunk are final
+  static constexpr int BSUB = POS + 128;                           // uint32 [32] subsection index b of the chain
   static constexpr int ORIG = BSUB + 128;                          // int [3][32] lattice origin of the chain
-  static constexpr int GMQ = ORIG + 384;                           // uint2 [PK_GMQ] geometric-mean requests
-  static constexpr int GMOUT = GMQ + PK_GMQ * 8;                   // int [32][2] results
-  static constexpr int NOFF = GMOUT + 256;                         // int [32] neighbour -> tile offset
-  static constexpr int TYPES = NOFF + 128;                         // TypeParams [9]
-  static constexpr int MBAR = TYPES + 9 * 32;                      // uint64
+  static constexpr int NOFF = ORIG + 384;                          // int [32] neighbour -> tile offset (entry NNB = centre = 0)
+  static constexpr int NCODE = NOFF + 128;                         // int [32] neighbour -> (dx+1) | (dy+1) << 2 | (dz+1) << 4
+  static constexpr int TYPES = NCODE + 128;                        // TypeParams [9]
+  static constexpr int LOGQ = TYPES + 9 * 32;                      // int [256] log2 table of the Act term
+  static constexpr int CNT = LOGQ + 1024;                          // int [4]: queue length, request count, redo flag
+  static constexpr int MBAR = CNT + 16;                            // uint64
   static constexpr int DTAB = MBAR + 16;                           // int32 [nT^3 + nT]
   static constexpr size_t bytes(int nT) { return (size_t)DTAB + ((size_t)nT * nT * nT + nT) * 4; }
 };
@@ -91,17 +106,17 @@ __device__ __forceinline__ unsigned long long tile_word(const TileLayout &L, int
   const unsigned long long w = (unsigned long long)(bx >> 1) + (unsigned long long)L.nact[col][0] * ((unsigned long long)(by >> 1) + (unsigned long long)L.nact[col][1] * (unsigned long long)(bz >> 1));
   return L.base[col] + ((((w >> 5) * (unsigned long long)L.TW + (unsigned long long)j) << 5) | (w & 31ull));
 }
-// home word of lattice site (x,y,z), all inside the lattice
+// home word of lattice site (x,y,z), all inside the lattice; S = L.S
 template <int DIM>
-__device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int x, int y, int z) {
-  const int S = L.S, T = S + 2;
+__device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int S, int x, int y, int z) {
+  const int T = S + 2;
   const int bx = x / S, by = y / S, bz = (DIM == 3) ? z / S : 0;
   const int j = (((DIM == 3) ? (z - bz * S + 1) * T : 0) + (y - by * S + 1)) * T + (x - bx * S + 1);
   return tile_word(L, bx, by, bz, j);
 }
 
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
   constexpr int T = G::T, TW = G::TW, NNB = G::NNB;
@@ -109,41 +124,50 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
   unsigned short *prop = reinterpret_cast<unsigned short *>(smem + M::PROP);
   unsigned short *queue = reinterpret_cast<unsigned short *>(smem + M::QUEUE);
+  uint2 *gmq = reinterpret_cast<uint2 *>(smem + M::GMQ);
+  int *gmout = reinterpret_cast<int *>(smem + M::GMOUT);
   uint32_t *dkey = reinterpret_cast<uint32_t *>(smem + M::DKEY);
   unsigned long long *ddvp = reinterpret_cast<unsigned long long *>(smem + M::DDVP);
   int *dn = reinterpret_cast<int *>(smem + M::DN);
   int *dslot = reinterpret_cast<int *>(smem + M::DSLOT);
   int *first = reinterpret_cast<int *>(smem + M::FIRST);
+  int *spos = reinterpret_cast<int *>(smem + M::POS);
   uint32_t *bsub = reinterpret_cast<uint32_t *>(smem + M::BSUB);
   int *orig = reinterpret_cast<int *>(smem + M::ORIG);
-  uint2 *gmq = reinterpret_cast<uint2 *>(smem + M::GMQ);
-  int *gmout = reinterpret_cast<int *>(smem + M::GMOUT);
   int *snoff = reinterpret_cast<int *>(smem + M::NOFF);
+  int *sncode = reinterpret_cast<int *>(smem + M::NCODE);
   TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
+  int *slog = reinterpret_cast<int *>(smem + M::LOGQ);
+  int *cnt = reinterpret_cast<int *>(smem + M::CNT);
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + M::MBAR);
   int32_t *sd = reinterpret_cast<int32_t *>(smem + M::DTAB);
   const int32_t *sdiag = sd + P.nT * P.nT * P.nT;
 
-  const int lane = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const unsigned long long grp_word = P.grp_base + (unsigned long long)blockIdx.x * (unsigned long long)(TW * 32);
   uint32_t *const gtile = P.tl.tiles + grp_word;   // this group's tiles in HBM
 
   // ---- a2: one bulk copy stages the 32 tiles; it overlaps the set-up and the first Philox blocks ----
-  if (lane == 0) { mbar_init(mbar, 1); fence_mbar_init(); }
-  __syncwarp();
-  if (lane == 0) { mbar_expect_tx(mbar, (uint32_t)(TW * 128)); bulk_load(tile, gtile, (uint32_t)(TW * 128), mbar); }
-
-  // small tables
-  {
-    int dx = 0, dy = 0, dz = 0;
-    if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
-    snoff[lane] = (dz * T + dy) * T + dx;
+  if (tid == 0) {
+    mbar_init(mbar, 1); fence_mbar_init();
+    mbar_expect_tx(mbar, (uint32_t)(TW * 128));
+    bulk_load(tile, gtile, (uint32_t)(TW * 128), mbar);
+    cnt[0] = 0; cnt[1] = 0; cnt[2] = 0;
   }
-  for (int i = lane; i < (P.nT + 1) * 8; i += 32) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-  for (int i = lane; i < P.nT * P.nT * P.nT + P.nT; i += 32) sd[i] = P.D[i];
+  // small tables
+  if (tid < 32) {
+    int dx = 0, dy = 0, dz = 0;
+    if (tid < NNB) nb_delta<DIM>(tid, dx, dy, dz);
+    snoff[tid] = (dz * T + dy) * T + dx;
+    sncode[tid] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
+    dn[tid] = 0; dslot[tid] = -1; first[tid] = PK_NOWIN;
+  }
+  for (int i = tid; i < (P.nT + 1) * 8; i += PK_THREADS) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+  for (int i = tid; i < P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
+  if constexpr (ACT) for (int i = tid; i < 256; i += PK_THREADS) slog[i] = P.logq16[i];
 
-  // this lane's chain
+  // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk)
   const unsigned long long w = (unsigned long long)blockIdx.x * 32ull + (unsigned long long)lane;
   const bool active = w < P.n_active;
   uint32_t b = 0;
@@ -158,24 +182,22 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
       b = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
       ox = bx * S; oy = by * S; oz = (DIM == 3) ? bz * S : 0;
     }
-    bsub[lane] = b; orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz;
+    if (wrp == 0) { bsub[lane] = b; orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz; }
   }
-  dn[lane] = 0; dslot[lane] = -1;
   const uint32_t mcs = *P.mcs_ptr;
   const int k = P.k;
   const int nchunk = (k + PK_CHUNK - 1) / PK_CHUNK;
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;
   bool staged = false;
-  const uint32_t *const tcol = tile + lane;   // this lane's own chain column
+  const uint32_t *const tcol = tile + lane;   // this thread's own chain column
 
   for (int ch = 0; ch < nchunk; ++ch) {
-    // ---- a3: 16 proposals of this lane's chain; kept in registers for screening and in shared memory for
-    //      whichever lane evaluates them ----
-    int pr[PK_CHUNK];
-#pragma unroll
-    for (int q = 0; q < PK_CHUNK / 4; ++q) {
-      const uint4 r = philox4x32_10(make_uint4((uint32_t)(ch * (PK_CHUNK / 4) + q), b, 2u * P.p, mcs), P.key0, P.key1);
+    // ---- a3: the 4 proposals this thread owns; kept in registers for screening and in shared memory for
+    //      whichever thread evaluates them ----
+    int pr[4];
+    {
+      const uint4 r = philox4x32_10(make_uint4((uint32_t)(ch * (PK_CHUNK / 4) + wrp), b, 2u * P.p, mcs), P.key0, P.key1);
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const uint32_t wd = pick(r, j);
@@ -183,39 +205,56 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
         const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
         const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
         const int toff = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-        pr[4 * q + j] = toff | (nb << 9);
-        prop[(4 * q + j) * 32 + lane] = (unsigned short)pr[4 * q + j];
+        pr[j] = toff | (nb << 9);
       }
     }
+    const int kk = min(PK_CHUNK, k - ch * PK_CHUNK);   // valid attempts of this chunk
+    __syncthreads();                                   // the previous chunk is finished (prop, pos are free)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) prop[(4 * wrp + j) * 32 + lane] = (unsigned short)pr[j];
+    if (wrp == 0) spos[lane] = active ? 0 : PK_CHUNK;
     if (!staged) {   // first use of the tiles
       while (!mbar_try_wait(mbar, 0)) {}
       staged = true;
     }
-    const int kk = min(PK_CHUNK, k - ch * PK_CHUNK);   // valid attempts of this chunk
-    int pos = active ? 0 : PK_CHUNK;                   // attempts < pos of this lane's chain are final
-    while (true) {
-      // ---- a4: screen the not yet final attempts of the own chain; compact all chains' survivors ----
-      first[lane] = PK_CHUNK;
-      int W = 0;
-#pragma unroll
-      for (int a = 0; a < PK_CHUNK; ++a) {
-        const int toff = pr[a] & 511;
-        const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[a] >> 9]) * 32];
-        const bool in = a >= pos && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
-        const unsigned m = __ballot_sync(FULL, in);
-        if (in) queue[W + __popc(m & lt)] = (unsigned short)(lane | (a << 5));
-        W += __popc(m);
-      }
-      if (W == 0) break;
-      __syncwarp();
+    __syncthreads();
 
-      for (int it = 0; it * 32 < W; ++it) {
-        // ---- a5-a7: one item per lane ----
-        const int qi = it * 32 + lane;
-        bool have = qi < W;
+    while (true) {
+      // ---- a4: screen the not yet final attempts this thread owns; compact all chains' survivors ----
+      if (wrp == 0) first[lane] = PK_NOWIN;   // nobody touches the winner slots before the next barrier
+      const int ps = spos[lane];
+      bool in[4];
+      unsigned m[4];
+      int tot = 0;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int a = 4 * wrp + j;
+        const int toff = pr[j] & 511;
+        const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[j] >> 9]) * 32];
+        in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
+        m[j] = __ballot_sync(FULL, in[j]);
+        tot += __popc(m[j]);
+      }
+      if (tot) {   // warp-uniform
+        int base = 0;
+        if (lane == 0) base = atomicAdd(cnt, tot);
+        base = __shfl_sync(FULL, base, 0);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (in[j]) queue[base + __popc(m[j] & lt)] = (unsigned short)(lane | ((4 * wrp + j) << 5));
+          base += __popc(m[j]);
+        }
+      }
+      __syncthreads();
+      const int W = cnt[0];
+      if (W == 0) break;   // CTA-uniform: cnt[0] is only reset at the end of a round
+
+      for (int sb = 0; sb < W; sb += PK_THREADS) {
+        // ---- a5-a7: one item per thread ----
+        const int qi = sb + tid;
+        const bool have = qi < W;
         const int item = have ? (int)queue[qi] : 0;
         const int c = item & 31, a = item >> 5;
-        have = have && first[c] > a;       // an earlier attempt of this chain was accepted in this round: stale
         const int prc = (int)prop[a * 32 + c];
         const int toff = prc & 511, nb = prc >> 9;
         const int soff = toff + snoff[nb];
@@ -225,21 +264,22 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
         const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
         const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
         long long dH = 0;
-        int dPA = 0, dPB = 0;
+        int nA = 0, nB = 0;
         bool go = false;
         TypeParams pa = st[P.nT], pb = st[P.nT];
+        bool wantA = false, wantB = false;
         if (have) {
           unsigned long long baseA = 0ull, baseB = 0ull;
           if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
           if (Bc != 0) baseB = LIVE ? __ldcg(P.liveVP + Bc) : __ldg(P.snapVP + Bc);
           const int32_t *Drow = sd + (tA * P.nT + tB) * P.nT;
-          int nA = 0, nB = 0, adh = 0;
+          int adh = 0;
 #pragma unroll
           for (int n = 0; n < NNB; ++n) {
-            const uint32_t m = tc[(toff + G::noff(n)) * 32] & CELL_MASK31;
-            nA += (m == mA) ? 1 : 0;
-            nB += (m == mB) ? 1 : 0;
-            adh += Drow[m >> 24];
+            const uint32_t mm = tc[(toff + G::noff(n)) * 32] & CELL_MASK31;
+            nA += (mm == mA) ? 1 : 0;
+            nB += (mm == mB) ? 1 : 0;
+            adh += Drow[mm >> 24];
           }
           // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
           adh += nB * sdiag[tB] - nA * sdiag[tA];
@@ -273,62 +313,78 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
           go = !(Bc != 0 && (uint32_t)(vpB >> 32) <= 1u);   // a cell is never erased (reading S13)
           if (A != 0) pa = st[tA];
           if (Bc != 0) pb = st[tB];                          // medium reads the all-zero row (S3)
-          dPA = NNB - 2 * nA; dPB = 2 * nB - NNB;
+          const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
           const int dva = (int)(uint32_t)(vpA >> 32) - pa.tgtV, dvb = (int)(uint32_t)(vpB >> 32) - pb.tgtV;
           dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
           const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
           dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
+          wantA = go && pa.lamA != 0; wantB = go && pb.lamA != 0;
         }
 
-        // ---- Act: the geometric means (Eq 9) that the items of this batch need, pooled over the lanes ----
+        // ---- Act: request the geometric means (Eq 9) this item needs ----
         if constexpr (ACT) {
-          const bool wantA = have && go && pa.lamA != 0, wantB = have && go && pb.lamA != 0;
           const unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
-          const int nGA = __popc(mwA), nG = nGA + __popc(mwB);
-          if (nG) {
-            if (wantA) gmq[__popc(mwA & lt)] = make_uint2((uint32_t)(soff | (c << 9) | (lane << 14)), mA);
-            if (wantB) gmq[nGA + __popc(mwB & lt)] = make_uint2((uint32_t)(toff | (c << 9) | (lane << 14) | (1 << 19)), mB);
-            __syncwarp();
-            for (int gi = lane; gi < nG; gi += 32) {
+          const int nGA = __popc(mwA), nGw = nGA + __popc(mwB);
+          if (nGw) {   // warp-uniform
+            int base = 0;
+            if (lane == 0) base = atomicAdd(cnt + 1, nGw);
+            base = __shfl_sync(FULL, base, 0);
+            if (wantA) gmq[base + __popc(mwA & lt)] = make_uint2((uint32_t)(soff | (c << 9) | (tid << 14)), mA);
+            if (wantB) gmq[base + nGA + __popc(mwB & lt)] = make_uint2((uint32_t)(toff | (c << 9) | (tid << 14) | (1 << 21)), mB);
+          }
+          __syncthreads();
+          const int nG = cnt[1];
+          if (nG) {   // CTA-uniform
+            for (int gi = tid; gi < nG; gi += PK_THREADS) {
               const uint2 rq = gmq[gi];
               const int ctr = (int)(rq.x & 511u), cc = (int)((rq.x >> 9) & 31u);
               const uint32_t mC = rq.y;
               const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
-              const int ox = orig[cc], oy = orig[32 + cc], oz = orig[64 + cc];
+              // the centre is inside the lattice (its cell is not medium); its coordinates, wrapped
+              int cx = orig[cc] - 1 + px, cy = orig[32 + cc] - 1 + py, cz = (DIM == 3) ? orig[64 + cc] - 1 + pz : 0;
+              cx += (cx < 0) ? P.X : (cx >= P.X) ? -P.X : 0;
+              cy += (cy < 0) ? P.Y : (cy >= P.Y) ? -P.Y : 0;
+              if (DIM == 3) cz += (cz < 0) ? P.Z : (cz >= P.Z) ? -P.Z : 0;
+              // does the neighbourhood reach over the lattice border / out of the halo-1 tile?
+              const bool edge = cx < 1 || cx > P.X - 2 || cy < 1 || cy > P.Y - 2 || (DIM == 3 && (cz < 1 || cz > P.Z - 2));
+              uint32_t outm = (px == 0 ? G::face(0, -1) : 0u) | (px == T - 1 ? G::face(0, 1) : 0u) |
+                              (py == 0 ? G::face(1, -1) : 0u) | (py == T - 1 ? G::face(1, 1) : 0u);
+              if (DIM == 3) outm |= (pz == 0 ? G::face(2, -1) : 0u) | (pz == T - 1 ? G::face(2, 1) : 0u);
               const uint32_t *const tq = tile + cc;
-              int ssum = 0, cnt = 0;
+              int ssum = 0, ncnt = 0;
               bool zero = false;
-#pragma unroll
-              for (int n = 0; n <= NNB; ++n) {
-                const int qx = px + G::dx(n), qy = py + G::dy(n), qz = pz + G::dz(n);
-                int gx = ox - 1 + qx, gy = oy - 1 + qy, gz = (DIM == 3) ? oz - 1 + qz : 0;
+#pragma unroll 1
+              for (int n = NNB; n >= 0 && !zero; --n) {   // n = NNB: the centre itself, first (rolled: keeps the code small)
+                const int code = sncode[n];
+                int gx = cx + (code & 3) - 1, gy = cy + ((code >> 2) & 3) - 1, gz = (DIM == 3) ? cz + ((code >> 4) & 3) - 1 : 0;
                 bool ok = true;   // false = outside a closed lattice: medium, never the same cell (S5)
-                if (gx < 0) { if (P.per[0]) gx += P.X; else ok = false; } else if (gx >= P.X) { if (P.per[0]) gx -= P.X; else ok = false; }
-                if (gy < 0) { if (P.per[1]) gy += P.Y; else ok = false; } else if (gy >= P.Y) { if (P.per[1]) gy -= P.Y; else ok = false; }
-                if (DIM == 3) { if (gz < 0) { if (P.per[2]) gz += P.Z; else ok = false; } else if (gz >= P.Z) { if (P.per[2]) gz -= P.Z; else ok = false; } }
+                if (edge) {
+                  if (gx < 0) { gx += P.X; ok = P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; ok = P.per[0] != 0; }
+                  if (gy < 0) { gy += P.Y; ok = ok && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; ok = ok && P.per[1] != 0; }
+                  if (DIM == 3) { if (gz < 0) { gz += P.Z; ok = ok && P.per[2] != 0; } else if (gz >= P.Z) { gz -= P.Z; ok = ok && P.per[2] != 0; } }
+                }
                 bool same = (n == NNB);
                 if (n != NNB && ok) {
-                  const bool in = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
                   // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
-                  const uint32_t wq = in ? tq[(ctr + G::noff(n)) * 32] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, gx, gy, gz));
+                  const uint32_t wq = ((outm >> n) & 1u) ? __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz)) : tq[(ctr + snoff[n]) * 32];
                   same = (wq & CELL_MASK31) == mC;
                 }
                 if (same) {
-                  // L2: sees the Act bytes this warp stored on earlier commits
+                  // L2: sees the Act bytes stored by earlier commits of this CTA
                   const int av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
-                  zero = zero || av == 0;
-                  ssum += __ldg(P.logq16 + av);
-                  ++cnt;
+                  zero = av == 0;
+                  ssum += slog[av];
+                  ++ncnt;
                 }
               }
               int g = 0;
-              if (!zero) { const int mm = ssum / cnt; g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
-              gmout[((rq.x >> 14) & 31u) * 2 + (rq.x >> 19)] = g;
+              if (!zero) { const int mm = ssum / ncnt; g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
+              gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
             }
-            __syncwarp();
+            __syncthreads();
             long long sideA = 0, sideB = 0;
-            if (wantA) { const int g = gmout[lane * 2]; if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g); }
-            if (wantB) { const int g = gmout[lane * 2 + 1]; if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g); }
+            if (wantA) { const int g = gmout[tid * 2]; if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g); }
+            if (wantB) { const int g = gmout[tid * 2 + 1]; if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g); }
             if (wantA || wantB) dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
           }
         }
@@ -346,91 +402,104 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
             if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
           }
         }
-        // ---- a9: the first accepted attempt of every chain wins; what was evaluated before it is final ----
-        if (acc) atomicMin(first + c, a);
-        __syncwarp();
-        if (have) {
-          const int f = first[c];
-          if (f >= a) ++n_eval;
-          if (acc && f == a) {
-            ++n_acc;
-            tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
-            gtile[toff * 32 + c] = wA;           // home word in HBM
-            const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
-            const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
-            const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
-            // halo replicas of this site in the tiles of the adjacent (inactive) subsections
-            const int bx = ox / S, by = oy / S, bz = oz / S;
+        // ---- a9: the first accepted attempt of every chain wins (it carries n_A, n_B for the commit) ----
+        if (acc) atomicMin(first + c, (a << 10) | (nA << 5) | nB);
+        if (ACT && tid == 0) cnt[1] = 0;   // every thread has read the request count
+        __syncthreads();
+      }
+
+      // ---- what lies before a chain's winner is final ----
+      const int fw = first[lane];
+      const int fa = fw >> 10;
 #pragma unroll
-            for (int dz = (DIM == 3 ? -1 : 0); dz <= (DIM == 3 ? 1 : 0); ++dz)
-#pragma unroll
-              for (int dy = -1; dy <= 1; ++dy)
-#pragma unroll
-                for (int dx = -1; dx <= 1; ++dx) {
-                  if (dx == 0 && dy == 0 && dz == 0) continue;
-                  if ((dx < 0 && px != 1) || (dx > 0 && px != S) || (dy < 0 && py != 1) || (dy > 0 && py != S) ||
-                      (dz < 0 && pz != 1) || (dz > 0 && pz != S)) continue;
-                  int nx = bx + dx, ny = by + dy, nz = bz + dz;
-                  bool ok = true;
-                  if (nx < 0) { if (P.per[0]) nx += P.nsub[0]; else ok = false; } else if (nx >= P.nsub[0]) { if (P.per[0]) nx -= P.nsub[0]; else ok = false; }
-                  if (ny < 0) { if (P.per[1]) ny += P.nsub[1]; else ok = false; } else if (ny >= P.nsub[1]) { if (P.per[1]) ny -= P.nsub[1]; else ok = false; }
-                  if (DIM == 3) { if (nz < 0) { if (P.per[2]) nz += P.nsub[2]; else ok = false; } else if (nz >= P.nsub[2]) { if (P.per[2]) nz -= P.nsub[2]; else ok = false; } }
-                  if (!ok) continue;
-                  const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
-                  P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
-                }
-            if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-              P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)pa.maxA;
-            // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
-            //      and, in deterministic mode, the chain's own-delta table
-#pragma unroll
-            for (int side = 0; side < 2; ++side) {
-              const uint32_t cell = side ? Bc : A;
-              if (cell == 0) continue;
-              const int sgn = side ? -1 : 1;
-              const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)(side ? dPB : dPA);
-              atomicAdd(P.liveVP + cell, d);
-              atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
-              atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
-              if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
-              if constexpr (!LIVE) {
-                const int ne = dn[c];
-                bool hit = false;
-                const int ns = min(ne, PK_DCAP);
-                for (int i = 0; i < ns; ++i)
-                  if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
-                if (!hit && ne > PK_DCAP) {
-                  const long long sl = (long long)dslot[c] * PK_SPILL;
-                  for (int i = 0; i < ne - PK_DCAP; ++i)
-                    if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
-                }
-                if (!hit) {
-                  if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = ne + 1; }
-                  else if (ne < PK_CAP) {
-                    int slot = dslot[c];
-                    if (slot < 0) {
-                      slot = atomicAdd(P.ovf_count, 1);
-                      if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
-                      dslot[c] = slot;
-                    }
-                    if (slot >= 0) {
-                      const long long sl = (long long)slot * PK_SPILL;
-                      P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
-                      dn[c] = ne + 1;
-                    }
-                  } else overflow = true;
-                }
+      for (int j = 0; j < 4; ++j) n_eval += (in[j] && 4 * wrp + j <= fa) ? 1u : 0u;
+      // ---- a9/a10: warp 0, lane = chain: commit the winners ----
+      if (wrp == 0) {
+        const int c = lane;
+        if (fw < PK_NOWIN) {
+          const int nA = (fw >> 5) & 31, nB = fw & 31;
+          const int prc = (int)prop[fa * 32 + c];
+          const int toff = prc & 511;
+          const int soff = toff + snoff[prc >> 9];
+          const uint32_t wA = tcol[soff * 32], wB = tcol[toff * 32];
+          const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+          ++n_acc;
+          tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
+          gtile[toff * 32 + c] = wA;           // home word in HBM
+          const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
+          const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
+          const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
+          // halo replicas of this site in the tiles of the adjacent (inactive) subsections
+          const int bx = ox / S, by = oy / S, bz = oz / S;
+          const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
+          const int fz = (DIM == 3) ? ((pz == 1) ? -1 : (pz == S) ? 1 : 0) : 0;
+          const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
+#pragma unroll 1
+          for (int msk = 1; msk < (1 << DIM); ++msk) {
+            if (msk & ~avail) continue;
+            const int dx = (msk & 1) ? fx : 0, dy = (msk & 2) ? fy : 0, dz = (msk & 4) ? fz : 0;
+            int nx = bx + dx, ny = by + dy, nz = bz + dz;
+            bool ok = true;
+            if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
+            if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }
+            if (DIM == 3) { if (nz < 0) { nz += P.nsub[2]; ok = ok && P.per[2] != 0; } else if (nz >= P.nsub[2]) { nz -= P.nsub[2]; ok = ok && P.per[2] != 0; } }
+            if (!ok) continue;
+            const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
+            P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
+          }
+          if constexpr (ACT)   // Max_act of the new owner; 0 for medium
+            P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[wA >> 24 & 127].maxA : 0);
+          // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
+          //      and, in deterministic mode, the chain's own-delta table
+#pragma unroll 1
+          for (int side = 0; side < 2; ++side) {
+            const uint32_t cell = side ? Bc : A;
+            if (cell == 0) continue;
+            const int sgn = side ? -1 : 1;
+            const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
+            const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
+            atomicAdd(P.liveVP + cell, d);
+            atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
+            atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
+            if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
+            if constexpr (!LIVE) {
+              const int ne = dn[c];
+              bool hit = false;
+              const int ns = min(ne, PK_DCAP);
+              for (int i = 0; i < ns; ++i)
+                if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
+              if (!hit && ne > PK_DCAP) {
+                const long long sl = (long long)dslot[c] * PK_SPILL;
+                for (int i = 0; i < ne - PK_DCAP; ++i)
+                  if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
+              }
+              if (!hit) {
+                if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = ne + 1; }
+                else if (ne < PK_CAP) {
+                  int slot = dslot[c];
+                  if (slot < 0) {
+                    slot = atomicAdd(P.ovf_count, 1);
+                    if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
+                    dslot[c] = slot;
+                  }
+                  if (slot >= 0) {
+                    const long long sl = (long long)slot * PK_SPILL;
+                    P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
+                    dn[c] = ne + 1;
+                  }
+                } else overflow = true;
               }
             }
           }
         }
-        __syncwarp();
+        // chains with an accepted copy continue behind it on the new state
+        const int np = (fw < PK_NOWIN) ? fa + 1 : PK_CHUNK;
+        spos[c] = np;
+        const bool redo = __any_sync(FULL, np < kk);
+        if (lane == 0) { cnt[0] = 0; cnt[2] = redo ? 1 : 0; }
       }
-      // ---- chains with an accepted copy continue behind it on the new state ----
-      const int f = first[lane];
-      pos = (f < PK_CHUNK) ? f + 1 : PK_CHUNK;
-      if (!__any_sync(FULL, pos < kk)) break;
-      __syncwarp();
+      __syncthreads();
+      if (cnt[2] == 0) break;
     }
   }
   if (!staged) { while (!mbar_try_wait(mbar, 0)) {} }   // never leave a bulk copy in flight
@@ -438,7 +507,7 @@ __global__ void __launch_bounds__(32) sweep_pool_kernel(const __grid_constant__ 
   n_acc = __reduce_add_sync(FULL, n_acc);
   const bool any_over = __any_sync(FULL, overflow);
   if (lane == 0) {
-    const int slot = (int)(blockIdx.x % COUNTER_SLOTS);
+    const int slot = (int)((blockIdx.x * PK_WARPS + wrp) % COUNTER_SLOTS);
     if (n_eval) atomicAdd(P.counters + 2 * slot, (unsigned long long)n_eval);
     if (n_acc) atomicAdd(P.counters + 2 * slot + 1, (unsigned long long)n_acc);
     if (any_over) atomicOr(P.error_flag, 1);
@@ -489,7 +558,7 @@ __global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
     const int x = (int)(i % X);
     const long long r = i / X;
-    ids[i] = L.tiles[home_word<DIM>(L, x, (int)(r % Y), (int)(r / Y))] & ID_MASK;
+    ids[i] = L.tiles[home_word<DIM>(L, L.S, x, (int)(r % Y), (int)(r / Y))] & ID_MASK;
   }
 }
 // recount of V, A (Moore interfaces with sites not of the same cell, L234) and the coordinate sums (L288) from the

@@ -573,7 +573,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
         sp.grp_base = sp.tl.base[col];
         const unsigned long long per_cta = c->pooled ? 32ull : (unsigned long long)c->wpc;
         const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
-        if (grid > 0x7fffffffULL) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
+        if (grid > 0x7fffffffULL || (c->pooled && n_active > 0x7fffffffULL)) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
         if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, c->stream));
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (c->timing) {

@@ -167,23 +167,24 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
   for (int i = tid; i < P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
   if constexpr (ACT) for (int i = tid; i < 256; i += PK_THREADS) slog[i] = P.logq16[i];
 
-  // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk)
-  const unsigned long long w = (unsigned long long)blockIdx.x * 32ull + (unsigned long long)lane;
-  const bool active = w < P.n_active;
-  uint32_t b = 0;
-  {
+  // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk); its geometry is
+  // worked out once, by warp 0 (the host limits n_active to 31 bits for this kernel)
+  const uint32_t w = blockIdx.x * 32u + (uint32_t)lane;
+  const bool active = w < (uint32_t)P.n_active;
+  if (wrp == 0) {
+    uint32_t b0 = 0;
     int ox = 0, oy = 0, oz = 0;
     if (active) {
-      const int ax = (int)(w % (unsigned)P.nact[0]);
-      const unsigned long long r1 = w / (unsigned)P.nact[0];
-      const int ay = (int)(r1 % (unsigned)P.nact[1]);
-      const int az = (int)(r1 / (unsigned)P.nact[1]);
-      const int bx = 2 * ax + P.col[0], by = 2 * ay + P.col[1], bz = (DIM == 3) ? 2 * az + P.col[2] : 0;
-      b = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
+      const uint32_t ax = w % (uint32_t)P.nact[0], r1 = w / (uint32_t)P.nact[0];
+      const uint32_t ay = r1 % (uint32_t)P.nact[1], az = r1 / (uint32_t)P.nact[1];
+      const int bx = 2 * (int)ax + P.col[0], by = 2 * (int)ay + P.col[1], bz = (DIM == 3) ? 2 * (int)az + P.col[2] : 0;
+      b0 = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
       ox = bx * S; oy = by * S; oz = (DIM == 3) ? bz * S : 0;
     }
-    if (wrp == 0) { bsub[lane] = b; orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz; }
+    bsub[lane] = b0; orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz;
   }
+  __syncthreads();
+  const uint32_t b = bsub[lane];
   const uint32_t mcs = *P.mcs_ptr;
   const int k = P.k;
   const int nchunk = (k + PK_CHUNK - 1) / PK_CHUNK;
@@ -323,6 +324,22 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
 
         // ---- Act: request the geometric means (Eq 9) this item needs ----
         if constexpr (ACT) {
+          // any zero makes the mean zero, and the centre belongs to its own neighbourhood: look at it first
+          if (wantA | wantB) {
+            const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
+            if (wantA) {
+              const int sz3 = (DIM == 3) ? soff / (T * T) : 0, sy3 = (soff / T) % T, sx3 = soff % T;
+              int gx = ox - 1 + sx3, gy = oy - 1 + sy3, gz = (DIM == 3) ? oz - 1 + sz3 : 0;
+              gx += (gx < 0) ? P.X : (gx >= P.X) ? -P.X : 0;   // the source holds a cell: it lies inside the lattice, possibly through the wrap
+              gy += (gy < 0) ? P.Y : (gy >= P.Y) ? -P.Y : 0;
+              if (DIM == 3) gz += (gz < 0) ? P.Z : (gz >= P.Z) ? -P.Z : 0;
+              wantA = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx) != 0;
+            }
+            if (wantB) {
+              const int tz3 = (DIM == 3) ? toff / (T * T) : 0, ty3 = (toff / T) % T, tx3 = toff % T;
+              wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
+            }
+          }
           const unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
           const int nGA = __popc(mwA), nGw = nGA + __popc(mwB);
           if (nGw) {   // warp-uniform
@@ -335,51 +352,39 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
           __syncthreads();
           const int nG = cnt[1];
           if (nG) {   // CTA-uniform
-            for (int gi = tid; gi < nG; gi += PK_THREADS) {
+            // one warp per request, lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of
+            // a request are in flight together
+            const int code = sncode[lane <= NNB ? lane : NNB];
+            const int mynoff = (lane < NNB) ? snoff[lane] : 0;
+            for (int gi = wrp; gi < nG; gi += PK_WARPS) {
               const uint2 rq = gmq[gi];
               const int ctr = (int)(rq.x & 511u), cc = (int)((rq.x >> 9) & 31u);
               const uint32_t mC = rq.y;
               const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
-              // the centre is inside the lattice (its cell is not medium); its coordinates, wrapped
-              int cx = orig[cc] - 1 + px, cy = orig[32 + cc] - 1 + py, cz = (DIM == 3) ? orig[64 + cc] - 1 + pz : 0;
-              cx += (cx < 0) ? P.X : (cx >= P.X) ? -P.X : 0;
-              cy += (cy < 0) ? P.Y : (cy >= P.Y) ? -P.Y : 0;
-              if (DIM == 3) cz += (cz < 0) ? P.Z : (cz >= P.Z) ? -P.Z : 0;
-              // does the neighbourhood reach over the lattice border / out of the halo-1 tile?
-              const bool edge = cx < 1 || cx > P.X - 2 || cy < 1 || cy > P.Y - 2 || (DIM == 3 && (cz < 1 || cz > P.Z - 2));
-              uint32_t outm = (px == 0 ? G::face(0, -1) : 0u) | (px == T - 1 ? G::face(0, 1) : 0u) |
-                              (py == 0 ? G::face(1, -1) : 0u) | (py == T - 1 ? G::face(1, 1) : 0u);
-              if (DIM == 3) outm |= (pz == 0 ? G::face(2, -1) : 0u) | (pz == T - 1 ? G::face(2, 1) : 0u);
-              const uint32_t *const tq = tile + cc;
-              int ssum = 0, ncnt = 0;
-              bool zero = false;
-#pragma unroll 1
-              for (int n = NNB; n >= 0 && !zero; --n) {   // n = NNB: the centre itself, first (rolled: keeps the code small)
-                const int code = sncode[n];
-                int gx = cx + (code & 3) - 1, gy = cy + ((code >> 2) & 3) - 1, gz = (DIM == 3) ? cz + ((code >> 4) & 3) - 1 : 0;
-                bool ok = true;   // false = outside a closed lattice: medium, never the same cell (S5)
-                if (edge) {
-                  if (gx < 0) { gx += P.X; ok = P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; ok = P.per[0] != 0; }
-                  if (gy < 0) { gy += P.Y; ok = ok && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; ok = ok && P.per[1] != 0; }
-                  if (DIM == 3) { if (gz < 0) { gz += P.Z; ok = ok && P.per[2] != 0; } else if (gz >= P.Z) { gz -= P.Z; ok = ok && P.per[2] != 0; } }
-                }
-                bool same = (n == NNB);
-                if (n != NNB && ok) {
-                  // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
-                  const uint32_t wq = ((outm >> n) & 1u) ? __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz)) : tq[(ctr + snoff[n]) * 32];
-                  same = (wq & CELL_MASK31) == mC;
-                }
-                if (same) {
-                  // L2: sees the Act bytes stored by earlier commits of this CTA
-                  const int av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
-                  zero = av == 0;
-                  ssum += slog[av];
-                  ++ncnt;
-                }
+              const int qx = px + (code & 3) - 1, qy = py + ((code >> 2) & 3) - 1, qz = (DIM == 3) ? pz + ((code >> 4) & 3) - 1 : 0;
+              int gx = orig[cc] - 1 + qx, gy = orig[32 + cc] - 1 + qy, gz = (DIM == 3) ? orig[64 + cc] - 1 + qz : 0;
+              bool ok = lane <= NNB;   // false = outside a closed lattice: medium, never the same cell (S5)
+              if (gx < 0) { gx += P.X; ok = ok && P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; ok = ok && P.per[0] != 0; }
+              if (gy < 0) { gy += P.Y; ok = ok && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; ok = ok && P.per[1] != 0; }
+              if (DIM == 3) { if (gz < 0) { gz += P.Z; ok = ok && P.per[2] != 0; } else if (gz >= P.Z) { gz -= P.Z; ok = ok && P.per[2] != 0; } }
+              bool same = ok && lane == NNB;
+              if (ok && lane < NNB) {
+                const bool intile = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
+                // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
+                const uint32_t wq = intile ? tile[(ctr + mynoff) * 32 + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
+                same = (wq & CELL_MASK31) == mC;
               }
-              int g = 0;
-              if (!zero) { const int mm = ssum / ncnt; g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
-              gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
+              int av = 1;
+              // L2: sees the Act bytes stored by earlier commits of this CTA
+              if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
+              const unsigned msame = __ballot_sync(FULL, same);
+              const unsigned mzero = __ballot_sync(FULL, same && av == 0);
+              const int ssum = __reduce_add_sync(FULL, same ? slog[av] : 0);
+              if (lane == 0) {
+                int g = 0;
+                if (!mzero) { const int mm = ssum / __popc(msame); g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
+                gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
+              }
             }
             __syncthreads();
             long long sideA = 0, sideB = 0;
@@ -413,22 +418,23 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
       const int fa = fw >> 10;
 #pragma unroll
       for (int j = 0; j < 4; ++j) n_eval += (in[j] && 4 * wrp + j <= fa) ? 1u : 0u;
-      // ---- a9/a10: warp 0, lane = chain: commit the winners ----
-      if (wrp == 0) {
+      // ---- a9/a10: commit the winners, lane = chain; the work is split over the warps:
+      //      warp 0 tile + halo replicas, warp 1 own-delta table, warp 2 / 3 the reductions of cell A / B ----
+      if (fw < PK_NOWIN) {
         const int c = lane;
-        if (fw < PK_NOWIN) {
-          const int nA = (fw >> 5) & 31, nB = fw & 31;
-          const int prc = (int)prop[fa * 32 + c];
-          const int toff = prc & 511;
-          const int soff = toff + snoff[prc >> 9];
-          const uint32_t wA = tcol[soff * 32], wB = tcol[toff * 32];
-          const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+        const int nA = (fw >> 5) & 31, nB = fw & 31;
+        const int prc = (int)prop[fa * 32 + c];
+        const int toff = prc & 511;
+        const int soff = toff + snoff[prc >> 9];
+        const uint32_t wA = tcol[soff * 32], wB = tcol[toff * 32];   // still the state of the round's start
+        const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+        const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
+        const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
+        const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
+        const unsigned long long dA = (1ull << 32) + (unsigned long long)(long long)(NNB - 2 * nA);
+        const unsigned long long dB = (unsigned long long)(-(1ll << 32)) + (unsigned long long)(long long)(2 * nB - NNB);
+        if (wrp == 0) {
           ++n_acc;
-          tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
-          gtile[toff * 32 + c] = wA;           // home word in HBM
-          const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
-          const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
-          const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
           // halo replicas of this site in the tiles of the adjacent (inactive) subsections
           const int bx = ox / S, by = oy / S, bz = oz / S;
           const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
@@ -447,22 +453,17 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
             const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
             P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
           }
+          gtile[toff * 32 + c] = wA;           // home word in HBM
           if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-            P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[wA >> 24 & 127].maxA : 0);
-          // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
-          //      and, in deterministic mode, the chain's own-delta table
+            P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[(wA >> 24) & 127].maxA : 0);
+        } else if (wrp == 1) {
+          // deterministic mode: the chain's own-delta table
+          if constexpr (!LIVE) {
 #pragma unroll 1
-          for (int side = 0; side < 2; ++side) {
-            const uint32_t cell = side ? Bc : A;
-            if (cell == 0) continue;
-            const int sgn = side ? -1 : 1;
-            const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
-            const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
-            atomicAdd(P.liveVP + cell, d);
-            atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
-            atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
-            if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
-            if constexpr (!LIVE) {
+            for (int side = 0; side < 2; ++side) {
+              const uint32_t cell = side ? Bc : A;
+              if (cell == 0) continue;
+              const unsigned long long d = side ? dB : dA;
               const int ne = dn[c];
               bool hit = false;
               const int ns = min(ne, PK_DCAP);
@@ -491,6 +492,25 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
               }
             }
           }
+        } else {
+          // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
+          const uint32_t cell = (wrp == 2) ? A : Bc;
+          if (cell != 0) {
+            const int sgn = (wrp == 2) ? 1 : -1;
+            atomicAdd(P.liveVP + cell, (wrp == 2) ? dA : dB);
+            atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
+            atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
+            if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
+          }
+        }
+      }
+      __syncthreads();   // every warp has read the old tile words of the winners
+      if (wrp == 0) {
+        const int c = lane;
+        if (fw < PK_NOWIN) {
+          const int prc = (int)prop[fa * 32 + c];
+          const int toff = prc & 511;
+          tile[toff * 32 + c] = tcol[(toff + snoff[prc >> 9]) * 32];   // id and type of the source; neither site is frozen
         }
         // chains with an accepted copy continue behind it on the new state
         const int np = (fw < PK_NOWIN) ? fa + 1 : PK_CHUNK;

@@ -27,7 +27,9 @@ constexpr int COUNTER_SLOTS = 256;
 
 struct __align__(16) TypeParams {  // per cell type, Tables 1-3 of the paper
   int32_t lamV, tgtV, lamP, tgtP;
-  int32_t lamA, maxA, pad0, pad1;
+  int32_t lamA, maxA;
+  int32_t cap;   // bound on this type's side of the Act bias: lamA * (largest Act value in the field) / maxA + 1
+  int32_t pad1;
 };
 
 // Tiled lattice layout of the pooled kernel (cpm_pool_kernel.cuh): every subsection owns a tile of (S+2)^d

@@ -6,6 +6,7 @@
 #include "cpm_device.cuh"
 #include "cpm_pool_kernel.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -68,6 +69,8 @@ struct cpm_ctx {
   size_t stage_a_cap = 0, stage_b_cap = 0, stage_c_cap = 0;
 
   std::vector<uint32_t> thr;
+  std::vector<TypeParams> types;   // host copy of the per-type records
+  int act_cap = 0;                 // largest Act value the field can hold right now
   long long Hmax = 0;
   uint32_t mcs_host = 0;      // mirror of the device counter
   uint64_t mcs_run = 0;       // MCS executed by this context (for the attempts counter)
@@ -199,6 +202,27 @@ int check_device_flag(cpm_ctx *c) {
   if (flag & 2) return fail(c, CPM_ERR_ARG, "cell id above max_cells in the lattice");
   if (flag & 4) return fail(c, CPM_ERR_ARG, "Act values must be integers in [0,255]");
   return CPM_OK;
+}
+
+// (Re)build the bound of one side of the Act bias and upload the per-type records.  The pooled kernel works a
+// geometric mean out only when the bias can change the outcome: a side lies in [0, lamA * GM / maxA] and GM <= the
+// largest Act value in the field: the largest Max_act after cpm_set_lattice (the field starts at 0 and only ever
+// receives Max_act values, L255), 255 once cpm_set_act has loaded caller-chosen values.  The slack covers the
+// rounding of the fixed-point mean (relative 2^-10 at most) and of the final shift.
+int upload_types(cpm_ctx *c, int user_values) {
+  int cap_val = 0;
+  for (int i = 0; i < c->nT; ++i) cap_val = std::max(cap_val, (int)c->types[i].maxA);
+  if (user_values) cap_val = 255;
+  c->act_cap = cap_val;
+  for (int i = 0; i < c->nT; ++i) {
+    TypeParams &t = c->types[i];
+    long long cap = 0;
+    if (t.lamA != 0) { const long long v = ((long long)t.lamA * cap_val) / t.maxA; cap = v + v / 1024 + 2; }
+    t.cap = (int32_t)std::min<long long>(cap, 0x3fffffffLL);
+  }
+  cudaError_t e = cudaMemcpyAsync(c->types_dev, c->types.data(), c->types.size() * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  return e == cudaSuccess ? CPM_OK : fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
 }
 
 void free_all(cpm_ctx *c) {
@@ -345,6 +369,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     t.lamA = (p->lambda_act && t.maxA != 0) ? p->lambda_act[i] : 0;
     types[i] = t;
   }
+  c->types = types;
   types[nT] = TypeParams{};
   // adhesion difference table of the pooled kernel: D[a][b][n] = J(a,n) - J(b,n), then the diagonal J(t,t)
   std::vector<int32_t> Dtab((size_t)nT * nT * nT + nT);
@@ -407,11 +432,11 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->D_dev, Dtab.data(), Dtab.size() * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->log_dev, logq.data(), 256 * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->exp_dev, expq.data(), 1024 * 4, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(c->types_dev, types.data(), (nT + 1) * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->thr_dev, c->thr.data(), c->thr.size() * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) rc = fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
   }
+  if (rc == CPM_OK) rc = upload_types(c, 0);
   if (rc != CPM_OK) { free_all(c); delete c; return rc; }
 
   // ---- launch-parameter template ----
@@ -478,6 +503,7 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
 
   CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
   if (c->act) CK(cudaMemsetAsync(c->act, 0, (size_t)c->sp.apitch * c->dim[1] * c->dim[2], c->stream));
+  if (c->act && c->act_cap == 255) { int rc0 = upload_types(c, 0); if (rc0 != CPM_OK) return rc0; }
   CK(cudaMemsetAsync(c->liveVP, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumx, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumy, 0, ncell * 8, c->stream));
@@ -531,6 +557,7 @@ int cpm_set_act(cpm_ctx *c, const float *act, int on_device) {
   CK(cudaSetDevice(c->device));
   int rc = check_device_flag(c);   // a pending error of an earlier cpm_step is reported, not discarded
   if (rc != CPM_OK) return rc;
+  if (c->act_cap != 255) { rc = upload_types(c, 1); if (rc != CPM_OK) return rc; }
   const float *s;
   CK(stage_in(const_cast<float **>(&s), &c->stage_a, &c->stage_a_cap, act, (size_t)c->N, on_device, c->stream));
   act_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s, c->act, c->sp.apitch, c->dim[0], c->dim[1], c->dim[2], c->error_flag);

@@ -41,7 +41,7 @@ constexpr int PK_CHUNK = 16;                 // attempts per chain between two p
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 4;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
-constexpr int PK_NOWIN = PK_CHUNK << 10;     // "no accepted attempt": winner slots hold a << 10 | nA << 5 | nB
+constexpr int PK_NOWIN = PK_CHUNK;           // "no accepted attempt" in a chain's winner slot
 constexpr uint32_t CELL_MASK31 = 0x7FFFFFFFu;   // type + id: equal iff same cell
 
 template <int DIM, int S>
@@ -74,14 +74,14 @@ struct PSmem {
   using G = PGeom<DIM, S>;
   static constexpr int TILE = 0;                                   // uint32 [TW][32]
   static constexpr int PROP = TILE + G::TW * 128;                  // uint16 [16][32]   toff | nb << 9
-  static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint16 [16 * 32]  chain | a << 5
+  static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint16 [4 segments][128]  chain | a << 5
   static constexpr int GMQ = QUEUE + PK_CHUNK * 64;                // uint2 [2 * PK_THREADS] geometric-mean requests
   static constexpr int GMOUT = GMQ + 2 * PK_THREADS * 8;           // int [PK_THREADS][2] results
   static constexpr int DKEY = GMOUT + PK_THREADS * 8;              // uint32 [DCAP][32]
   static constexpr int DDVP = DKEY + PK_DCAP * 128;                // uint64 [DCAP][32]
   static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] entries of the chain's own-delta table
   static constexpr int DSLOT = DN + 128;                           // int [32] spill slot of the chain or -1
-  static constexpr int FIRST = DSLOT + 128;                        // int [32] winner of the round: a << 10 | nA << 5 | nB
+  static constexpr int FIRST = DSLOT + 128;                        // int [32] first accepted attempt of the round
   static constexpr int POS = FIRST + 128;                          // int [32] attempts < pos of the chunk are final
   static constexpr int BSUB = POS + 128;                           // uint32 [32] subsection index b of the chain
   static constexpr int ORIG = BSUB + 128;                          // int [3][32] lattice origin of the chain
@@ -89,8 +89,8 @@ struct PSmem {
   static constexpr int NCODE = NOFF + 128;                         // int [32] neighbour -> (dx+1) | (dy+1) << 2 | (dz+1) << 4
   static constexpr int TYPES = NCODE + 128;                        // TypeParams [9]
   static constexpr int LOGQ = TYPES + 9 * 32;                      // int [256] log2 table of the Act term
-  static constexpr int CNT = LOGQ + 1024;                          // int [4]: queue length, request count, redo flag
-  static constexpr int MBAR = CNT + 16;                            // uint64
+  static constexpr int CNT = LOGQ + 1024;                          // int [8]: [1] request count, [2] redo flag, [4..7] queue segment lengths
+  static constexpr int MBAR = CNT + 32;                            // uint64
   static constexpr int DTAB = MBAR + 16;                           // int32 [nT^3 + nT]
   static constexpr size_t bytes(int nT) { return (size_t)DTAB + ((size_t)nT * nT * nT + nT) * 4; }
 };
@@ -116,7 +116,7 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
 }
 
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
   constexpr int T = G::T, TW = G::TW, NNB = G::NNB;
@@ -221,302 +221,296 @@ __global__ void __launch_bounds__(PK_THREADS) sweep_pool_kernel(const __grid_con
     __syncthreads();
 
     while (true) {
-      // ---- a4: screen the not yet final attempts this thread owns; compact all chains' survivors ----
+      // ---- a4: screen the not yet final attempts this thread owns; every warp compacts the survivors of its four
+      //      attempt indices into its own queue segment (segment w holds attempts 4w..4w+3 of all chains) ----
       if (wrp == 0) first[lane] = PK_NOWIN;   // nobody touches the winner slots before the next barrier
-      const int ps = spos[lane];
-      bool in[4];
-      unsigned m[4];
-      int tot = 0;
+      {
+        const int ps = spos[lane];
+        bool in[4];
+        unsigned m[4];
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int a = 4 * wrp + j;
-        const int toff = pr[j] & 511;
-        const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[j] >> 9]) * 32];
-        in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
-        m[j] = __ballot_sync(FULL, in[j]);
-        tot += __popc(m[j]);
-      }
-      if (tot) {   // warp-uniform
-        int base = 0;
-        if (lane == 0) base = atomicAdd(cnt, tot);
-        base = __shfl_sync(FULL, base, 0);
+        for (int j = 0; j < 4; ++j) {
+          const int a = 4 * wrp + j;
+          const int toff = pr[j] & 511;
+          const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[j] >> 9]) * 32];
+          in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
+          m[j] = __ballot_sync(FULL, in[j]);
+        }
+        int base = wrp * PK_THREADS;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           if (in[j]) queue[base + __popc(m[j] & lt)] = (unsigned short)(lane | ((4 * wrp + j) << 5));
           base += __popc(m[j]);
         }
+        if (lane == 0) cnt[4 + wrp] = base - wrp * PK_THREADS;
       }
       __syncthreads();
-      const int W = cnt[0];
-      if (W == 0) break;   // CTA-uniform: cnt[0] is only reset at the end of a round
+      // a round takes the leading segments that fit one item per thread (nearly always all four); the attempts
+      // of the others are screened again in the next round
+      int e0 = cnt[4], e1 = e0 + cnt[5], e2 = e1 + cnt[6], e3 = e2 + cnt[7];
+      int nseg = 4;
+      if (e3 > PK_THREADS) { nseg = (e2 <= PK_THREADS) ? 3 : (e1 <= PK_THREADS) ? 2 : 1; }
+      const int W = nseg == 4 ? e3 : nseg == 3 ? e2 : nseg == 2 ? e1 : e0;
+      const int a_lim = 4 * nseg;            // attempts < a_lim are covered by this round
+      if (W == 0 && nseg == 4) break;        // CTA-uniform: nothing left in this chunk
 
-      for (int sb = 0; sb < W; sb += PK_THREADS) {
-        // ---- a5-a7: one item per thread ----
-        const int qi = sb + tid;
-        const bool have = qi < W;
-        const int item = have ? (int)queue[qi] : 0;
-        const int c = item & 31, a = item >> 5;
-        const int prc = (int)prop[a * 32 + c];
-        const int toff = prc & 511, nb = prc >> 9;
-        const int soff = toff + snoff[nb];
-        const uint32_t *const tc = tile + c;
-        const uint32_t wA = tc[soff * 32], wB = tc[toff * 32];
-        const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
-        const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
-        const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
-        long long dH = 0;
-        int nA = 0, nB = 0;
-        bool go = false;
-        TypeParams pa = st[P.nT], pb = st[P.nT];
-        bool wantA = false, wantB = false;
-        if (have) {
-          unsigned long long baseA = 0ull, baseB = 0ull;
-          if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
-          if (Bc != 0) baseB = LIVE ? __ldcg(P.liveVP + Bc) : __ldg(P.snapVP + Bc);
-          const int32_t *Drow = sd + (tA * P.nT + tB) * P.nT;
-          int adh = 0;
+      // ---- a5-a7: one item per thread ----
+      const bool have = tid < W;
+      int item = 0;
+      if (have) {
+        const int sg = (tid >= e0 ? 1 : 0) + (tid >= e1 ? 1 : 0) + (tid >= e2 ? 1 : 0);
+        const int off = tid - (sg == 0 ? 0 : sg == 1 ? e0 : sg == 2 ? e1 : e2);
+        item = (int)queue[sg * PK_THREADS + off];
+      }
+      const int c = item & 31, a = item >> 5;
+      const int prc = (int)prop[a * 32 + c];
+      const int toff = prc & 511, nb = prc >> 9;
+      const int soff = toff + snoff[nb];
+      const uint32_t *const tc = tile + c;
+      const uint32_t wA = tc[soff * 32], wB = tc[toff * 32];
+      const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+      const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
+      const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
+      long long dH = 0;
+      int nA = 0, nB = 0;
+      bool go = false;
+      TypeParams pa = st[P.nT], pb = st[P.nT];
+      bool wantA = false, wantB = false;
+      if (have) {
+        unsigned long long baseA = 0ull, baseB = 0ull;
+        if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
+        if (Bc != 0) baseB = LIVE ? __ldcg(P.liveVP + Bc) : __ldg(P.snapVP + Bc);
+        const int32_t *Drow = sd + (tA * P.nT + tB) * P.nT;
+        int adh = 0;
 #pragma unroll
-          for (int n = 0; n < NNB; ++n) {
-            const uint32_t mm = tc[(toff + G::noff(n)) * 32] & CELL_MASK31;
-            nA += (mm == mA) ? 1 : 0;
-            nB += (mm == mB) ? 1 : 0;
-            adh += Drow[mm >> 24];
-          }
-          // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
-          adh += nB * sdiag[tB] - nA * sdiag[tA];
-          dH = adh;
-          // a6: per-cell {V,P} as this attempt sees it: snapshot + the chain's own deltas / live
-          unsigned long long vpA = baseA, vpB = baseB;
-          if constexpr (!LIVE) {
-            const int ne = dn[c];
-            if (ne > 0) {
-              unsigned long long dA = 0ull, dB = 0ull;
-              const int ns = min(ne, PK_DCAP);
-              for (int i = 0; i < ns; ++i) {
-                const uint32_t key = dkey[i * 32 + c];
-                const unsigned long long v = ddvp[i * 32 + c];
+        for (int n = 0; n < NNB; ++n) {
+          const uint32_t mm = tc[(toff + G::noff(n)) * 32] & CELL_MASK31;
+          nA += (mm == mA) ? 1 : 0;
+          nB += (mm == mB) ? 1 : 0;
+          adh += Drow[mm >> 24];
+        }
+        // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
+        adh += nB * sdiag[tB] - nA * sdiag[tA];
+        dH = adh;
+        // a6: per-cell {V,P} as this attempt sees it: snapshot + the chain's own deltas / live
+        unsigned long long vpA = baseA, vpB = baseB;
+        if constexpr (!LIVE) {
+          const int ne = dn[c];
+          if (ne > 0) {
+            unsigned long long dA = 0ull, dB = 0ull;
+            const int ns = min(ne, PK_DCAP);
+            for (int i = 0; i < ns; ++i) {
+              const uint32_t key = dkey[i * 32 + c];
+              const unsigned long long v = ddvp[i * 32 + c];
+              if (key == A) dA = v;
+              if (key == Bc) dB = v;
+            }
+            if (ne > PK_DCAP) {
+              const long long sl = (long long)dslot[c] * PK_SPILL;
+              for (int i = 0; i < ne - PK_DCAP; ++i) {
+                const uint32_t key = __ldcg(P.ovf_keys + sl + i);
+                const unsigned long long v = __ldcg(P.ovf_dvp + sl + i);
                 if (key == A) dA = v;
                 if (key == Bc) dB = v;
               }
-              if (ne > PK_DCAP) {
-                const long long sl = (long long)dslot[c] * PK_SPILL;
-                for (int i = 0; i < ne - PK_DCAP; ++i) {
-                  const uint32_t key = __ldcg(P.ovf_keys + sl + i);
-                  const unsigned long long v = __ldcg(P.ovf_dvp + sl + i);
-                  if (key == A) dA = v;
-                  if (key == Bc) dB = v;
-                }
-              }
-              if (A != 0) vpA += dA;
-              if (Bc != 0) vpB += dB;
             }
+            if (A != 0) vpA += dA;
+            if (Bc != 0) vpB += dB;
           }
-          go = !(Bc != 0 && (uint32_t)(vpB >> 32) <= 1u);   // a cell is never erased (reading S13)
-          if (A != 0) pa = st[tA];
-          if (Bc != 0) pb = st[tB];                          // medium reads the all-zero row (S3)
-          const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
-          const int dva = (int)(uint32_t)(vpA >> 32) - pa.tgtV, dvb = (int)(uint32_t)(vpB >> 32) - pb.tgtV;
-          dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
-          const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
-          dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
-          wantA = go && pa.lamA != 0; wantB = go && pb.lamA != 0;
         }
-
-        // ---- Act: request the geometric means (Eq 9) this item needs ----
+        go = !(Bc != 0 && (uint32_t)(vpB >> 32) <= 1u);   // a cell is never erased (reading S13)
+        if (A != 0) pa = st[tA];
+        if (Bc != 0) pb = st[tB];                          // medium reads the all-zero row (S3)
+        const int dPA = NNB - 2 * nA, dPB = 2 * nB - NNB;
+        const int dva = (int)(uint32_t)(vpA >> 32) - pa.tgtV, dvb = (int)(uint32_t)(vpB >> 32) - pb.tgtV;
+        dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
+        const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
+        dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
         if constexpr (ACT) {
-          // any zero makes the mean zero, and the centre belongs to its own neighbourhood: look at it first
-          if (wantA | wantB) {
-            const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
-            if (wantA) {
-              const int sz3 = (DIM == 3) ? soff / (T * T) : 0, sy3 = (soff / T) % T, sx3 = soff % T;
-              int gx = ox - 1 + sx3, gy = oy - 1 + sy3, gz = (DIM == 3) ? oz - 1 + sz3 : 0;
-              gx += (gx < 0) ? P.X : (gx >= P.X) ? -P.X : 0;   // the source holds a cell: it lies inside the lattice, possibly through the wrap
-              gy += (gy < 0) ? P.Y : (gy >= P.Y) ? -P.Y : 0;
-              if (DIM == 3) gz += (gz < 0) ? P.Z : (gz >= P.Z) ? -P.Z : 0;
-              wantA = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx) != 0;
-            }
-            if (wantB) {
-              const int tz3 = (DIM == 3) ? toff / (T * T) : 0, ty3 = (toff / T) % T, tx3 = toff % T;
-              wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
-            }
+          // The Act bias lies in [-capB, +capA] (cap = lamA * largest Act value in the field / maxA, host-built):
+          // it is only worked out when it can change the outcome.
+          const long long capA = pa.lamA != 0 ? pa.cap : 0, capB = pb.lamA != 0 ? pb.cap : 0;
+          const bool matters = go && !P.accept_all && dH + capB > 0 && dH - capA <= P.Hmax;
+          wantA = matters && pa.lamA != 0; wantB = matters && pb.lamA != 0;
+        }
+      }
+
+      // ---- Act: request the geometric means (Eq 9) this item needs ----
+      if constexpr (ACT) {
+        // any zero makes the mean zero, and the centre belongs to its own neighbourhood: look at it first
+        if (wantA | wantB) {
+          const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
+          if (wantA) {
+            const int sz3 = (DIM == 3) ? soff / (T * T) : 0, sy3 = (soff / T) % T, sx3 = soff % T;
+            int gx = ox - 1 + sx3, gy = oy - 1 + sy3, gz = (DIM == 3) ? oz - 1 + sz3 : 0;
+            gx += (gx < 0) ? P.X : (gx >= P.X) ? -P.X : 0;   // the source holds a cell: it lies inside the lattice, possibly through the wrap
+            gy += (gy < 0) ? P.Y : (gy >= P.Y) ? -P.Y : 0;
+            if (DIM == 3) gz += (gz < 0) ? P.Z : (gz >= P.Z) ? -P.Z : 0;
+            wantA = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx) != 0;
           }
-          const unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
-          const int nGA = __popc(mwA), nGw = nGA + __popc(mwB);
-          if (nGw) {   // warp-uniform
-            int base = 0;
-            if (lane == 0) base = atomicAdd(cnt + 1, nGw);
-            base = __shfl_sync(FULL, base, 0);
-            if (wantA) gmq[base + __popc(mwA & lt)] = make_uint2((uint32_t)(soff | (c << 9) | (tid << 14)), mA);
-            if (wantB) gmq[base + nGA + __popc(mwB & lt)] = make_uint2((uint32_t)(toff | (c << 9) | (tid << 14) | (1 << 21)), mB);
+          if (wantB) {
+            const int tz3 = (DIM == 3) ? toff / (T * T) : 0, ty3 = (toff / T) % T, tx3 = toff % T;
+            wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
           }
-          __syncthreads();
-          const int nG = cnt[1];
-          if (nG) {   // CTA-uniform
-            // one warp per request, lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of
-            // a request are in flight together
-            const int code = sncode[lane <= NNB ? lane : NNB];
-            const int mynoff = (lane < NNB) ? snoff[lane] : 0;
-            for (int gi = wrp; gi < nG; gi += PK_WARPS) {
-              const uint2 rq = gmq[gi];
-              const int ctr = (int)(rq.x & 511u), cc = (int)((rq.x >> 9) & 31u);
-              const uint32_t mC = rq.y;
-              const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
-              const int qx = px + (code & 3) - 1, qy = py + ((code >> 2) & 3) - 1, qz = (DIM == 3) ? pz + ((code >> 4) & 3) - 1 : 0;
-              int gx = orig[cc] - 1 + qx, gy = orig[32 + cc] - 1 + qy, gz = (DIM == 3) ? orig[64 + cc] - 1 + qz : 0;
-              bool ok = lane <= NNB;   // false = outside a closed lattice: medium, never the same cell (S5)
+        }
+        const unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
+        const int nGA = __popc(mwA), nGw = nGA + __popc(mwB);
+        if (nGw) {   // warp-uniform
+          int base = 0;
+          if (lane == 0) base = atomicAdd(cnt + 1, nGw);
+          base = __shfl_sync(FULL, base, 0);
+          if (wantA) gmq[base + __popc(mwA & lt)] = make_uint2((uint32_t)(soff | (c << 9) | (tid << 14)), mA);
+          if (wantB) gmq[base + nGA + __popc(mwB & lt)] = make_uint2((uint32_t)(toff | (c << 9) | (tid << 14) | (1 << 21)), mB);
+        }
+        __syncthreads();
+        const int nG = cnt[1];
+        if (nG) {   // CTA-uniform
+          // one warp per request, lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of
+          // a request are in flight together
+          const int code = sncode[lane <= NNB ? lane : NNB];
+          const int ddx = (code & 3) - 1, ddy = ((code >> 2) & 3) - 1, ddz = (DIM == 3) ? ((code >> 4) & 3) - 1 : 0;
+          const int mynoff = (lane < NNB) ? snoff[lane] : 0;
+          for (int gi = wrp; gi < nG; gi += PK_WARPS) {
+            const uint2 rq = gmq[gi];
+            const int ctr = (int)(rq.x & 511u), cc = (int)((rq.x >> 9) & 31u);
+            const uint32_t mC = rq.y;
+            const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
+            // the centre is inside the lattice (its cell is not medium), possibly through the wrap
+            int cx = orig[cc] - 1 + px, cy = orig[32 + cc] - 1 + py, cz = (DIM == 3) ? orig[64 + cc] - 1 + pz : 0;
+            cx += (cx < 0) ? P.X : (cx >= P.X) ? -P.X : 0;
+            cy += (cy < 0) ? P.Y : (cy >= P.Y) ? -P.Y : 0;
+            if (DIM == 3) cz += (cz < 0) ? P.Z : (cz >= P.Z) ? -P.Z : 0;
+            int gx = cx + ddx, gy = cy + ddy, gz = cz + ddz;
+            bool ok = lane <= NNB;   // false = outside a closed lattice: medium, never the same cell (S5)
+            if (cx < 1 || cx > P.X - 2 || cy < 1 || cy > P.Y - 2 || (DIM == 3 && (cz < 1 || cz > P.Z - 2))) {   // warp-uniform
               if (gx < 0) { gx += P.X; ok = ok && P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; ok = ok && P.per[0] != 0; }
               if (gy < 0) { gy += P.Y; ok = ok && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; ok = ok && P.per[1] != 0; }
               if (DIM == 3) { if (gz < 0) { gz += P.Z; ok = ok && P.per[2] != 0; } else if (gz >= P.Z) { gz -= P.Z; ok = ok && P.per[2] != 0; } }
-              bool same = ok && lane == NNB;
-              if (ok && lane < NNB) {
-                const bool intile = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
-                // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
-                const uint32_t wq = intile ? tile[(ctr + mynoff) * 32 + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
-                same = (wq & CELL_MASK31) == mC;
-              }
-              int av = 1;
-              // L2: sees the Act bytes stored by earlier commits of this CTA
-              if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
-              const unsigned msame = __ballot_sync(FULL, same);
-              const unsigned mzero = __ballot_sync(FULL, same && av == 0);
-              const int ssum = __reduce_add_sync(FULL, same ? slog[av] : 0);
-              if (lane == 0) {
-                int g = 0;
-                if (!mzero) { const int mm = ssum / __popc(msame); g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
-                gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
-              }
             }
-            __syncthreads();
-            long long sideA = 0, sideB = 0;
-            if (wantA) { const int g = gmout[tid * 2]; if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g); }
-            if (wantB) { const int g = gmout[tid * 2 + 1]; if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g); }
-            if (wantA || wantB) dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
+            bool same = ok && lane == NNB;
+            if (ok && lane < NNB) {
+              const int qx = px + ddx, qy = py + ddy, qz = pz + ddz;
+              const bool intile = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
+              // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
+              const uint32_t wq = intile ? tile[(ctr + mynoff) * 32 + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
+              same = (wq & CELL_MASK31) == mC;
+            }
+            int av = 1;
+            // L2: sees the Act bytes stored by earlier commits of this CTA
+            if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
+            const unsigned msame = __ballot_sync(FULL, same);
+            const unsigned mzero = __ballot_sync(FULL, same && av == 0);
+            const int ssum = __reduce_add_sync(FULL, same ? slog[av] : 0);
+            if (lane == 0) {
+              int g = 0;
+              if (!mzero) { const int mm = ssum / __popc(msame); g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
+              gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
+            }
           }
+          __syncthreads();
+          long long sideA = 0, sideB = 0;
+          if (wantA) { const int g = gmout[tid * 2]; if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g); }
+          if (wantB) { const int g = gmout[tid * 2 + 1]; if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g); }
+          if (wantA || wantB) dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
         }
-
-        // ---- a8: Metropolis (Eq 2) against the integer threshold table; the acceptance word (Philox stream 1)
-        //      is drawn only for uphill moves inside the table ----
-        bool acc = have && go;
-        const bool uphill = acc && dH > 0 && !P.accept_all;
-        if (uphill && dH > P.Hmax) acc = false;
-        const bool draw = uphill && acc;
-        if (__any_sync(FULL, draw)) {
-          if (draw) {
-            const int ag = ch * PK_CHUNK + a;
-            const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, bsub[c], 2u * P.p + 1u, mcs), P.key0, P.key1);
-            if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
-          }
-        }
-        // ---- a9: the first accepted attempt of every chain wins (it carries n_A, n_B for the commit) ----
-        if (acc) atomicMin(first + c, (a << 10) | (nA << 5) | nB);
-        if (ACT && tid == 0) cnt[1] = 0;   // every thread has read the request count
-        __syncthreads();
       }
 
-      // ---- what lies before a chain's winner is final ----
-      const int fw = first[lane];
-      const int fa = fw >> 10;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) n_eval += (in[j] && 4 * wrp + j <= fa) ? 1u : 0u;
-      // ---- a9/a10: commit the winners, lane = chain; the work is split over the warps:
-      //      warp 0 tile + halo replicas, warp 1 own-delta table, warp 2 / 3 the reductions of cell A / B ----
-      if (fw < PK_NOWIN) {
-        const int c = lane;
-        const int nA = (fw >> 5) & 31, nB = fw & 31;
-        const int prc = (int)prop[fa * 32 + c];
-        const int toff = prc & 511;
-        const int soff = toff + snoff[prc >> 9];
-        const uint32_t wA = tcol[soff * 32], wB = tcol[toff * 32];   // still the state of the round's start
-        const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+      // ---- a8: Metropolis (Eq 2) against the integer threshold table; the acceptance word (Philox stream 1)
+      //      is drawn only for uphill moves inside the table ----
+      bool acc = have && go;
+      const bool uphill = acc && dH > 0 && !P.accept_all;
+      if (uphill && dH > P.Hmax) acc = false;
+      const bool draw = uphill && acc;
+      if (__any_sync(FULL, draw)) {
+        if (draw) {
+          const int ag = ch * PK_CHUNK + a;
+          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, bsub[c], 2u * P.p + 1u, mcs), P.key0, P.key1);
+          if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
+        }
+      }
+      // ---- a9: the first accepted attempt of every chain wins ----
+      if (acc) atomicMin(first + c, a);
+      __syncthreads();
+      const int fa = have ? first[c] : 0;
+      if (have && a <= fa) ++n_eval;   // what lies before a chain's winner (and the winner) is final
+      if (acc && a == fa) {
+        // ---- a9/a10: this thread evaluated the winner of chain c: it commits it ----
+        ++n_acc;
+        tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
+        gtile[toff * 32 + c] = wA;           // home word in HBM
         const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
         const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
         const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
-        const unsigned long long dA = (1ull << 32) + (unsigned long long)(long long)(NNB - 2 * nA);
-        const unsigned long long dB = (unsigned long long)(-(1ll << 32)) + (unsigned long long)(long long)(2 * nB - NNB);
-        if (wrp == 0) {
-          ++n_acc;
-          // halo replicas of this site in the tiles of the adjacent (inactive) subsections
-          const int bx = ox / S, by = oy / S, bz = oz / S;
-          const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
-          const int fz = (DIM == 3) ? ((pz == 1) ? -1 : (pz == S) ? 1 : 0) : 0;
-          const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
+        // halo replicas of this site in the tiles of the adjacent (inactive) subsections
+        const int bx = ox / S, by = oy / S, bz = oz / S;
+        const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
+        const int fz = (DIM == 3) ? ((pz == 1) ? -1 : (pz == S) ? 1 : 0) : 0;
+        const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
 #pragma unroll 1
-          for (int msk = 1; msk < (1 << DIM); ++msk) {
-            if (msk & ~avail) continue;
-            const int dx = (msk & 1) ? fx : 0, dy = (msk & 2) ? fy : 0, dz = (msk & 4) ? fz : 0;
-            int nx = bx + dx, ny = by + dy, nz = bz + dz;
-            bool ok = true;
-            if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
-            if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }
-            if (DIM == 3) { if (nz < 0) { nz += P.nsub[2]; ok = ok && P.per[2] != 0; } else if (nz >= P.nsub[2]) { nz -= P.nsub[2]; ok = ok && P.per[2] != 0; } }
-            if (!ok) continue;
-            const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
-            P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
-          }
-          gtile[toff * 32 + c] = wA;           // home word in HBM
-          if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-            P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[(wA >> 24) & 127].maxA : 0);
-        } else if (wrp == 1) {
-          // deterministic mode: the chain's own-delta table
+        for (int msk = 1; msk < (1 << DIM); ++msk) {
+          if (msk & ~avail) continue;
+          const int dx = (msk & 1) ? fx : 0, dy = (msk & 2) ? fy : 0, dz = (msk & 4) ? fz : 0;
+          int nx = bx + dx, ny = by + dy, nz = bz + dz;
+          bool ok = true;
+          if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
+          if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }
+          if (DIM == 3) { if (nz < 0) { nz += P.nsub[2]; ok = ok && P.per[2] != 0; } else if (nz >= P.nsub[2]) { nz -= P.nsub[2]; ok = ok && P.per[2] != 0; } }
+          if (!ok) continue;
+          const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
+          P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
+        }
+        if constexpr (ACT)   // Max_act of the new owner; 0 for medium
+          P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)pa.maxA;
+        // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
+        //      and, in deterministic mode, the chain's own-delta table
+#pragma unroll 1
+        for (int side = 0; side < 2; ++side) {
+          const uint32_t cell = side ? Bc : A;
+          if (cell == 0) continue;
+          const int sgn = side ? -1 : 1;
+          const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
+          const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
+          atomicAdd(P.liveVP + cell, d);
+          atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
+          atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
+          if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
           if constexpr (!LIVE) {
-#pragma unroll 1
-            for (int side = 0; side < 2; ++side) {
-              const uint32_t cell = side ? Bc : A;
-              if (cell == 0) continue;
-              const unsigned long long d = side ? dB : dA;
-              const int ne = dn[c];
-              bool hit = false;
-              const int ns = min(ne, PK_DCAP);
-              for (int i = 0; i < ns; ++i)
-                if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
-              if (!hit && ne > PK_DCAP) {
-                const long long sl = (long long)dslot[c] * PK_SPILL;
-                for (int i = 0; i < ne - PK_DCAP; ++i)
-                  if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
-              }
-              if (!hit) {
-                if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = ne + 1; }
-                else if (ne < PK_CAP) {
-                  int slot = dslot[c];
-                  if (slot < 0) {
-                    slot = atomicAdd(P.ovf_count, 1);
-                    if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
-                    dslot[c] = slot;
-                  }
-                  if (slot >= 0) {
-                    const long long sl = (long long)slot * PK_SPILL;
-                    P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
-                    dn[c] = ne + 1;
-                  }
-                } else overflow = true;
-              }
+            const int ne = dn[c];
+            bool hit = false;
+            const int ns = min(ne, PK_DCAP);
+            for (int i = 0; i < ns; ++i)
+              if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
+            if (!hit && ne > PK_DCAP) {
+              const long long sl = (long long)dslot[c] * PK_SPILL;
+              for (int i = 0; i < ne - PK_DCAP; ++i)
+                if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
             }
-          }
-        } else {
-          // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
-          const uint32_t cell = (wrp == 2) ? A : Bc;
-          if (cell != 0) {
-            const int sgn = (wrp == 2) ? 1 : -1;
-            atomicAdd(P.liveVP + cell, (wrp == 2) ? dA : dB);
-            atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
-            atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
-            if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
+            if (!hit) {
+              if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = ne + 1; }
+              else if (ne < PK_CAP) {
+                int slot = dslot[c];
+                if (slot < 0) {
+                  slot = atomicAdd(P.ovf_count, 1);
+                  if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
+                  dslot[c] = slot;
+                }
+                if (slot >= 0) {
+                  const long long sl = (long long)slot * PK_SPILL;
+                  P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
+                  dn[c] = ne + 1;
+                }
+              } else overflow = true;
+            }
           }
         }
       }
-      __syncthreads();   // every warp has read the old tile words of the winners
       if (wrp == 0) {
-        const int c = lane;
-        if (fw < PK_NOWIN) {
-          const int prc = (int)prop[fa * 32 + c];
-          const int toff = prc & 511;
-          tile[toff * 32 + c] = tcol[(toff + snoff[prc >> 9]) * 32];   // id and type of the source; neither site is frozen
-        }
-        // chains with an accepted copy continue behind it on the new state
-        const int np = (fw < PK_NOWIN) ? fa + 1 : PK_CHUNK;
-        spos[c] = np;
+        // chains with an accepted copy continue behind it on the new state, the others behind the attempts covered
+        const int fw = first[lane];
+        const int np = (fw < PK_NOWIN) ? fw + 1 : a_lim;
+        spos[lane] = np;
         const bool redo = __any_sync(FULL, np < kk);
-        if (lane == 0) { cnt[0] = 0; cnt[2] = redo ? 1 : 0; }
+        if (lane == 0) { cnt[1] = 0; cnt[2] = redo ? 1 : 0; }
       }
       __syncthreads();
       if (cnt[2] == 0) break;

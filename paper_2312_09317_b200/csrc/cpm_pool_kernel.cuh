@@ -75,9 +75,7 @@ struct PSmem {
   static constexpr int TILE = 0;                                   // uint32 [TW][32]
   static constexpr int PROP = TILE + G::TW * 128;                  // uint16 [16][32]   toff | nb << 9
   static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint16 [4 segments][128]  chain | a << 5
-  static constexpr int GMQ = QUEUE + PK_CHUNK * 64;                // uint2 [2 * PK_THREADS] geometric-mean requests
-  static constexpr int GMOUT = GMQ + 2 * PK_THREADS * 8;           // int [PK_THREADS][2] results
-  static constexpr int DKEY = GMOUT + PK_THREADS * 8;              // uint32 [DCAP][32]
+  static constexpr int DKEY = QUEUE + PK_CHUNK * 64;               // uint32 [DCAP][32]
   static constexpr int DDVP = DKEY + PK_DCAP * 128;                // uint64 [DCAP][32]
   static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] entries of the chain's own-delta table
   static constexpr int DSLOT = DN + 128;                           // int [32] spill slot of the chain or -1
@@ -88,8 +86,7 @@ struct PSmem {
   static constexpr int NOFF = ORIG + 384;                          // int [32] neighbour -> tile offset (entry NNB = centre = 0)
   static constexpr int NCODE = NOFF + 128;                         // int [32] neighbour -> (dx+1) | (dy+1) << 2 | (dz+1) << 4
   static constexpr int TYPES = NCODE + 128;                        // TypeParams [9]
-  static constexpr int LOGQ = TYPES + 9 * 32;                      // int [256] log2 table of the Act term
-  static constexpr int CNT = LOGQ + 1024;                          // int [8]: [1] request count, [2] redo flag, [4..7] queue segment lengths
+  static constexpr int CNT = TYPES + 9 * 32;                       // int [8]: [1] request count, [2] redo flag, [4..7] queue segment lengths
   static constexpr int MBAR = CNT + 32;                            // uint64
   static constexpr int DTAB = MBAR + 16;                           // int32 [nT^3 + nT]
   static constexpr size_t bytes(int nT) { return (size_t)DTAB + ((size_t)nT * nT * nT + nT) * 4; }
@@ -124,8 +121,6 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
   unsigned short *prop = reinterpret_cast<unsigned short *>(smem + M::PROP);
   unsigned short *queue = reinterpret_cast<unsigned short *>(smem + M::QUEUE);
-  uint2 *gmq = reinterpret_cast<uint2 *>(smem + M::GMQ);
-  int *gmout = reinterpret_cast<int *>(smem + M::GMOUT);
   uint32_t *dkey = reinterpret_cast<uint32_t *>(smem + M::DKEY);
   unsigned long long *ddvp = reinterpret_cast<unsigned long long *>(smem + M::DDVP);
   int *dn = reinterpret_cast<int *>(smem + M::DN);
@@ -137,7 +132,6 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
   int *snoff = reinterpret_cast<int *>(smem + M::NOFF);
   int *sncode = reinterpret_cast<int *>(smem + M::NCODE);
   TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
-  int *slog = reinterpret_cast<int *>(smem + M::LOGQ);
   int *cnt = reinterpret_cast<int *>(smem + M::CNT);
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + M::MBAR);
   int32_t *sd = reinterpret_cast<int32_t *>(smem + M::DTAB);
@@ -165,7 +159,6 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
   }
   for (int i = tid; i < (P.nT + 1) * 8; i += PK_THREADS) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
   for (int i = tid; i < P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
-  if constexpr (ACT) for (int i = tid; i < 256; i += PK_THREADS) slog[i] = P.logq16[i];
 
   // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk); its geometry is
   // worked out once, by warp 0 (the host limits n_active to 31 bits for this kernel)
@@ -254,25 +247,30 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
       const int a_lim = 4 * nseg;            // attempts < a_lim are covered by this round
       if (W == 0 && nseg == 4) break;        // CTA-uniform: nothing left in this chunk
 
-      // ---- a5-a7: one item per thread ----
+      // ---- a5-a7: one item per thread; warps without items go straight to the barrier ----
       const bool have = tid < W;
+      int c = 0, a = 0, toff = 0, nA = 0, nB = 0, maxA_new = 0;
+      uint32_t wA = 0u, A = 0u, Bc = 0u;
+      bool acc = false;
+      if (32 * wrp < W) {   // warp-uniform
       int item = 0;
       if (have) {
         const int sg = (tid >= e0 ? 1 : 0) + (tid >= e1 ? 1 : 0) + (tid >= e2 ? 1 : 0);
         const int off = tid - (sg == 0 ? 0 : sg == 1 ? e0 : sg == 2 ? e1 : e2);
         item = (int)queue[sg * PK_THREADS + off];
       }
-      const int c = item & 31, a = item >> 5;
+      c = item & 31; a = item >> 5;
       const int prc = (int)prop[a * 32 + c];
-      const int toff = prc & 511, nb = prc >> 9;
+      toff = prc & 511;
+      const int nb = prc >> 9;
       const int soff = toff + snoff[nb];
       const uint32_t *const tc = tile + c;
-      const uint32_t wA = tc[soff * 32], wB = tc[toff * 32];
-      const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+      wA = tc[soff * 32];
+      const uint32_t wB = tc[toff * 32];
+      A = wA & ID_MASK; Bc = wB & ID_MASK;
       const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
       const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
       long long dH = 0;
-      int nA = 0, nB = 0;
       bool go = false;
       TypeParams pa = st[P.nT], pb = st[P.nT];
       bool wantA = false, wantB = false;
@@ -284,10 +282,10 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         int adh = 0;
 #pragma unroll
         for (int n = 0; n < NNB; ++n) {
-          const uint32_t mm = tc[(toff + G::noff(n)) * 32] & CELL_MASK31;
-          nA += (mm == mA) ? 1 : 0;
-          nB += (mm == mB) ? 1 : 0;
-          adh += Drow[mm >> 24];
+          const uint32_t raw = tc[(toff + G::noff(n)) * 32];
+          if (((raw ^ wA) & CELL_MASK31) == 0u) ++nA;
+          if (((raw ^ wB) & CELL_MASK31) == 0u) ++nB;
+          adh += Drow[(raw >> 24) & 127u];
         }
         // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
         adh += nB * sdiag[tB] - nA * sdiag[tA];
@@ -335,7 +333,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         }
       }
 
-      // ---- Act: request the geometric means (Eq 9) this item needs ----
+      // ---- Act: the geometric means (Eq 9) the items of this warp need, one after the other, by the whole warp ----
       if constexpr (ACT) {
         // any zero makes the mean zero, and the centre belongs to its own neighbourhood: look at it first
         if (wantA | wantB) {
@@ -353,27 +351,20 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
             wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
           }
         }
-        const unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
-        const int nGA = __popc(mwA), nGw = nGA + __popc(mwB);
-        if (nGw) {   // warp-uniform
-          int base = 0;
-          if (lane == 0) base = atomicAdd(cnt + 1, nGw);
-          base = __shfl_sync(FULL, base, 0);
-          if (wantA) gmq[base + __popc(mwA & lt)] = make_uint2((uint32_t)(soff | (c << 9) | (tid << 14)), mA);
-          if (wantB) gmq[base + nGA + __popc(mwB & lt)] = make_uint2((uint32_t)(toff | (c << 9) | (tid << 14) | (1 << 21)), mB);
-        }
-        __syncthreads();
-        const int nG = cnt[1];
-        if (nG) {   // CTA-uniform
-          // one warp per request, lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of
-          // a request are in flight together
+        unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
+        if (mwA | mwB) {   // warp-uniform
+          // lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of a request are in flight together
           const int code = sncode[lane <= NNB ? lane : NNB];
           const int ddx = (code & 3) - 1, ddy = ((code >> 2) & 3) - 1, ddz = (DIM == 3) ? ((code >> 4) & 3) - 1 : 0;
           const int mynoff = (lane < NNB) ? snoff[lane] : 0;
-          for (int gi = wrp; gi < nG; gi += PK_WARPS) {
-            const uint2 rq = gmq[gi];
-            const int ctr = (int)(rq.x & 511u), cc = (int)((rq.x >> 9) & 31u);
-            const uint32_t mC = rq.y;
+          int gA = 0, gB = 0;
+          while (mwA | mwB) {
+            const bool sideB = mwA == 0u;
+            const int src = __ffs(sideB ? mwB : mwA) - 1;
+            if (sideB) mwB &= mwB - 1; else mwA &= mwA - 1;
+            const int ctr = __shfl_sync(FULL, sideB ? toff : soff, src);
+            const int cc = __shfl_sync(FULL, c, src);
+            const uint32_t mC = __shfl_sync(FULL, sideB ? mB : mA, src);
             const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
             // the centre is inside the lattice (its cell is not medium), possibly through the wrap
             int cx = orig[cc] - 1 + px, cy = orig[32 + cc] - 1 + py, cz = (DIM == 3) ? orig[64 + cc] - 1 + pz : 0;
@@ -400,24 +391,21 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
             if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
             const unsigned msame = __ballot_sync(FULL, same);
             const unsigned mzero = __ballot_sync(FULL, same && av == 0);
-            const int ssum = __reduce_add_sync(FULL, same ? slog[av] : 0);
-            if (lane == 0) {
-              int g = 0;
-              if (!mzero) { const int mm = ssum / __popc(msame); g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
-              gmout[((rq.x >> 14) & 127u) * 2 + (rq.x >> 21)] = g;
-            }
+            const int ssum = __reduce_add_sync(FULL, same ? __ldg(P.logq16 + av) : 0);
+            int g = 0;
+            if (!mzero) { const int mm = ssum / __popc(msame); g = __ldg(P.expq16 + ((mm >> 6) & 1023)) << (mm >> 16); }
+            if (lane == src) { if (sideB) gB = g; else gA = g; }
           }
-          __syncthreads();
-          long long sideA = 0, sideB = 0;
-          if (wantA) { const int g = gmout[tid * 2]; if (g != 0) sideA = act_side(pa.lamA, pa.maxA, g); }
-          if (wantB) { const int g = gmout[tid * 2 + 1]; if (g != 0) sideB = act_side(pb.lamA, pb.maxA, g); }
-          if (wantA || wantB) dH -= (sideA - sideB + 32768) >> 16;   // copies FROM active areas are favoured (L259)
+          long long sideA = 0, sideB2 = 0;
+          if (wantA && gA != 0) sideA = act_side(pa.lamA, pa.maxA, gA);
+          if (wantB && gB != 0) sideB2 = act_side(pb.lamA, pb.maxA, gB);
+          if (wantA || wantB) dH -= (sideA - sideB2 + 32768) >> 16;   // copies FROM active areas are favoured (L259)
         }
       }
 
       // ---- a8: Metropolis (Eq 2) against the integer threshold table; the acceptance word (Philox stream 1)
       //      is drawn only for uphill moves inside the table ----
-      bool acc = have && go;
+      acc = have && go;
       const bool uphill = acc && dH > 0 && !P.accept_all;
       if (uphill && dH > P.Hmax) acc = false;
       const bool draw = uphill && acc;
@@ -428,8 +416,10 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
           if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
         }
       }
+      maxA_new = pa.maxA;
       // ---- a9: the first accepted attempt of every chain wins ----
       if (acc) atomicMin(first + c, a);
+      }
       __syncthreads();
       const int fa = have ? first[c] : 0;
       if (have && a <= fa) ++n_eval;   // what lies before a chain's winner (and the winner) is final
@@ -460,7 +450,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
           P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
         }
         if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-          P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)pa.maxA;
+          P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)maxA_new;
         // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
         //      and, in deterministic mode, the chain's own-delta table
 #pragma unroll 1
@@ -510,7 +500,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         const int np = (fw < PK_NOWIN) ? fw + 1 : a_lim;
         spos[lane] = np;
         const bool redo = __any_sync(FULL, np < kk);
-        if (lane == 0) { cnt[1] = 0; cnt[2] = redo ? 1 : 0; }
+        if (lane == 0) cnt[2] = redo ? 1 : 0;
       }
       __syncthreads();
       if (cnt[2] == 0) break;

@@ -371,12 +371,14 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   }
   c->types = types;
   types[nT] = TypeParams{};
-  // adhesion difference table of the pooled kernel: D[a][b][n] = J(a,n) - J(b,n), then the diagonal J(t,t)
-  std::vector<int32_t> Dtab((size_t)nT * nT * nT + nT);
+  // adhesion difference table of the pooled kernel: D[a][b][n][frozen] = J(a,n) - J(b,n) (the byte offset into a
+  // row is the top byte of a lattice word: type * 8 + frozen * 4), then the diagonal J(t,t)
+  std::vector<int32_t> Dtab((size_t)2 * nT * nT * nT + nT);
   for (int a = 0; a < nT; ++a)
     for (int b2 = 0; b2 < nT; ++b2)
-      for (int n = 0; n < nT; ++n) Dtab[((size_t)a * nT + b2) * nT + n] = p->J[a * nT + n] - p->J[b2 * nT + n];
-  for (int t = 0; t < nT; ++t) Dtab[(size_t)nT * nT * nT + t] = p->J[t * nT + t];
+      for (int n = 0; n < nT; ++n)
+        for (int f = 0; f < 2; ++f) Dtab[(((size_t)a * nT + b2) * nT + n) * 2 + f] = p->J[a * nT + n] - p->J[b2 * nT + n];
+  for (int t = 0; t < nT; ++t) Dtab[(size_t)2 * nT * nT * nT + t] = p->J[t * nT + t];
 
   // ---- tiled layout of the pooled kernel: per colour, groups of 32 tiles of (S+2)^d words ----
   TileLayout &tl = sp.tl;
@@ -411,7 +413,11 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   if (c->pooled) {
     alloc((void **)&tl.tiles, c->tile_words * 4);
     if (c->mode == CPM_MODE_DETERMINISTIC) {
-      sp.ovf_cap = 65536;   // spill slots for chains that change more than PK_DCAP distinct cells in one activation
+      // spill slots for chains that change more than PK_DCAP distinct cells in one activation: one for every 8th
+      // chain of the largest colour (a few per cent of the chains need one), between 64 Ki and 1 Mi slots
+      unsigned long long most = 0;
+      for (int col = 0; col < 8; ++col) most = std::max(most, c->n_act_col[col]);
+      sp.ovf_cap = (int)std::min<unsigned long long>(std::max<unsigned long long>(most / 8, 65536ull), 1048576ull);
       alloc((void **)&c->ovf_keys, (size_t)sp.ovf_cap * PK_SPILL * 4);
       alloc((void **)&c->ovf_dvp, (size_t)sp.ovf_cap * PK_SPILL * 8);
     }

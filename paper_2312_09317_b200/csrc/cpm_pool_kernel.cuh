@@ -39,10 +39,16 @@ constexpr int PK_WARPS = 4;                  // warps per CTA = per group of 32 
 constexpr int PK_THREADS = 32 * PK_WARPS;
 constexpr int PK_CHUNK = 16;                 // attempts per chain between two pooled evaluations (4 per thread)
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
-constexpr int PK_DCAP = 4;                   // of which the first live in shared memory, the rest in a spill slot
+constexpr int PK_DCAP = 3;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
 constexpr int PK_NOWIN = PK_CHUNK;           // "no accepted attempt" in a chain's winner slot
-constexpr uint32_t CELL_MASK31 = 0x7FFFFFFFu;   // type + id: equal iff same cell
+// lattice word of the tiled layout: [type:5 | frozen:1 | 00 | id:24]: the top byte is the byte offset type * 8 +
+// frozen * 4 into a row of the adhesion table, so a neighbour's adhesion term costs one multiply-high, one load
+// and one add
+constexpr uint32_t PK_FROZEN = 1u << 26;
+constexpr uint32_t PK_CELL = ~PK_FROZEN;        // type + id: equal iff same cell
+constexpr int PK_TYPE_SHIFT = 27;
+constexpr uint32_t CELL_MASK31 = PK_CELL;
 
 template <int DIM, int S>
 struct PGeom {
@@ -74,23 +80,26 @@ struct PSmem {
   using G = PGeom<DIM, S>;
   static constexpr int TILE = 0;                                   // uint32 [TW][32]
   static constexpr int PROP = TILE + G::TW * 128;                  // uint16 [16][32]   toff | nb << 9
-  static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint16 [4 segments][128]  chain | a << 5
-  static constexpr int DKEY = QUEUE + PK_CHUNK * 64;               // uint32 [DCAP][32]
+  static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint8 [4 segments][128]  chain | (a & 3) << 5 (segment w holds attempts 4w..4w+3)
+  static constexpr int DKEY = QUEUE + PK_WARPS * PK_THREADS;               // uint32 [DCAP][32]
   static constexpr int DDVP = DKEY + PK_DCAP * 128;                // uint64 [DCAP][32]
-  static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] entries of the chain's own-delta table
-  static constexpr int DSLOT = DN + 128;                           // int [32] spill slot of the chain or -1
-  static constexpr int FIRST = DSLOT + 128;                        // int [32] first accepted attempt of the round
+  static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] own-delta table of the chain: entries | (spill slot + 1) << 8
+  static constexpr int FIRST = DN + 128;                           // int [32] first accepted attempt of the round
   static constexpr int POS = FIRST + 128;                          // int [32] attempts < pos of the chunk are final
-  static constexpr int BSUB = POS + 128;                           // uint32 [32] subsection index b of the chain
-  static constexpr int ORIG = BSUB + 128;                          // int [3][32] lattice origin of the chain
+  static constexpr int ORIG = POS + 128;                           // int [3][32] lattice origin of the chain
   static constexpr int NOFF = ORIG + 384;                          // int [32] neighbour -> tile offset (entry NNB = centre = 0)
-  static constexpr int NCODE = NOFF + 128;                         // int [32] neighbour -> (dx+1) | (dy+1) << 2 | (dz+1) << 4
-  static constexpr int TYPES = NCODE + 128;                        // TypeParams [9]
-  static constexpr int CNT = TYPES + 9 * 32;                       // int [8]: [1] request count, [2] redo flag, [4..7] queue segment lengths
+  static constexpr int CNT = NOFF + 128;                           // int [8]: [2] redo flag, [4..7] queue segment lengths
   static constexpr int MBAR = CNT + 32;                            // uint64
-  static constexpr int DTAB = MBAR + 16;                           // int32 [nT^3 + nT]
-  static constexpr size_t bytes(int nT) { return (size_t)DTAB + ((size_t)nT * nT * nT + nT) * 4; }
+  static constexpr int TYPES = MBAR + 16;                          // TypeParams [nT + 1], then int32 [nT][nT][nT][2] adhesion
+                                                                   // differences, then [nT] J(t,t)
+  static constexpr size_t bytes(int nT) { return (size_t)TYPES + (size_t)(nT + 1) * 32 + ((size_t)2 * nT * nT * nT + nT) * 4; }
 };
+
+// n += ((raw ^ w) & PK_CELL) == 0, as one logic op with a predicate result and one predicated add
+__device__ __forceinline__ void count_same(int &n, uint32_t raw, uint32_t w) {
+  asm("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tlop3.b32 t, %1, %2, %3, 0x28;\n\tsetp.eq.u32 p, t, 0;\n\t@p add.s32 %0, %0, 1;\n\t}"
+      : "+r"(n) : "r"(raw), "r"(w), "r"(PK_CELL));
+}
 
 __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -113,29 +122,26 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
 }
 
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
   constexpr int T = G::T, TW = G::TW, NNB = G::NNB;
   extern __shared__ __align__(128) unsigned char smem[];
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
   unsigned short *prop = reinterpret_cast<unsigned short *>(smem + M::PROP);
-  unsigned short *queue = reinterpret_cast<unsigned short *>(smem + M::QUEUE);
+  unsigned char *queue = smem + M::QUEUE;
   uint32_t *dkey = reinterpret_cast<uint32_t *>(smem + M::DKEY);
   unsigned long long *ddvp = reinterpret_cast<unsigned long long *>(smem + M::DDVP);
   int *dn = reinterpret_cast<int *>(smem + M::DN);
-  int *dslot = reinterpret_cast<int *>(smem + M::DSLOT);
   int *first = reinterpret_cast<int *>(smem + M::FIRST);
   int *spos = reinterpret_cast<int *>(smem + M::POS);
-  uint32_t *bsub = reinterpret_cast<uint32_t *>(smem + M::BSUB);
   int *orig = reinterpret_cast<int *>(smem + M::ORIG);
   int *snoff = reinterpret_cast<int *>(smem + M::NOFF);
-  int *sncode = reinterpret_cast<int *>(smem + M::NCODE);
-  TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
   int *cnt = reinterpret_cast<int *>(smem + M::CNT);
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + M::MBAR);
-  int32_t *sd = reinterpret_cast<int32_t *>(smem + M::DTAB);
-  const int32_t *sdiag = sd + P.nT * P.nT * P.nT;
+  TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
+  int32_t *sd = reinterpret_cast<int32_t *>(smem + M::TYPES + (P.nT + 1) * 32);
+  const int32_t *sdiag = sd + 2 * P.nT * P.nT * P.nT;
 
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const unsigned lt = (1u << lane) - 1u;
@@ -154,30 +160,27 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
     int dx = 0, dy = 0, dz = 0;
     if (tid < NNB) nb_delta<DIM>(tid, dx, dy, dz);
     snoff[tid] = (dz * T + dy) * T + dx;
-    sncode[tid] = (dx + 1) | ((dy + 1) << 2) | ((dz + 1) << 4);
-    dn[tid] = 0; dslot[tid] = -1; first[tid] = PK_NOWIN;
+    dn[tid] = 0; first[tid] = PK_NOWIN;
   }
   for (int i = tid; i < (P.nT + 1) * 8; i += PK_THREADS) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-  for (int i = tid; i < P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
+  for (int i = tid; i < 2 * P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
 
   // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk); its geometry is
   // worked out once, by warp 0 (the host limits n_active to 31 bits for this kernel)
   const uint32_t w = blockIdx.x * 32u + (uint32_t)lane;
   const bool active = w < (uint32_t)P.n_active;
   if (wrp == 0) {
-    uint32_t b0 = 0;
     int ox = 0, oy = 0, oz = 0;
     if (active) {
       const uint32_t ax = w % (uint32_t)P.nact[0], r1 = w / (uint32_t)P.nact[0];
       const uint32_t ay = r1 % (uint32_t)P.nact[1], az = r1 / (uint32_t)P.nact[1];
       const int bx = 2 * (int)ax + P.col[0], by = 2 * (int)ay + P.col[1], bz = (DIM == 3) ? 2 * (int)az + P.col[2] : 0;
-      b0 = (uint32_t)(bx + P.nsub[0] * (by + P.nsub[1] * bz));
       ox = bx * S; oy = by * S; oz = (DIM == 3) ? bz * S : 0;
     }
-    bsub[lane] = b0; orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz;
+    orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz;
   }
   __syncthreads();
-  const uint32_t b = bsub[lane];
+  const uint32_t b = active ? (uint32_t)(orig[lane] / S + P.nsub[0] * (orig[32 + lane] / S + P.nsub[1] * (orig[64 + lane] / S))) : 0u;
   const uint32_t mcs = *P.mcs_ptr;
   const int k = P.k;
   const int nchunk = (k + PK_CHUNK - 1) / PK_CHUNK;
@@ -226,13 +229,13 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
           const int a = 4 * wrp + j;
           const int toff = pr[j] & 511;
           const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[j] >> 9]) * 32];
-          in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && ((int)(wt | ws) >= 0);
+          in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u);
           m[j] = __ballot_sync(FULL, in[j]);
         }
         int base = wrp * PK_THREADS;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-          if (in[j]) queue[base + __popc(m[j] & lt)] = (unsigned short)(lane | ((4 * wrp + j) << 5));
+          if (in[j]) queue[base + __popc(m[j] & lt)] = (unsigned char)(lane | (j << 5));
           base += __popc(m[j]);
         }
         if (lane == 0) cnt[4 + wrp] = base - wrp * PK_THREADS;
@@ -257,7 +260,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
       if (have) {
         const int sg = (tid >= e0 ? 1 : 0) + (tid >= e1 ? 1 : 0) + (tid >= e2 ? 1 : 0);
         const int off = tid - (sg == 0 ? 0 : sg == 1 ? e0 : sg == 2 ? e1 : e2);
-        item = (int)queue[sg * PK_THREADS + off];
+        item = (int)queue[sg * PK_THREADS + off] | (sg << 7);   // chain | a << 5
       }
       c = item & 31; a = item >> 5;
       const int prc = (int)prop[a * 32 + c];
@@ -269,7 +272,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
       const uint32_t wB = tc[toff * 32];
       A = wA & ID_MASK; Bc = wB & ID_MASK;
       const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
-      const int tA = (int)(mA >> 24), tB = (int)(mB >> 24);
+      const int tA = (int)(wA >> PK_TYPE_SHIFT), tB = (int)(wB >> PK_TYPE_SHIFT);
       long long dH = 0;
       bool go = false;
       TypeParams pa = st[P.nT], pb = st[P.nT];
@@ -278,14 +281,14 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         unsigned long long baseA = 0ull, baseB = 0ull;
         if (A != 0) baseA = LIVE ? __ldcg(P.liveVP + A) : __ldg(P.snapVP + A);
         if (Bc != 0) baseB = LIVE ? __ldcg(P.liveVP + Bc) : __ldg(P.snapVP + Bc);
-        const int32_t *Drow = sd + (tA * P.nT + tB) * P.nT;
+        const char *Drow = reinterpret_cast<const char *>(sd + (tA * P.nT + tB) * P.nT * 2);   // [type][frozen] -> J(tA,type) - J(tB,type)
         int adh = 0;
 #pragma unroll
         for (int n = 0; n < NNB; ++n) {
           const uint32_t raw = tc[(toff + G::noff(n)) * 32];
-          if (((raw ^ wA) & CELL_MASK31) == 0u) ++nA;
-          if (((raw ^ wB) & CELL_MASK31) == 0u) ++nB;
-          adh += Drow[(raw >> 24) & 127u];
+          count_same(nA, raw, wA);
+          count_same(nB, raw, wB);
+          adh += *reinterpret_cast<const int32_t *>(Drow + (raw >> 24));
         }
         // a neighbour of cell A has type tA: its J(tA,tA) term drops out (sigma_n == A); same for B
         adh += nB * sdiag[tB] - nA * sdiag[tA];
@@ -293,7 +296,8 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         // a6: per-cell {V,P} as this attempt sees it: snapshot + the chain's own deltas / live
         unsigned long long vpA = baseA, vpB = baseB;
         if constexpr (!LIVE) {
-          const int ne = dn[c];
+          const int di = dn[c];
+          const int ne = di & 255;
           if (ne > 0) {
             unsigned long long dA = 0ull, dB = 0ull;
             const int ns = min(ne, PK_DCAP);
@@ -304,7 +308,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
               if (key == Bc) dB = v;
             }
             if (ne > PK_DCAP) {
-              const long long sl = (long long)dslot[c] * PK_SPILL;
+              const long long sl = (long long)((di >> 8) - 1) * PK_SPILL;
               for (int i = 0; i < ne - PK_DCAP; ++i) {
                 const uint32_t key = __ldcg(P.ovf_keys + sl + i);
                 const unsigned long long v = __ldcg(P.ovf_dvp + sl + i);
@@ -354,8 +358,8 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
         unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
         if (mwA | mwB) {   // warp-uniform
           // lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of a request are in flight together
-          const int code = sncode[lane <= NNB ? lane : NNB];
-          const int ddx = (code & 3) - 1, ddy = ((code >> 2) & 3) - 1, ddz = (DIM == 3) ? ((code >> 4) & 3) - 1 : 0;
+          int ddx = 0, ddy = 0, ddz = 0;
+          if (lane < NNB) nb_delta<DIM>(lane, ddx, ddy, ddz);
           const int mynoff = (lane < NNB) ? snoff[lane] : 0;
           int gA = 0, gB = 0;
           while (mwA | mwB) {
@@ -412,7 +416,7 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
       if (__any_sync(FULL, draw)) {
         if (draw) {
           const int ag = ch * PK_CHUNK + a;
-          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, bsub[c], 2u * P.p + 1u, mcs), P.key0, P.key1);
+          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)(orig[c] / S + P.nsub[0] * (orig[32 + c] / S + P.nsub[1] * (orig[64 + c] / S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
           if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
         }
       }
@@ -465,29 +469,29 @@ __global__ void __launch_bounds__(PK_THREADS, 6) sweep_pool_kernel(const __grid_
           atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
           if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
           if constexpr (!LIVE) {
-            const int ne = dn[c];
+            const int di = dn[c];
+            const int ne = di & 255;
+            int slot = (di >> 8) - 1;
             bool hit = false;
             const int ns = min(ne, PK_DCAP);
             for (int i = 0; i < ns; ++i)
               if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
             if (!hit && ne > PK_DCAP) {
-              const long long sl = (long long)dslot[c] * PK_SPILL;
+              const long long sl = (long long)slot * PK_SPILL;
               for (int i = 0; i < ne - PK_DCAP; ++i)
                 if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
             }
             if (!hit) {
-              if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = ne + 1; }
+              if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = di + 1; }
               else if (ne < PK_CAP) {
-                int slot = dslot[c];
                 if (slot < 0) {
                   slot = atomicAdd(P.ovf_count, 1);
                   if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
-                  dslot[c] = slot;
                 }
                 if (slot >= 0) {
                   const long long sl = (long long)slot * PK_SPILL;
                   P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
-                  dn[c] = ne + 1;
+                  dn[c] = (ne + 1) | ((slot + 1) << 8);
                 }
               } else overflow = true;
             }
@@ -549,7 +553,7 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
         const long long gi = (long long)x + (long long)X * ((long long)y + (long long)Y * z);
         uint32_t id = ids[gi];
         if (id > max_cells) { atomicOr(error_flag, 2); id = 0; }
-        word = id | ((uint32_t)ctype[id] << 24) | ((frozen && frozen[gi]) ? 0x80000000u : 0u);
+        word = id | ((uint32_t)ctype[id] << PK_TYPE_SHIFT) | ((frozen && frozen[gi]) ? PK_FROZEN : 0u);
       }
     }
     L.tiles[L.base[col] + i] = word;

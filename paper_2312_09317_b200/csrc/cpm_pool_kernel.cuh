@@ -41,7 +41,7 @@ constexpr int PK_CHUNK = 16;                 // attempts per chain between two p
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 3;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
-constexpr int PK_NOWIN = PK_CHUNK;           // "no accepted attempt" in a chain's winner slot
+constexpr int PK_NOWIN = PK_CHUNK << 10;     // "no accepted attempt": a chain's winner slot holds a << 10 | n_A << 5 | n_B
 // lattice word of the tiled layout: [type:5 | frozen:1 | 00 | id:24]: the top byte is the byte offset type * 8 +
 // frozen * 4 into a row of the adhesion table, so a neighbour's adhesion term costs one multiply-high, one load
 // and one add
@@ -88,8 +88,9 @@ struct PSmem {
   static constexpr int POS = FIRST + 128;                          // int [32] attempts < pos of the chunk are final
   static constexpr int ORIG = POS + 128;                           // int [3][32] lattice origin of the chain
   static constexpr int NOFF = ORIG + 384;                          // int [32] neighbour -> tile offset (entry NNB = centre = 0)
-  static constexpr int CNT = NOFF + 128;                           // int [8]: [2] redo flag, [4..7] queue segment lengths
-  static constexpr int MBAR = CNT + 32;                            // uint64
+  static constexpr int CNT = NOFF + 128;                           // int [8]: [2] redo flag, [3] chains that continue, [4..7] queue segment lengths
+  static constexpr int RLIST = CNT + 32;                           // uint8 [32] the chains that continue in the next round
+  static constexpr int MBAR = RLIST + 32;                            // uint64
   static constexpr int TYPES = MBAR + 16;                          // TypeParams [nT + 1], then int32 [nT][nT][nT][2] adhesion
                                                                    // differences, then [nT] J(t,t)
   static constexpr size_t bytes(int nT) { return (size_t)TYPES + (size_t)(nT + 1) * 32 + ((size_t)2 * nT * nT * nT + nT) * 4; }
@@ -138,6 +139,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
   int *orig = reinterpret_cast<int *>(smem + M::ORIG);
   int *snoff = reinterpret_cast<int *>(smem + M::NOFF);
   int *cnt = reinterpret_cast<int *>(smem + M::CNT);
+  unsigned char *rlist = smem + M::RLIST;
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + M::MBAR);
   TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
   int32_t *sd = reinterpret_cast<int32_t *>(smem + M::TYPES + (P.nT + 1) * 32);
@@ -216,11 +218,12 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
     }
     __syncthreads();
 
+    bool first_round = true;
     while (true) {
-      // ---- a4: screen the not yet final attempts this thread owns; every warp compacts the survivors of its four
-      //      attempt indices into its own queue segment (segment w holds attempts 4w..4w+3 of all chains) ----
       if (wrp == 0) first[lane] = PK_NOWIN;   // nobody touches the winner slots before the next barrier
-      {
+      if (first_round || cnt[3] > 8) {
+        // ---- a4: screen the not yet final attempts this thread owns; every warp compacts the survivors of its four
+        //      attempt indices into its own queue segment (segment w holds attempts 4w..4w+3 of all chains) ----
         const int ps = spos[lane];
         bool in[4];
         unsigned m[4];
@@ -239,7 +242,24 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
           base += __popc(m[j]);
         }
         if (lane == 0) cnt[4 + wrp] = base - wrp * PK_THREADS;
+      } else {
+        // ---- a4 for the few (<= 8) chains that continue behind an accepted copy: thread (r, a) screens attempt a
+        //      of the r-th such chain; the segment counters were cleared at the end of the last round ----
+        const int r = tid >> 4, a = tid & 15;
+        if (r < cnt[3]) {
+          const int c = (int)rlist[r];
+          if (a >= spos[c] && a < kk) {
+            const int prc = (int)prop[a * 32 + c];
+            const int toff = prc & 511;
+            const uint32_t wt = tile[toff * 32 + c], ws = tile[(toff + snoff[prc >> 9]) * 32 + c];
+            if ((((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u)) {
+              const int sg = a >> 2;
+              queue[sg * PK_THREADS + atomicAdd(cnt + 4 + sg, 1)] = (unsigned char)(c | ((a & 3) << 5));
+            }
+          }
+        }
       }
+      first_round = false;
       __syncthreads();
       // a round takes the leading segments that fit one item per thread (nearly always all four); the attempts
       // of the others are screened again in the next round
@@ -252,9 +272,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
 
       // ---- a5-a7: one item per thread; warps without items go straight to the barrier ----
       const bool have = tid < W;
-      int c = 0, a = 0, toff = 0, nA = 0, nB = 0, maxA_new = 0;
-      uint32_t wA = 0u, A = 0u, Bc = 0u;
-      bool acc = false;
+      int c = 0, a = 0;
       if (32 * wrp < W) {   // warp-uniform
       int item = 0;
       if (have) {
@@ -264,13 +282,12 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
       }
       c = item & 31; a = item >> 5;
       const int prc = (int)prop[a * 32 + c];
-      toff = prc & 511;
-      const int nb = prc >> 9;
+      const int toff = prc & 511, nb = prc >> 9;
+      int nA = 0, nB = 0;
       const int soff = toff + snoff[nb];
       const uint32_t *const tc = tile + c;
-      wA = tc[soff * 32];
-      const uint32_t wB = tc[toff * 32];
-      A = wA & ID_MASK; Bc = wB & ID_MASK;
+      const uint32_t wA = tc[soff * 32], wB = tc[toff * 32];
+      const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
       const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
       const int tA = (int)(wA >> PK_TYPE_SHIFT), tB = (int)(wB >> PK_TYPE_SHIFT);
       long long dH = 0;
@@ -409,7 +426,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
 
       // ---- a8: Metropolis (Eq 2) against the integer threshold table; the acceptance word (Philox stream 1)
       //      is drawn only for uphill moves inside the table ----
-      acc = have && go;
+      bool acc = have && go;
       const bool uphill = acc && dH > 0 && !P.accept_all;
       if (uphill && dH > P.Hmax) acc = false;
       const bool draw = uphill && acc;
@@ -420,15 +437,21 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
           if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
         }
       }
-      maxA_new = pa.maxA;
       // ---- a9: the first accepted attempt of every chain wins ----
-      if (acc) atomicMin(first + c, a);
+      if (acc) atomicMin(first + c, (a << 10) | (nA << 5) | nB);
       }
       __syncthreads();
-      const int fa = have ? first[c] : 0;
-      if (have && a <= fa) ++n_eval;   // what lies before a chain's winner (and the winner) is final
-      if (acc && a == fa) {
-        // ---- a9/a10: this thread evaluated the winner of chain c: it commits it ----
+      if (have && a <= (first[c] >> 10)) ++n_eval;   // what lies before a chain's winner (and the winner) is final
+      if (wrp == 0 && first[lane] < PK_NOWIN) {
+        // ---- a9/a10: warp 0, lane = chain, commits the winners (n_A, n_B come with the winner slot; the tile still
+        //      holds the state of the round's start) ----
+        const int fw = first[lane];
+        const int c = lane, nA = (fw >> 5) & 31, nB = fw & 31;
+        const int prc = (int)prop[(fw >> 10) * 32 + c];
+        const int toff = prc & 511;
+        const uint32_t wA = tcol[(toff + snoff[prc >> 9]) * 32], wB = tcol[toff * 32];
+        const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
+        const int maxA_new = (A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0;
         ++n_acc;
         tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
         gtile[toff * 32 + c] = wA;           // home word in HBM
@@ -501,10 +524,12 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
       if (wrp == 0) {
         // chains with an accepted copy continue behind it on the new state, the others behind the attempts covered
         const int fw = first[lane];
-        const int np = (fw < PK_NOWIN) ? fw + 1 : a_lim;
+        const int np = (fw < PK_NOWIN) ? (fw >> 10) + 1 : max(spos[lane], a_lim);
         spos[lane] = np;
-        const bool redo = __any_sync(FULL, np < kk);
-        if (lane == 0) cnt[2] = redo ? 1 : 0;
+        const unsigned rm = __ballot_sync(FULL, np < kk);
+        if (np < kk) rlist[__popc(rm & lt)] = (unsigned char)lane;
+        if (lane == 0) { cnt[2] = rm != 0u; cnt[3] = __popc(rm); }
+        if (lane < 4) cnt[4 + lane] = 0;
       }
       __syncthreads();
       if (cnt[2] == 0) break;

@@ -28,12 +28,15 @@ sys.path.insert(0, ROOT)
 
 METRIC = "copy_attempts_per_s"
 UNIT = "attempts/s"
-# algorithmic bytes per copy attempt of the sweep kernel in THIS layout:
-# id word read + write-back (4+4 B), Act byte read + write-back (1+1 B)
-BYTES_PER_ATTEMPT_ACT = 10.0
-BYTES_PER_ATTEMPT_NOACT = 8.0
-# SURVEY.md 8(d)'s model (float32 Act field, explicit decay folded in): 8 B / 16 B
+# ALGORITHMIC bytes per copy attempt, SURVEY.md 8(d)'s model: id word read + write-back
+# = 8 B; with the Act extension + 8 B (float32 Act read + write-back, decay folded in) = 16 B.  roofline.achieved
+# and roofline.frac use this figure.
 SURVEY_BYTES_ACT, SURVEY_BYTES_NOACT = 16.0, 8.0
+# what THIS layout has to move per attempt (extra key roofline.frac_layout_bytes): id word read + write-back
+# (4 + 4 B), Act byte read + write-back (1 + 1 B)
+LAYOUT_BYTES_ACT, LAYOUT_BYTES_NOACT = 10.0, 8.0
+BURN_IN_MCS = 10          # 10 MCS burn-in before anything is timed (the first MCS are a transient)
+CPU_SAMPLE_3D, CPU_SAMPLE_2D = 256, 4096   # edge of the corner crop both oracle legs run
 
 
 def parse_dims(s):
@@ -108,6 +111,39 @@ class ClockSampler:
         return out
 
 
+def source_hash():
+    """SHA-256 over the CUDA sources the library is built from: ties a stored ncu figure to the code it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2312_09317_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(name.encode()); h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def static_capture(config, dims, S):
+    """DRAM bytes per sweep launch (and warp-instructions per attempt) from the committed `ncu --set full` capture,
+    profiles/traffic_per_launch.csv.  It is a STATIC figure: it is only reported when the capture was taken on the
+    very kernel sources being timed (source_hash), otherwise traffic is null."""
+    tpath = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")
+    try:
+        rows = [r.split(",") for r in open(tpath).read().splitlines()]
+        hdr, rows = rows[0], rows[1:]
+        key = "%s_%s" % (config, "x".join(map(str, dims)))
+        cur = source_hash()
+        for f in rows:
+            r = dict(zip(hdr, f))
+            if r["workload"] == key and int(r["subsection"]) == S:
+                if r.get("source_hash") != cur:
+                    return None, "stale: %s was captured on sources %s, timed sources are %s" % (r.get("source"), r.get("source_hash"), cur), None
+                wipa = float(r["warp_instr_per_attempt"]) if r.get("warp_instr_per_attempt") else None
+                return int(r["dram_bytes_per_sweep_launch"]), "static ncu capture %s (sources %s)" % (r.get("source"), cur), {"warp_instr_per_attempt": wipa}
+    except Exception:
+        pass
+    return None, "no capture for this workload", None
+
+
 def build_workload(name, dims, rank):
     import cpm_inputs as ci
     cfg = ci.make_config(name, dims=dims)
@@ -130,13 +166,36 @@ def reduce_over_ranks(times, counts, world, device):
     return [float(v) for v in t.tolist()], [int(v) for v in c.tolist()]
 
 
-def oracle_rate(cfg, sample_dims, n_mcs, warm=0):
-    """Attempts/s of the oracle, as it stands, on a corner crop of the workload (one host core)."""
+def host_info():
+    """What SURVEY.md 8(d) asks to print beside the oracle's time: core count and CPU model of the box."""
+    model = "unknown"
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model}
+
+
+def cpu_sample_dims(dims):
+    return tuple(min(d, CPU_SAMPLE_3D if len(dims) == 3 else CPU_SAMPLE_2D) for d in dims)
+
+
+def make_oracle(cfg, sample_dims, params):
+    """The oracle, as it stands, on a corner crop of the workload, with the schedule of the GPU leg (same S, k)."""
     import cpm_inputs as ci
     from oracle import binding as ob
     crop = ci.crop_config(cfg, sample_dims)
-    o = ob.Oracle(crop["dims"], max_cells=crop["max_cells"], **crop["params"])
+    o = ob.Oracle(crop["dims"], max_cells=crop["max_cells"], **params)
     o.set_lattice(crop["ids"], crop["frozen"], crop["cell_type"])
+    return o
+
+
+def oracle_rate(cfg, sample_dims, params, n_mcs, warm=0):
+    """Attempts/s of the oracle on the crop (one host core), over n_mcs MCS after `warm` untimed ones."""
+    o = make_oracle(cfg, sample_dims, params)
     if warm:
         o.step(warm)
     t0 = time.perf_counter()
@@ -146,33 +205,31 @@ def oracle_rate(cfg, sample_dims, n_mcs, warm=0):
     return n / dt, dt
 
 
+def sample_text(sample, cfg_name, first, n_mcs):
+    return "corner crop %s of the %s workload, MCS %d..%d of the run, 1 MCS per step, one core" % (
+        "x".join(map(str, sample)), cfg_name, first + 1, first + n_mcs)
+
+
 def run_reference(args, rank, world):
     """--impl reference: the oracle on the host cores, bounded sample per step."""
     if rank != 0:
         return
-    dims = parse_dims(args.dims) if args.dims else (1024, 1024, 1024)
-    sample = tuple(min(d, 128) for d in dims)
-    gen_dims = tuple(min(d, 256) for d in dims)       # the crop only needs the corner of the workload
-    cfg = build_workload(args.config, gen_dims, 0)
-    import cpm_inputs as ci
-    from oracle import binding as ob
-    crop = ci.crop_config(cfg, sample)
-    o = ob.Oracle(crop["dims"], max_cells=crop["max_cells"], **crop["params"])
-    o.set_lattice(crop["ids"], crop["frozen"], crop["cell_type"])
-    o.step(args.warmup)
-    t0 = time.perf_counter()
-    o.step(args.steps)
-    dt = time.perf_counter() - t0
+    cfg = build_workload(args.config, parse_dims(args.dims) if args.dims else None, 0)   # the workload of the ours arm
+    dims = cfg["dims"]
+    sample = cpu_sample_dims(dims)                    # the same crop the cpu_baseline leg of the ours arm runs
+    params = dict(cfg["params"]); params["subsection"] = args.subsection
+    value, dt = oracle_rate(cfg, sample, params, args.steps, warm=args.warmup)
     n_step = int(np.prod(sample))
-    value = n_step * args.steps / dt
-    sample_txt = "corner crop %s of the %s workload, 1 MCS per step" % ("x".join(map(str, sample)), args.config)
+    sample_txt = sample_text(sample, args.config, args.warmup, args.steps)
+    hi = host_info()
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int64", "data": "synthetic",
         "config": {"workload": "%s %s (oracle on a bounded sample)" % (args.config, "x".join(map(str, dims))),
                    "sample": sample_txt},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample_txt},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample_txt,
+                         "nproc": hi["nproc"], "cpu_model": hi["cpu_model"]},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "mcs_per_s_on_sample": args.steps / dt,
     }
@@ -191,8 +248,9 @@ def main():
     ap.add_argument("--mode", type=int, default=0, help="0 deterministic (default), 1 live atomics")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-live", action="store_true", help="skip the extra LIVE-mode measurement")
     args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    args.warmup = max(args.warmup, BURN_IN_MCS)   # both arms: the same burn-in, so the same MCS window is timed
 
     rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
     if args.impl == "reference":
@@ -271,27 +329,54 @@ def main():
 
     (ms, e2e_s, sweep_ms), (launches,) = reduce_over_ranks([ms, e2e_s, sweep_ms], [launches], world, "cuda")
 
+    # ---- extra: the paper-faithful LIVE mode (atomics on live per-cell values, L51-53) on the same workload ----
+    live = None
+    if args.mode == 0 and not args.no_live:
+        del g
+        gl = pk.CPM(dims, max_cells=cfg["max_cells"], mode=1, device=local, **params)
+        gl.set_lattice(ids_h, frozen_h, ctype_h)
+        gl.step(args.warmup)
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_live = min(args.steps, 5)
+        f0.record()
+        gl.step(n_live)
+        f1.record()
+        barrier()
+        live_ms = f0.elapsed_time(f1)
+        (live_ms,), _ = reduce_over_ranks([live_ms], [0], world, "cuda")
+        live = {"value": world * N * n_live / (live_ms * 1e-3), "unit": UNIT, "ms_per_step": live_ms / n_live, "steps": n_live}
+        del gl
+
     if rank == 0:
         value = world * N * args.steps / (ms * 1e-3)
         e2e_value = world * N * e2e_steps / e2e_s
         peak, peak_src = measured_peak_gbs()
-        bpa = BYTES_PER_ATTEMPT_ACT if act_on else BYTES_PER_ATTEMPT_NOACT
+        bpa = SURVEY_BYTES_ACT if act_on else SURVEY_BYTES_NOACT
+        layout_bpa = LAYOUT_BYTES_ACT if act_on else LAYOUT_BYTES_NOACT
         attempts_per_launch = N * args.steps / max(sweep_n, 1)
         avg_launch_s = (sweep_ms * 1e-3) / max(sweep_n, 1)
         achieved = bpa * attempts_per_launch / avg_launch_s / 1e9
-        survey_bpa = SURVEY_BYTES_ACT if act_on else SURVEY_BYTES_NOACT
-        traffic = None
-        # dram bytes per sweep launch from the committed ncu --set full capture (profiles/traffic_per_launch.csv)
-        tpath = os.path.join(ROOT, "profiles", "traffic_per_launch.csv")
-        if os.path.exists(tpath):
-            try:
-                key = "%s_%s" % (args.config, "x".join(map(str, dims)))
-                for row in open(tpath).read().splitlines()[1:]:
-                    f = row.split(",")
-                    if f[0] == key and int(f[1]) == sched["S"]:
-                        traffic = int(f[2])
-            except Exception:
-                traffic = None
+        kernel_name = "sweep_pool_kernel" if info0["pooled"] else "sweep_kernel"
+        traffic, traffic_src, prof = static_capture(args.config, dims, sched["S"])
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "traffic_source": traffic_src, "kernel": kernel_name, "bytes_per_attempt": bpa,
+                "launches_timed": int(sweep_n), "avg_launch_ms": 1e3 * avg_launch_s, "peak_source": peak_src,
+                "kernel_share_of_step": sweep_ms / ms,
+                "frac_layout_bytes": layout_bpa * attempts_per_launch / avg_launch_s / 1e9 / peak,
+                "layout_bytes_per_attempt": layout_bpa,
+                # what limits the kernel today is not HBM: issue slots and barrier latency
+                "limiter": "issue/latency (DESIGN.md section 7), not HBM"}
+        if prof and prof.get("warp_instr_per_attempt"):
+            # the plain-ALU side SURVEY.md 8(d) asks for: warp-instructions issued per second against
+            # SMs x 4 schedulers x SM clock (one warp-instruction per scheduler and cycle)
+            sm_mhz = clocks.get("sm_mhz") or 1965.0
+            issue_peak = 148 * 4 * sm_mhz * 1e6
+            roof["alu"] = {"warp_instr_per_attempt": prof["warp_instr_per_attempt"],
+                           "achieved": prof["warp_instr_per_attempt"] * attempts_per_launch / avg_launch_s,
+                           "peak": issue_peak, "unit": "warp-instr/s",
+                           "frac": prof["warp_instr_per_attempt"] * attempts_per_launch / avg_launch_s / issue_peak,
+                           "source": traffic_src}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -299,31 +384,30 @@ def main():
             "config": {"workload": "%s %s" % (args.config, "x".join(map(str, dims))), "cells": int(cfg["max_cells"]),
                        "mode": "deterministic" if args.mode == 0 else "live_atomics", "subsection": sched["S"],
                        "attempts_per_activation": sched["k"], "phase_steps_per_mcs": sched["phase_steps_per_mcs"],
-                       "act": bool(act_on), "l2": "inputs larger than L2 (no flush needed)",
+                       "act": bool(act_on), "l2": "inputs larger than L2 (no flush needed)", "burn_in_mcs": args.warmup,
                        "parallelism": "replicas x%d" % world, "input_generation_s": round(t_gen, 1)},
             "mcs_per_s": world * args.steps / (ms * 1e-3),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "kernel": "sweep_pool_kernel" if info0["pooled"] else "sweep_kernel", "bytes_per_attempt": bpa,
-                         "launches_timed": int(sweep_n), "avg_launch_ms": 1e3 * avg_launch_s, "peak_source": peak_src,
-                         "kernel_share_of_step": sweep_ms / ms,
-                         "frac_with_survey_model_bytes": survey_bpa * attempts_per_launch / avg_launch_s / 1e9 / peak},
+            "roofline": roof,
             "counters": {"evaluated_frac": counters["evaluated"] / max(counters["attempts"], 1),
                          "accepted_frac": counters["accepted"] / max(counters["attempts"], 1)},
         }
+        if live is not None:
+            line["live_mode"] = live
         if not args.no_cpu_baseline:
-            sample = tuple(min(d, 256 if len(dims) == 3 else 4096) for d in dims)
-            n_mcs = 3
+            sample = cpu_sample_dims(dims)
+            hi = host_info()
+            n_mcs = min(args.steps, 10)
+            base = {"unit": UNIT, "cores": 1, "kind": "oracle", "nproc": hi["nproc"], "cpu_model": hi["cpu_model"]}
             try:
-                v, dt = oracle_rate(cfg, sample, n_mcs)
-                line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                        "sample": "corner crop %s of the workload, first %d MCS (%.1f s)" % (
-                                            "x".join(map(str, sample)), n_mcs, dt)}
+                v, dt = oracle_rate(cfg, sample, params, n_mcs, warm=args.warmup)
+                base.update({"value": v, "sample": sample_text(sample, args.config, args.warmup, n_mcs) + " (%.1f s timed)" % dt})
             except Exception as ex:  # the baseline is a reported extra, never a reason to lose the bench line
-                line["cpu_baseline"] = {"value": None, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "failed: %r" % (ex,)}
+                base.update({"value": None, "sample": "failed: %r" % (ex,)})
+            line["cpu_baseline"] = base
         print(json.dumps(line))
     if world > 1:
         dist.barrier()

@@ -362,72 +362,3 @@ def test_C4_256_cubed_scheduler_choice_bit_exact(pk, oracle_mod):
     g, o = _run(pk, oracle_mod, cfg, 3, 1, act=True, subsection=0)
     assert g.get_schedule() == {"S": 4, "k": 64, "phase_steps_per_mcs": 8}
     assert g.get_launch_info()["pooled"]
-
-
-def test_C4_full_size_properties(pk):
-    """BASELINE config 4 at its full size (1024^3, ~1.04 M cells, 20 % obstacles) in bench.py's launch
-    configuration.  The oracle needs > 1 min per MCS here, so this checks what must hold at any size:
-    (i) the volume and coordinate-sum tallies equal a recount of the lattice (the paper's invariant, L57,
-    L288); (ii) perimeters equal a recount for every cell that lies inside a 128^3 corner block;
-    (iii) obstacle voxels never change and no cell disappears; (iv) a second context with the same
-    seed reproduces the lattice bit for bit (counter-based RNG, deterministic mode)."""
-    import cpm_inputs as ci
-    cfg = ci.make_config("C4")
-    assert cfg["dims"] == (1024, 1024, 1024)
-    params = dict(cfg["params"]); params["subsection"] = 0
-    n = cfg["max_cells"] + 1
-
-    def run():
-        g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], **params)
-        g.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
-        g.step(2)
-        return g, g.get_lattice()
-
-    g, lat = run()
-    assert g.get_launch_info()["pooled"] and g.get_schedule()["S"] == 4
-    st = g.get_cell_stats()
-    c = g.get_counters()
-    assert c["attempts"] == 2 * 1024 ** 3 and 0 < c["accepted"] < c["evaluated"] < c["attempts"]
-    assert (lat != cfg["ids"]).any()
-
-    # (i) volumes and coordinate sums, slab by slab
-    V = np.zeros(n, np.int64); sx = np.zeros(n, np.int64); sy = np.zeros(n, np.int64); sz = np.zeros(n, np.int64)
-    xs = np.arange(1024, dtype=np.float64)
-    for z0 in range(0, 1024, 32):
-        blk = lat[z0:z0 + 32].reshape(-1).astype(np.int64)
-        V += np.bincount(blk, minlength=n)
-        sx += np.bincount(blk, weights=np.tile(xs, 32 * 1024), minlength=n).astype(np.int64)
-        sy += np.bincount(blk, weights=np.tile(np.repeat(xs, 1024), 32), minlength=n).astype(np.int64)
-        sz += np.bincount(blk, weights=np.repeat(xs[z0:z0 + 32], 1024 * 1024), minlength=n).astype(np.int64)
-    for a in (V, sx, sy, sz):
-        a[0] = 0
-    np.testing.assert_array_equal(st["volume"].astype(np.int64), V)
-    np.testing.assert_array_equal(st["sum_x"].astype(np.int64), sx)
-    np.testing.assert_array_equal(st["sum_y"].astype(np.int64), sy)
-    np.testing.assert_array_equal(st["sum_z"].astype(np.int64), sz)
-
-    # (ii) perimeters of the cells that lie strictly inside the 128^3 corner block
-    B = 128
-    blk = lat[:B, :B, :B]
-    Vb, Pb, _, _, _ = H.recount(blk, cfg["max_cells"], 3)
-    face = np.zeros(n, bool)
-    for sl in (blk[-1], blk[:, -1], blk[:, :, -1]):     # faces towards the rest of the lattice
-        face[np.unique(sl)] = True
-    inside = (Vb > 0) & (Vb == V) & ~face
-    inside[0] = False
-    assert inside.sum() > 500
-    np.testing.assert_array_equal(st["perimeter"].astype(np.int64)[inside], Pb[inside])
-
-    # (iii) obstacles and conservation
-    fz = cfg["frozen"].astype(bool)
-    assert (lat[fz] == cfg["ids"][fz]).all()
-    V0 = np.bincount(cfg["ids"].reshape(-1).astype(np.int64), minlength=n)
-    assert ((V[1:] > 0) == (V0[1:] > 0)).all()
-
-    # (iv) reproducibility
-    del g
-    g2, lat2 = run()
-    assert np.array_equal(lat, lat2)
-    st2 = g2.get_cell_stats()
-    for k in st:
-        np.testing.assert_array_equal(st[k], st2[k])

@@ -313,6 +313,13 @@ def main():
     launches = g.get_launch_info()["launches"] - l0
     clocks = sampler.stop()
     counters = g.get_counters()
+    # the same K steps again the way cpm_step runs them for a user: one CUDA graph per MCS, no per-launch events
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record()
+    g.step(args.steps)
+    g1.record()
+    barrier()
+    graph_ms = g0.elapsed_time(g1)
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the inputs, MCS, D2H of the lattice ----
     e2e_steps = max(1, min(args.e2e_steps, args.steps))
@@ -327,7 +334,7 @@ def main():
     h2d = ids_h.numel() * 4 + (frozen_h.numel() if frozen_h is not None else 0) + ctype_h.numel()
     d2h = out_h.numel() * 4
 
-    (ms, e2e_s, sweep_ms), (launches,) = reduce_over_ranks([ms, e2e_s, sweep_ms], [launches], world, "cuda")
+    (ms, e2e_s, sweep_ms, graph_ms), (launches,) = reduce_over_ranks([ms, e2e_s, sweep_ms, graph_ms], [launches], world, "cuda")
 
     # ---- extra: the paper-faithful LIVE mode (atomics on live per-cell values, L51-53) on the same workload ----
     live = None
@@ -390,6 +397,9 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps},
             "gpu_launches": int(launches),
+            # the timed region above launches the kernels one by one with an event pair around every sweep launch;
+            # this is the same K steps replayed as CUDA graphs (what cpm_step does when per-launch timing is off)
+            "graph_replay": {"value": world * N * args.steps / (graph_ms * 1e-3), "unit": UNIT, "ms_per_step": graph_ms / args.steps},
             "clocks": clocks,
             "roofline": roof,
             "counters": {"evaluated_frac": counters["evaluated"] / max(counters["attempts"], 1),

@@ -33,7 +33,8 @@ enum { CPM_OK = 0, CPM_ERR_ARG = -1, CPM_ERR_DIMS = -2, CPM_ERR_UNSUPPORTED = -3
 enum { CPM_MOORE = 0 }; /* the only neighbourhood the paper uses (L225): 8 / 26 neighbours */
 enum {
   CPM_FLAG_WARP_KERNEL = 1, /* use the warp-per-subsection kernel even where the pooled kernel applies */
-  CPM_FLAG_NO_TMA = 2       /* warp-per-subsection kernel: stage tiles with plain loads instead of TMA */
+  CPM_FLAG_NO_TMA = 2,      /* warp-per-subsection kernel: stage tiles with plain loads instead of TMA */
+  CPM_FLAG_NO_GRAPH = 4     /* launch the kernels of an MCS one by one instead of as one CUDA graph per MCS */
 };
 enum {
   CPM_MODE_DETERMINISTIC = 0, /* per-cell state read from a phase-start snapshot + the worker's own
@@ -87,7 +88,8 @@ int  cpm_set_mcs(cpm_ctx *ctx, uint32_t mcs);
 
 /* Run n_mcs Monte Carlo steps (one MCS = N copy attempts, L65): for each repetition and each
  * of the 2^d checkerboard colours, all subsections of that colour run k sequential copy
- * attempts concurrently (L49); then the Act field decays by 1 (L255).  Asynchronous. */
+ * attempts concurrently (L49); then the Act field decays by 1 (L255).  Asynchronous: the launches of one
+ * MCS are captured once into a CUDA graph and replayed on the context's stream. */
 int  cpm_step(cpm_ctx *ctx, uint32_t n_mcs);
 
 int  cpm_get_lattice(cpm_ctx *ctx, uint32_t *ids, int on_device);

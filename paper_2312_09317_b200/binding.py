@@ -12,7 +12,7 @@ import numpy as np
 from . import build as _build
 
 MODE_DETERMINISTIC, MODE_LIVE_ATOMICS = 0, 1
-FLAG_WARP_KERNEL, FLAG_NO_TMA = 1, 2
+FLAG_WARP_KERNEL, FLAG_NO_TMA, FLAG_NO_GRAPH = 1, 2, 4
 
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "cpm.h")
 

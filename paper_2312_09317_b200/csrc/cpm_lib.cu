@@ -76,6 +76,13 @@ struct cpm_ctx {
   uint64_t mcs_run = 0;       // MCS executed by this context (for the attempts counter)
   uint64_t launches = 0, sweep_launches = 0;
 
+  // one CUDA graph = one MCS (every launch parameter but the MCS counter, which the kernels read from device
+  // memory, repeats from MCS to MCS); captured on a stream of the context's own, launched on the caller's
+  bool use_graph = true;
+  cudaStream_t cap_stream = nullptr;
+  cudaGraphExec_t mcs_graph = nullptr;
+  uint64_t graph_launches = 0, graph_sweeps = 0;   // kernels / sweep kernels in one MCS
+
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;
   size_t ev_used = 0;
@@ -232,6 +239,71 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
   cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
+  if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+}
+
+// a1: the work of ONE Monte Carlo step on stream st: R repetitions x 2^d colours of the sweep kernel, the
+// snapshot refresh after each, then the Act decay (which also advances the device MCS counter)
+int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
+  const int ncol = 1 << c->d;
+  const size_t ncell = (size_t)c->max_cells + 1;
+  for (int rep = 0; rep < c->R; ++rep)
+    for (int col = 0; col < ncol; ++col) {
+      SweepParams sp = c->sp;
+      sp.p = (uint32_t)(rep * ncol + col);
+      unsigned long long n_active = 1;
+      for (int a = 0; a < 3; ++a) {
+        sp.col[a] = (a < c->d) ? ((col >> a) & 1) : 0;
+        sp.nact[a] = (a < c->d) ? (c->nsub[a] - sp.col[a] + 1) / 2 : 1;
+        n_active *= (unsigned long long)sp.nact[a];
+      }
+      if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
+      sp.n_active = n_active;
+      sp.grp_base = sp.tl.base[col];
+      const unsigned long long per_cta = c->pooled ? 32ull : (unsigned long long)c->wpc;
+      const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
+      if (grid > 0x7fffffffULL || (c->pooled && n_active > 0x7fffffffULL)) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
+      if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, st));
+      cudaEvent_t e0 = nullptr, e1 = nullptr;
+      if (timed) {
+        while (c->ev_pool.size() < c->ev_used + 2) { cudaEvent_t e; CK(cudaEventCreate(&e)); c->ev_pool.push_back(e); }
+        e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
+        CK(cudaEventRecord(e0, st));
+      }
+      if (c->pooled) c->tfn<<<(unsigned)grid, PK_THREADS, c->cta_smem, st>>>(sp);
+      else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, st>>>(c->tm_lat, sp);
+      if (timed) CK(cudaEventRecord(e1, st));
+      c->launches++; c->sweep_launches++;
+      // deterministic mode: the next phase-step reads the values as of its own start
+      if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, st));
+    }
+  if (c->act_enabled) {
+    const long long n_vec = c->sp.apitch * c->dim[1] * c->dim[2] / 16;
+    act_decay_kernel<<<grid_for(n_vec), 256, 0, st>>>((uint4 *)c->act, n_vec, c->mcs_dev);
+  } else {
+    mcs_increment_kernel<<<1, 1, 0, st>>>(c->mcs_dev);
+  }
+  c->launches++;
+  return CPM_OK;
+}
+
+// capture one MCS into a graph (once per context)
+int build_mcs_graph(cpm_ctx *c) {
+  if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+  const uint64_t l0 = c->launches, s0 = c->sweep_launches;
+  CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+  int rc = enqueue_mcs(c, c->cap_stream, false);
+  cudaGraph_t g = nullptr;
+  cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+  c->graph_launches = c->launches - l0; c->graph_sweeps = c->sweep_launches - s0;
+  c->launches = l0; c->sweep_launches = s0;   // nothing ran yet
+  if (rc != CPM_OK) { if (g) cudaGraphDestroy(g); return rc; }
+  if (e != cudaSuccess) return fail(c, CPM_ERR_CUDA, std::string("stream capture: ") + cudaGetErrorString(e));
+  e = cudaGraphInstantiate(&c->mcs_graph, g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) { c->mcs_graph = nullptr; return fail(c, CPM_ERR_CUDA, std::string("graph instantiate: ") + cudaGetErrorString(e)); }
+  return CPM_OK;
 }
 
 }  // namespace
@@ -310,6 +382,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->S = S; c->sites = (int)sites; c->k = (int)k; c->R = (int)(sites / k);
   c->nNb = (d == 2) ? 8 : 26;
   c->act_enabled = any_act;
+  c->use_graph = !(p->flags & CPM_FLAG_NO_GRAPH);
   c->nsets = (sites <= 512) ? 1 : 4;
   // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
   c->use_tma = !(p->flags & CPM_FLAG_NO_TMA) && (S % 4 == 0);
@@ -588,46 +661,17 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
   if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
   CPM_GUARD_BEGIN
   CK(cudaSetDevice(c->device));
-  const int ncol = 1 << c->d;
-  const size_t ncell = (size_t)c->max_cells + 1;
+  // per-launch events need the plain launch sequence; otherwise one graph launch per MCS
+  const bool graph = c->use_graph && !c->timing;
+  if (graph && !c->mcs_graph) { int rc = build_mcs_graph(c); if (rc != CPM_OK) return rc; }
   for (uint32_t m = 0; m < n_mcs; ++m) {
-    for (int rep = 0; rep < c->R; ++rep)
-      for (int col = 0; col < ncol; ++col) {
-        SweepParams sp = c->sp;
-        sp.p = (uint32_t)(rep * ncol + col);
-        unsigned long long n_active = 1;
-        for (int a = 0; a < 3; ++a) {
-          sp.col[a] = (a < c->d) ? ((col >> a) & 1) : 0;
-          sp.nact[a] = (a < c->d) ? (c->nsub[a] - sp.col[a] + 1) / 2 : 1;
-          n_active *= (unsigned long long)sp.nact[a];
-        }
-        if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
-        sp.n_active = n_active;
-        sp.grp_base = sp.tl.base[col];
-        const unsigned long long per_cta = c->pooled ? 32ull : (unsigned long long)c->wpc;
-        const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
-        if (grid > 0x7fffffffULL || (c->pooled && n_active > 0x7fffffffULL)) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
-        if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, c->stream));
-        cudaEvent_t e0 = nullptr, e1 = nullptr;
-        if (c->timing) {
-          while (c->ev_pool.size() < c->ev_used + 2) { cudaEvent_t e; CK(cudaEventCreate(&e)); c->ev_pool.push_back(e); }
-          e0 = c->ev_pool[c->ev_used++]; e1 = c->ev_pool[c->ev_used++];
-          CK(cudaEventRecord(e0, c->stream));
-        }
-        if (c->pooled) c->tfn<<<(unsigned)grid, PK_THREADS, c->cta_smem, c->stream>>>(sp);
-        else c->fn<<<(unsigned)grid, 32 * c->wpc, c->cta_smem, c->stream>>>(c->tm_lat, sp);
-        if (c->timing) CK(cudaEventRecord(e1, c->stream));
-        c->launches++; c->sweep_launches++;
-        // deterministic mode: the next phase-step reads the values as of its own start
-        if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
-      }
-    if (c->act_enabled) {
-      const long long n_vec = c->sp.apitch * c->dim[1] * c->dim[2] / 16;
-      act_decay_kernel<<<grid_for(n_vec), 256, 0, c->stream>>>((uint4 *)c->act, n_vec, c->mcs_dev);
+    if (graph) {
+      CK(cudaGraphLaunch(c->mcs_graph, c->stream));
+      c->launches += c->graph_launches; c->sweep_launches += c->graph_sweeps;
     } else {
-      mcs_increment_kernel<<<1, 1, 0, c->stream>>>(c->mcs_dev);
+      int rc = enqueue_mcs(c, c->stream, c->timing);
+      if (rc != CPM_OK) return rc;
     }
-    c->launches++;
     c->mcs_host++; c->mcs_run++;
   }
   CK(cudaGetLastError());

@@ -145,3 +145,34 @@ def read_kat(path):
             v = [int(t, 16) for t in line.split()]
             rows.append((v[0:4], v[4:6], v[6:10]))
     return rows
+
+
+def build_toolkit_philox(force=False):
+    """Builds tests/cuda/curand_philox_check.cu (the CUDA toolkit's own Philox4x32-10, pin P8(i)) for sm_100a and
+    returns the loaded library.  nvcc cross-compiles without a GPU; calling it needs one."""
+    import ctypes
+    import os
+    import subprocess
+    here = os.path.dirname(os.path.abspath(__file__))
+    src = os.path.join(here, "cuda", "curand_philox_check.cu")
+    lib = os.path.join(here, "cuda", "libcurand_philox_check.so")
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        tmp = lib + ".%d.tmp" % os.getpid()
+        subprocess.check_call([os.environ.get("NVCC", "nvcc"), "-gencode", "arch=compute_100a,code=sm_100a", "-O2",
+                               "-shared", "-Xcompiler", "-fPIC", "-o", tmp, src])
+        os.replace(tmp, lib)
+    L = ctypes.CDLL(lib)
+    L.toolkit_philox4x32_10.restype = ctypes.c_int
+    L.toolkit_philox4x32_10.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64]
+    return L
+
+
+def toolkit_philox(ctr, key, device=0):
+    """curand_Philox4x32_10 on n (ctr[4], key[2]) pairs -> uint32[n, 4]."""
+    L = build_toolkit_philox()
+    c = np.ascontiguousarray(np.asarray(ctr, dtype=np.uint32)).reshape(-1, 4)
+    k = np.ascontiguousarray(np.asarray(key, dtype=np.uint32)).reshape(-1, 2)
+    out = np.zeros((len(c), 4), np.uint32)
+    rc = L.toolkit_philox4x32_10(device, c.ctypes.data, k.ctypes.data, out.ctypes.data, len(c))
+    assert rc == 0, rc
+    return out

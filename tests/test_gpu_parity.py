@@ -54,19 +54,31 @@ def _run(pk, ob, cfg, n_mcs, every, act=False, **over):
     return g, o
 
 
-def test_philox_device_equals_oracle_and_kat(pk, oracle_mod):
-    """P8: device Philox vs published vectors and vs the oracle's on 10^5 random inputs."""
+def test_philox_device_equals_oracle_toolkit_and_kat(pk, oracle_mod):
+    """P8: the device Philox4x32-10 the sweep uses vs (a) the published known-answer vectors,
+    (i) the CUDA toolkit's own curand_Philox4x32_10 (tests/cuda/curand_philox_check.cu) and (ii) the oracle's,
+    on ALL of 10^6 random (counter, key) pairs -- three independent implementations, every output word."""
+    import ctypes
     import os
     rows = H.read_kat(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt"))
     out = pk.debug_philox([r[0] for r in rows], [r[1] for r in rows])
     np.testing.assert_array_equal(out, np.array([r[2] for r in rows], np.uint32))
+    np.testing.assert_array_equal(H.toolkit_philox([r[0] for r in rows], [r[1] for r in rows]), np.array([r[2] for r in rows], np.uint32))
     rng = np.random.default_rng(1)
-    n = 100000
+    n = 1000000
     ctr = rng.integers(0, 1 << 32, (n, 4), dtype=np.uint64).astype(np.uint32)
     key = rng.integers(0, 1 << 32, (n, 2), dtype=np.uint64).astype(np.uint32)
+    # counters of the shape the sweep uses (small attempt-quad, subsection, 2p + stream, mcs) in the first rows
+    ctr[:1000, 0] = np.arange(1000) % 16; ctr[:1000, 2] = np.arange(1000) % 16; ctr[:1000, 3] = np.arange(1000) // 16
     dev = pk.debug_philox(ctr, key)
-    for i in range(0, n, 97):
-        np.testing.assert_array_equal(dev[i], oracle_mod.philox4x32_10(ctr[i], key[i]))
+    np.testing.assert_array_equal(dev, H.toolkit_philox(ctr, key))
+    ora = np.zeros((n, 4), np.uint32)
+    f = oracle_mod.lib().oracle_philox4x32_10
+    f.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    pc, pk_, po = ctr.ctypes.data, key.ctypes.data, ora.ctypes.data
+    for i in range(n):
+        f(pc + 16 * i, pk_ + 8 * i, po + 16 * i)
+    np.testing.assert_array_equal(dev, ora)
 
 
 @pytest.mark.parametrize("T", [20.0, 10.0, 0.7, 137.5])
@@ -234,6 +246,30 @@ def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     gm.set_lattice(cfg["ids"], None, cfg["cell_type"])
     gm.step(3)
     np.testing.assert_array_equal(gm.get_lattice(), o.get_lattice())
+
+
+@pytest.mark.parametrize("name,dims", [("C1", None), ("C3", (32, 32, 32))])
+def test_graph_and_plain_launches_agree(pk, oracle_mod, name, dims):
+    """cpm_step replays one CUDA graph per MCS; CPM_FLAG_NO_GRAPH launches the same kernels one by one, and so does
+    a context with per-launch timing on.  All three equal the oracle, launch counts included."""
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims)
+    act = name == "C3"
+    g, o = _run(pk, oracle_mod, cfg, 6, 3, act=act)
+    gp, _ = _pair(pk, oracle_mod, cfg, flags=pk.FLAG_NO_GRAPH)
+    gp.step(6)
+    _compare(gp, o, act, "plain launches")
+    gt, _ = _pair(pk, oracle_mod, cfg)
+    gt.step(2)
+    gt.set_kernel_timing(True)
+    gt.step(2)
+    ms, n = gt.get_kernel_timing(reset=True)
+    gt.set_kernel_timing(False)
+    gt.step(2)
+    _compare(gt, o, act, "graph / timed / graph")
+    per_mcs = g.get_schedule()["phase_steps_per_mcs"]
+    assert n == 2 * per_mcs and ms > 0
+    assert g.get_launch_info()["sweep_launches"] == gp.get_launch_info()["sweep_launches"] == gt.get_launch_info()["sweep_launches"] == 6 * per_mcs
 
 
 def test_live_mode_equals_deterministic_while_no_cell_is_shared(pk, oracle_mod):

@@ -261,7 +261,7 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
       sp.n_active = n_active;
       sp.grp_base = sp.tl.base[col];
-      const unsigned long long per_cta = c->pooled ? 32ull : (unsigned long long)c->wpc;
+      const unsigned long long per_cta = c->pooled ? (unsigned long long)PK_GC : (unsigned long long)c->wpc;
       const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
       if (grid > 0x7fffffffULL || (c->pooled && n_active > 0x7fffffffULL)) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
       if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, st));
@@ -415,7 +415,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   // per CTA: warp tiles, 64 B of mbarriers, neighbour-offset tables (256 B), type records, J
   const size_t table_bytes = 64 + 256 + (size_t)(nT + 1) * sizeof(TypeParams) + (size_t)nT * nT * 4;
   c->cta_smem = (size_t)c->wpc * sp.warp_smem_bytes + table_bytes;
-  if (c->pooled) { c->wpc = PK_WARPS; c->cta_smem = pool_smem; }
+  if (c->pooled) { c->wpc = PK_THREADS / 32; c->cta_smem = pool_smem; }
   if (c->cta_smem > smem_cap) { delete c; return CPM_ERR_UNSUPPORTED; }
 
   // ---- host-built tables ----
@@ -466,9 +466,9 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
       na *= (unsigned long long)tl.nact[col][a];
     }
     c->n_act_col[col] = na;
-    c->grp_col[col] = (na + 31ull) / 32ull;
+    c->grp_col[col] = (na + (unsigned long long)(PK_GC - 1)) / (unsigned long long)PK_GC;
     tl.base[col] = c->tile_words;
-    c->tile_words += (size_t)(c->grp_col[col] * (unsigned long long)tl.TW * 32ull);
+    c->tile_words += (size_t)(c->grp_col[col] * (unsigned long long)tl.TW * (unsigned long long)PK_GC);
   }
 
   // ---- device state ----
@@ -591,7 +591,7 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
     const TileLayout &tl = c->sp.tl;
     for (int col = 0; col < (1 << c->d); ++col) {
       if (c->n_act_col[col] == 0) continue;
-      const long long words = (long long)(c->grp_col[col] * (unsigned long long)tl.TW * 32ull);
+      const long long words = (long long)(c->grp_col[col] * (unsigned long long)tl.TW * (unsigned long long)PK_GC);
       if (c->d == 2)
         tile_pack_kernel<2><<<grid_for(words), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
                                                                      c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
@@ -602,7 +602,7 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
     }
     for (int col = 0; col < (1 << c->d); ++col) {
       if (c->n_act_col[col] == 0) continue;
-      const long long thr = (long long)c->grp_col[col] * 32;
+      const long long thr = (long long)c->n_act_col[col];
       if (c->d == 2)
         tile_recount_kernel<2><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz);
       else

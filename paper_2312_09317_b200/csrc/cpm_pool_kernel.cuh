@@ -1,33 +1,37 @@
 // cpm_pool_kernel.cuh -- sm_100a sweep kernel for small power-of-two subsections (3D S = 2, 4; 2D S = 2..16):
-// one CTA of four warps owns a GROUP of 32 active checkerboard subsections ("chains") and evaluates their copy
-// attempts SPECULATIVELY IN PARALLEL, pooled over the 32 chains, while keeping the exact sequential
-// semantics of every chain (the attempts of one subsection are applied in order).
+// one WARP owns a GROUP of 8 active checkerboard subsections ("chains") and evaluates their copy attempts
+// SPECULATIVELY IN PARALLEL, pooled over the 8 chains, while keeping the exact sequential semantics of every
+// chain (the attempts of one subsection are applied in order).  Warps never wait for one
+// another: a CTA is one warp, all synchronisation is __syncwarp().
 //
 // Data layout in HBM: the lattice is stored as per-subsection TILES WITH HALO
-// ((S+2)^d words each, the halo replicated from the neighbouring subsections), 32 same-colour tiles
-// interleaved: word j of chain c of group g at  base[colour] + ((g * TW + j) << 5) + c.  A group is one
-// contiguous block of TW * 128 bytes, so
-//   a2  ONE bulk asynchronous copy (TMA, cp.async.bulk -> SASS UBLKCP) stages the tiles of all 32 chains,
-//       already in the bank-conflict-free order the kernel wants (bank = chain); completion on an mbarrier
-//       while the CTA draws its first random numbers;
+// ((S+2)^d words each, the halo replicated from the neighbouring subsections), 8 same-colour tiles
+// interleaved: word j of chain c of group g at  base[colour] + ((g * TW + j) << 3) + c.  A group is one
+// contiguous block of TW * 32 bytes, so
+//   a2  ONE bulk asynchronous copy (TMA, cp.async.bulk -> SASS UBLKCP) stages the tiles of the 8 chains, already
+//       in the order the kernel wants (bank = chain + 8 (j mod 4)); completion on an mbarrier while the warp
+//       draws its random numbers;
 //   a10 there is no tile write-back: an accepted copy stores its word to the home tile and to the (at most
 //       2^d - 1) halo replicas in the neighbouring subsections' tiles, which are inactive in this phase-step.
-// Per chunk of 16 attempts per chain (512 attempts per CTA), thread (warp w, lane c) owns attempts 4w..4w+3 of
-// chain c:
-//   a3  one Philox4x32-10 block per thread (counter (a>>2, b, 2p, mcs), reading S15) -> 4 proposals;
-//   a4  the owner thread screens them against its chain's tile (same cell / frozen); ballot + popc + one
-//       shared-memory atomic per warp compact the surviving attempts of all chains into one queue;
-//   a5-a7 the queue is evaluated one item per thread whatever chain it belongs to: neighbour census from the
+// Lane (q, c) = (lane >> 3, lane & 7) serves chain c:
+//   a3  all proposals of (up to) 64 attempts per chain are drawn up front: one Philox4x32-10 block (counter
+//       (a>>2, b, 2p, mcs), reading S15) = 4 attempts, quads q, q+4, ... per lane; decoded proposals go to shared
+//       memory;
+//   a4  every chain has its own position (attempts before it are final).  Per round the lanes of a chain screen
+//       the next 4 NJ attempts behind its position against its tile (same cell / frozen); ballot + popc compact
+//       the surviving attempts of all 8 chains into one queue, ordered by distance from the chain's position; at
+//       most 32 are taken per round (a chain's window ends at its first attempt left out);
+//   a5-a7 the queue is evaluated one item per lane whatever chain it belongs to: neighbour census from the
 //       chain's tile column, per-cell state (snapshot + the chain's own deltas / live), dH in int64;
-//   Act the geometric means (Eq 9) the items need are requested through a second queue and computed one per
-//       thread (a request is dropped when the centre's own Act value is 0: any zero makes the mean 0);
+//   Act the geometric means (Eq 9) the items need are computed by the whole warp, one request after the other
+//       (lanes = the sites of the neighbourhood);
 //   a8  Metropolis; an accepted item enters a shared-memory atomicMin on its chain's slot, keyed by the attempt
 //       index, so the FIRST accepted attempt of every chain wins;
 //   a9  nothing is committed before every item of the round is decided: all of them saw the state at the start
-//       of the round, what lies before a chain's winner is final, the winner is committed, and the attempts
-//       after it are screened and evaluated again in the next round on the new state.  Rounds per chunk =
-//       1 + the largest number of accepted copies any chain has in the chunk, so the result equals k
-//       sequential attempts per subsection exactly;
+//       of the round, what lies before a chain's winner is final, the winner is committed (8 lanes per winner:
+//       home word and halo replicas, the reductions of both cells), the chain continues behind its winner on the
+//       new state and the others behind their window, so the result equals k sequential attempts per subsection
+//       exactly;
 //   a10 the integer deltas of a committed copy go to the live per-cell arrays at once as 64-bit reductions.
 // Nothing here is shared with oracle/.
 #pragma once
@@ -35,13 +39,15 @@
 
 namespace cpm {
 
-constexpr int PK_WARPS = 4;                  // warps per CTA = per group of 32 chains
-constexpr int PK_THREADS = 32 * PK_WARPS;
-constexpr int PK_CHUNK = 16;                 // attempts per chain between two pooled evaluations (4 per thread)
+constexpr int PK_GS = 3;                     // log2 of the chains per group
+constexpr int PK_GC = 1 << PK_GS;            // chains per warp = per group
+constexpr int PK_THREADS = 32;               // one warp per CTA
+constexpr int PK_SUPER = 64;                 // attempts per chain whose proposals are drawn up front
+constexpr int PK_NJ = 5;                     // a chain's window per round: 4 NJ attempts behind its position
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 3;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
-constexpr int PK_NOWIN = PK_CHUNK << 10;     // "no accepted attempt": a chain's winner slot holds a << 10 | n_A << 5 | n_B
+constexpr int PK_NOWIN = PK_SUPER << 10;     // "no accepted attempt": a chain's winner slot holds a << 10 | n_A << 5 | n_B
 // lattice word of the tiled layout: [type:5 | frozen:1 | 00 | id:24]: the top byte is the byte offset type * 8 +
 // frozen * 4 into a row of the adhesion table, so a neighbour's adhesion term costs one multiply-high, one load
 // and one add
@@ -66,32 +72,23 @@ struct PGeom {
   static __host__ __device__ constexpr int dy(int n) { return (idx27(n) / 3) % 3 - 1; }
   static __host__ __device__ constexpr int dz(int n) { return DIM == 3 ? idx27(n) / 9 - 1 : 0; }
   static __host__ __device__ constexpr int noff(int n) { return (dz(n) * T + dy(n)) * T + dx(n); }   // in tile words
-  // neighbours with offset d (-1 / +1) along axis ax, as a bit mask over n
-  static __host__ __device__ constexpr uint32_t face(int ax, int d) {
-    uint32_t m = 0;
-    for (int n = 0; n < NNB; ++n) if ((ax == 0 ? dx(n) : ax == 1 ? dy(n) : dz(n)) == d) m |= 1u << n;
-    return m;
-  }
 };
 
-// shared-memory carve-up of one CTA; D (nT^3 + nT words) comes last
+// shared-memory carve-up of one warp; D (2 nT^3 + nT words) comes last
 template <int DIM, int S>
 struct PSmem {
   using G = PGeom<DIM, S>;
-  static constexpr int TILE = 0;                                   // uint32 [TW][32]
-  static constexpr int PROP = TILE + G::TW * 128;                  // uint16 [16][32]   toff | nb << 9
-  static constexpr int QUEUE = PROP + PK_CHUNK * 64;               // uint8 [4 segments][128]  chain | (a & 3) << 5 (segment w holds attempts 4w..4w+3)
-  static constexpr int DKEY = QUEUE + PK_WARPS * PK_THREADS;               // uint32 [DCAP][32]
-  static constexpr int DDVP = DKEY + PK_DCAP * 128;                // uint64 [DCAP][32]
-  static constexpr int DN = DDVP + PK_DCAP * 256;                  // int [32] own-delta table of the chain: entries | (spill slot + 1) << 8
-  static constexpr int FIRST = DN + 128;                           // int [32] first accepted attempt of the round
-  static constexpr int POS = FIRST + 128;                          // int [32] attempts < pos of the chunk are final
-  static constexpr int ORIG = POS + 128;                           // int [3][32] lattice origin of the chain
-  static constexpr int NOFF = ORIG + 384;                          // int [32] neighbour -> tile offset (entry NNB = centre = 0)
-  static constexpr int CNT = NOFF + 128;                           // int [8]: [2] redo flag, [3] chains that continue, [4..7] queue segment lengths
-  static constexpr int RLIST = CNT + 32;                           // uint8 [32] the chains that continue in the next round
-  static constexpr int MBAR = RLIST + 32;                            // uint64
-  static constexpr int TYPES = MBAR + 16;                          // TypeParams [nT + 1], then int32 [nT][nT][nT][2] adhesion
+  static constexpr int TILE = 0;                                   // uint32 [TW][8]
+  static constexpr int DDVP = TILE + G::TW * 4 * PK_GC;            // uint64 [DCAP][8]
+  static constexpr int MBAR = DDVP + PK_DCAP * 8 * PK_GC;          // uint64
+  static constexpr int DKEY = MBAR + 8;                            // uint32 [DCAP][8]
+  static constexpr int PROP = DKEY + PK_DCAP * 4 * PK_GC;          // uint16 [64][8]   toff | nb << 9
+  static constexpr int QUEUE = PROP + PK_SUPER * 2 * PK_GC;        // uint16 [32 NJ]   chain | a << 3
+  static constexpr int DN = QUEUE + 32 * PK_NJ * 2;                // int [8] own-delta table of the chain: entries | (spill slot + 1) << 8
+  static constexpr int FIRST = DN + 4 * PK_GC;                     // int [8] first accepted attempt of the round
+  static constexpr int ORIG = FIRST + 4 * PK_GC;                   // int [3][8] lattice origin of the chain
+  static constexpr int NOFF = ORIG + 12 * PK_GC;                   // int [32] neighbour -> tile offset (entry NNB = centre = 0)
+  static constexpr int TYPES = (NOFF + 128 + 15) / 16 * 16;        // TypeParams [nT + 1], then int32 [nT][nT][nT][2] adhesion
                                                                    // differences, then [nT] J(t,t)
   static constexpr size_t bytes(int nT) { return (size_t)TYPES + (size_t)(nT + 1) * 32 + ((size_t)2 * nT * nT * nT + nT) * 4; }
 };
@@ -111,7 +108,7 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
 __device__ __forceinline__ unsigned long long tile_word(const TileLayout &L, int bx, int by, int bz, int j) {
   const int col = (bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2);
   const unsigned long long w = (unsigned long long)(bx >> 1) + (unsigned long long)L.nact[col][0] * ((unsigned long long)(by >> 1) + (unsigned long long)L.nact[col][1] * (unsigned long long)(bz >> 1));
-  return L.base[col] + ((((w >> 5) * (unsigned long long)L.TW + (unsigned long long)j) << 5) | (w & 31ull));
+  return L.base[col] + ((((w >> PK_GS) * (unsigned long long)L.TW + (unsigned long long)j) << PK_GS) | (w & (unsigned long long)(PK_GC - 1)));
 }
 // home word of lattice site (x,y,z), all inside the lattice; S = L.S
 template <int DIM>
@@ -123,80 +120,72 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
 }
 
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
-  constexpr int T = G::T, TW = G::TW, NNB = G::NNB;
+  constexpr int T = G::T, TW = G::TW, NNB = G::NNB, GC = PK_GC, NJ = PK_NJ;
   extern __shared__ __align__(128) unsigned char smem[];
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
   unsigned short *prop = reinterpret_cast<unsigned short *>(smem + M::PROP);
-  unsigned char *queue = smem + M::QUEUE;
+  unsigned short *queue = reinterpret_cast<unsigned short *>(smem + M::QUEUE);
   uint32_t *dkey = reinterpret_cast<uint32_t *>(smem + M::DKEY);
   unsigned long long *ddvp = reinterpret_cast<unsigned long long *>(smem + M::DDVP);
   int *dn = reinterpret_cast<int *>(smem + M::DN);
   int *first = reinterpret_cast<int *>(smem + M::FIRST);
-  int *spos = reinterpret_cast<int *>(smem + M::POS);
   int *orig = reinterpret_cast<int *>(smem + M::ORIG);
   int *snoff = reinterpret_cast<int *>(smem + M::NOFF);
-  int *cnt = reinterpret_cast<int *>(smem + M::CNT);
-  unsigned char *rlist = smem + M::RLIST;
   uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + M::MBAR);
   TypeParams *st = reinterpret_cast<TypeParams *>(smem + M::TYPES);
   int32_t *sd = reinterpret_cast<int32_t *>(smem + M::TYPES + (P.nT + 1) * 32);
   const int32_t *sdiag = sd + 2 * P.nT * P.nT * P.nT;
 
-  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  const int lane = threadIdx.x;
+  const int c = lane & (GC - 1), q = lane >> PK_GS;   // this lane serves chain c; q = its slot among the chain's 4 lanes
   const unsigned lt = (1u << lane) - 1u;
-  const unsigned long long grp_word = P.grp_base + (unsigned long long)blockIdx.x * (unsigned long long)(TW * 32);
-  uint32_t *const gtile = P.tl.tiles + grp_word;   // this group's tiles in HBM
+  uint32_t *const gtile = P.tl.tiles + P.grp_base + (unsigned long long)blockIdx.x * (unsigned long long)(TW * GC);   // this group's tiles in HBM
 
-  // ---- a2: one bulk copy stages the 32 tiles; it overlaps the set-up and the first Philox blocks ----
-  if (tid == 0) {
+  // ---- a2: one bulk copy stages the 8 tiles; it overlaps the set-up and the Philox blocks ----
+  if (lane == 0) {
     mbar_init(mbar, 1); fence_mbar_init();
-    mbar_expect_tx(mbar, (uint32_t)(TW * 128));
-    bulk_load(tile, gtile, (uint32_t)(TW * 128), mbar);
-    cnt[0] = 0; cnt[1] = 0; cnt[2] = 0;
+    mbar_expect_tx(mbar, (uint32_t)(TW * 4 * GC));
+    bulk_load(tile, gtile, (uint32_t)(TW * 4 * GC), mbar);
   }
   // small tables
-  if (tid < 32) {
+  {
     int dx = 0, dy = 0, dz = 0;
-    if (tid < NNB) nb_delta<DIM>(tid, dx, dy, dz);
-    snoff[tid] = (dz * T + dy) * T + dx;
-    dn[tid] = 0; first[tid] = PK_NOWIN;
+    if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
+    snoff[lane] = (dz * T + dy) * T + dx;
   }
-  for (int i = tid; i < (P.nT + 1) * 8; i += PK_THREADS) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-  for (int i = tid; i < 2 * P.nT * P.nT * P.nT + P.nT; i += PK_THREADS) sd[i] = P.D[i];
-
-  // the chain this thread screens: c = lane (warp w owns attempts 4w..4w+3 of every chunk); its geometry is
-  // worked out once, by warp 0 (the host limits n_active to 31 bits for this kernel)
-  const uint32_t w = blockIdx.x * 32u + (uint32_t)lane;
-  const bool active = w < (uint32_t)P.n_active;
-  if (wrp == 0) {
-    int ox = 0, oy = 0, oz = 0;
-    if (active) {
+  for (int i = lane; i < (P.nT + 1) * 8; i += 32) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+  for (int i = lane; i < 2 * P.nT * P.nT * P.nT + P.nT; i += 32) sd[i] = P.D[i];
+  // geometry of the chains (the host limits n_active to 31 bits for this kernel)
+  if (lane < GC) {
+    const uint32_t w = blockIdx.x * (uint32_t)GC + (uint32_t)lane;
+    int ox = -1, oy = 0, oz = 0;    // ox < 0: no such chain (ragged last group)
+    if (w < (uint32_t)P.n_active) {
       const uint32_t ax = w % (uint32_t)P.nact[0], r1 = w / (uint32_t)P.nact[0];
       const uint32_t ay = r1 % (uint32_t)P.nact[1], az = r1 / (uint32_t)P.nact[1];
-      const int bx = 2 * (int)ax + P.col[0], by = 2 * (int)ay + P.col[1], bz = (DIM == 3) ? 2 * (int)az + P.col[2] : 0;
-      ox = bx * S; oy = by * S; oz = (DIM == 3) ? bz * S : 0;
+      ox = (2 * (int)ax + P.col[0]) * S; oy = (2 * (int)ay + P.col[1]) * S; oz = (DIM == 3) ? (2 * (int)az + P.col[2]) * S : 0;
     }
-    orig[lane] = ox; orig[32 + lane] = oy; orig[64 + lane] = oz;
+    orig[lane] = ox; orig[GC + lane] = oy; orig[2 * GC + lane] = oz;
+    dn[lane] = 0; first[lane] = PK_NOWIN;
   }
-  __syncthreads();
-  const uint32_t b = active ? (uint32_t)(orig[lane] / S + P.nsub[0] * (orig[32 + lane] / S + P.nsub[1] * (orig[64 + lane] / S))) : 0u;
+  __syncwarp();
+  const bool active = orig[c] >= 0;
+  const uint32_t b = active ? (uint32_t)(orig[c] / S + P.nsub[0] * (orig[GC + c] / S + P.nsub[1] * (orig[2 * GC + c] / S))) : 0u;
   const uint32_t mcs = *P.mcs_ptr;
   const int k = P.k;
-  const int nchunk = (k + PK_CHUNK - 1) / PK_CHUNK;
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;
   bool staged = false;
-  const uint32_t *const tcol = tile + lane;   // this thread's own chain column
+  const uint32_t *const tcol = tile + c;   // this lane's own chain column
 
-  for (int ch = 0; ch < nchunk; ++ch) {
-    // ---- a3: the 4 proposals this thread owns; kept in registers for screening and in shared memory for
-    //      whichever thread evaluates them ----
-    int pr[4];
-    {
-      const uint4 r = philox4x32_10(make_uint4((uint32_t)(ch * (PK_CHUNK / 4) + wrp), b, 2u * P.p, mcs), P.key0, P.key1);
+  for (int sc = 0; sc < k; sc += PK_SUPER) {
+    const int kk = min(PK_SUPER, k - sc);   // attempts of this stretch
+    // ---- a3: the proposals of the stretch, quads q, q + 4, ... of chain c ----
+#pragma unroll 1
+    for (int qq = q; 4 * qq < kk; qq += 4) {
+      const uint4 r = philox4x32_10(make_uint4((uint32_t)((sc >> 2) + qq), b, 2u * P.p, mcs), P.key0, P.key1);
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const uint32_t wd = pick(r, j);
@@ -204,89 +193,66 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
         const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
         const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
         const int toff = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-        pr[j] = toff | (nb << 9);
+        prop[(4 * qq + j) * GC + c] = (unsigned short)(toff | (nb << 9));
       }
     }
-    const int kk = min(PK_CHUNK, k - ch * PK_CHUNK);   // valid attempts of this chunk
-    __syncthreads();                                   // the previous chunk is finished (prop, pos are free)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) prop[(4 * wrp + j) * 32 + lane] = (unsigned short)pr[j];
-    if (wrp == 0) spos[lane] = active ? 0 : PK_CHUNK;
+    int pos = active ? 0 : kk;   // attempts < pos of this stretch are final (same value in the 4 lanes of a chain)
     if (!staged) {   // first use of the tiles
       while (!mbar_try_wait(mbar, 0)) {}
       staged = true;
     }
-    __syncthreads();
+    __syncwarp();
 
-    bool first_round = true;
     while (true) {
-      if (wrp == 0) first[lane] = PK_NOWIN;   // nobody touches the winner slots before the next barrier
-      if (first_round || cnt[3] > 8) {
-        // ---- a4: screen the not yet final attempts this thread owns; every warp compacts the survivors of its four
-        //      attempt indices into its own queue segment (segment w holds attempts 4w..4w+3 of all chains) ----
-        const int ps = spos[lane];
-        bool in[4];
-        unsigned m[4];
+      // ---- a4: screen the window of this lane's chain: relative attempts q, q + 4, ... behind its position;
+      //      the queue is ordered by (relative attempt, chain) ----
+      bool in[NJ];
+      unsigned m[NJ];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int a = 4 * wrp + j;
-          const int toff = pr[j] & 511;
-          const uint32_t wt = tcol[toff * 32], ws = tcol[(toff + snoff[pr[j] >> 9]) * 32];
-          in[j] = a >= ps && a < kk && (((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u);
-          m[j] = __ballot_sync(FULL, in[j]);
+      for (int j = 0; j < NJ; ++j) {
+        const int a = pos + q + 4 * j;
+        const bool ok = a < kk;
+        uint32_t wt = 0u, ws = 0u;
+        if (ok) {
+          const int prc = (int)prop[a * GC + c];
+          const int toff = prc & 511;
+          wt = tcol[toff * GC]; ws = tcol[(toff + snoff[prc >> 9]) * GC];
         }
-        int base = wrp * PK_THREADS;
+        in[j] = ok && (((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u);
+        m[j] = __ballot_sync(FULL, in[j]);
+      }
+      int W = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          if (in[j]) queue[base + __popc(m[j] & lt)] = (unsigned char)(lane | (j << 5));
+      for (int j = 0; j < NJ; ++j) {
+        if (in[j]) queue[W + __popc(m[j] & lt)] = (unsigned short)(c | ((pos + q + 4 * j) << PK_GS));
+        W += __popc(m[j]);
+      }
+      int lim = 4 * NJ;   // the window of this lane's chain covered by this round
+      if (W > 32) {       // warp-uniform, rare: a round takes the first 32 items; a chain's window ends at its first item left out
+        int fu = 4 * NJ, base = 0;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+          if (in[j] && base + __popc(m[j] & lt) >= 32) fu = min(fu, q + 4 * j);
           base += __popc(m[j]);
         }
-        if (lane == 0) cnt[4 + wrp] = base - wrp * PK_THREADS;
-      } else {
-        // ---- a4 for the few (<= 8) chains that continue behind an accepted copy: thread (r, a) screens attempt a
-        //      of the r-th such chain; the segment counters were cleared at the end of the last round ----
-        const int r = tid >> 4, a = tid & 15;
-        if (r < cnt[3]) {
-          const int c = (int)rlist[r];
-          if (a >= spos[c] && a < kk) {
-            const int prc = (int)prop[a * 32 + c];
-            const int toff = prc & 511;
-            const uint32_t wt = tile[toff * 32 + c], ws = tile[(toff + snoff[prc >> 9]) * 32 + c];
-            if ((((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u)) {
-              const int sg = a >> 2;
-              queue[sg * PK_THREADS + atomicAdd(cnt + 4 + sg, 1)] = (unsigned char)(c | ((a & 3) << 5));
-            }
-          }
-        }
+        fu = min(fu, __shfl_xor_sync(FULL, fu, 8));
+        fu = min(fu, __shfl_xor_sync(FULL, fu, 16));
+        lim = fu; W = 32;
       }
-      first_round = false;
-      __syncthreads();
-      // a round takes the leading segments that fit one item per thread (nearly always all four); the attempts
-      // of the others are screened again in the next round
-      int e0 = cnt[4], e1 = e0 + cnt[5], e2 = e1 + cnt[6], e3 = e2 + cnt[7];
-      int nseg = 4;
-      if (e3 > PK_THREADS) { nseg = (e2 <= PK_THREADS) ? 3 : (e1 <= PK_THREADS) ? 2 : 1; }
-      const int W = nseg == 4 ? e3 : nseg == 3 ? e2 : nseg == 2 ? e1 : e0;
-      const int a_lim = 4 * nseg;            // attempts < a_lim are covered by this round
-      if (W == 0 && nseg == 4) break;        // CTA-uniform: nothing left in this chunk
+      __syncwarp();
 
-      // ---- a5-a7: one item per thread; warps without items go straight to the barrier ----
-      const bool have = tid < W;
-      int c = 0, a = 0;
-      if (32 * wrp < W) {   // warp-uniform
-      int item = 0;
-      if (have) {
-        const int sg = (tid >= e0 ? 1 : 0) + (tid >= e1 ? 1 : 0) + (tid >= e2 ? 1 : 0);
-        const int off = tid - (sg == 0 ? 0 : sg == 1 ? e0 : sg == 2 ? e1 : e2);
-        item = (int)queue[sg * PK_THREADS + off] | (sg << 7);   // chain | a << 5
-      }
-      c = item & 31; a = item >> 5;
-      const int prc = (int)prop[a * 32 + c];
+      // ---- a5-a7: one item per lane ----
+      const bool have = lane < W;
+      int ci = 0, a = 0;
+      if (W > 0) {   // warp-uniform
+      const int item = have ? (int)queue[lane] : 0;
+      ci = item & (GC - 1); a = item >> PK_GS;
+      const int prc = (int)prop[a * GC + ci];
       const int toff = prc & 511, nb = prc >> 9;
       int nA = 0, nB = 0;
       const int soff = toff + snoff[nb];
-      const uint32_t *const tc = tile + c;
-      const uint32_t wA = tc[soff * 32], wB = tc[toff * 32];
+      const uint32_t *const tc = tile + ci;
+      const uint32_t wA = tc[soff * GC], wB = tc[toff * GC];
       const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
       const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
       const int tA = (int)(wA >> PK_TYPE_SHIFT), tB = (int)(wB >> PK_TYPE_SHIFT);
@@ -302,7 +268,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
         int adh = 0;
 #pragma unroll
         for (int n = 0; n < NNB; ++n) {
-          const uint32_t raw = tc[(toff + G::noff(n)) * 32];
+          const uint32_t raw = tc[(toff + G::noff(n)) * GC];
           count_same(nA, raw, wA);
           count_same(nB, raw, wB);
           adh += *reinterpret_cast<const int32_t *>(Drow + (raw >> 24));
@@ -313,14 +279,14 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
         // a6: per-cell {V,P} as this attempt sees it: snapshot + the chain's own deltas / live
         unsigned long long vpA = baseA, vpB = baseB;
         if constexpr (!LIVE) {
-          const int di = dn[c];
+          const int di = dn[ci];
           const int ne = di & 255;
           if (ne > 0) {
             unsigned long long dA = 0ull, dB = 0ull;
             const int ns = min(ne, PK_DCAP);
             for (int i = 0; i < ns; ++i) {
-              const uint32_t key = dkey[i * 32 + c];
-              const unsigned long long v = ddvp[i * 32 + c];
+              const uint32_t key = dkey[i * GC + ci];
+              const unsigned long long v = ddvp[i * GC + ci];
               if (key == A) dA = v;
               if (key == Bc) dB = v;
             }
@@ -358,7 +324,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
       if constexpr (ACT) {
         // any zero makes the mean zero, and the centre belongs to its own neighbourhood: look at it first
         if (wantA | wantB) {
-          const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
+          const int ox = orig[ci], oy = orig[GC + ci], oz = orig[2 * GC + ci];
           if (wantA) {
             const int sz3 = (DIM == 3) ? soff / (T * T) : 0, sy3 = (soff / T) % T, sx3 = soff % T;
             int gx = ox - 1 + sx3, gy = oy - 1 + sy3, gz = (DIM == 3) ? oz - 1 + sz3 : 0;
@@ -384,11 +350,11 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
             const int src = __ffs(sideB ? mwB : mwA) - 1;
             if (sideB) mwB &= mwB - 1; else mwA &= mwA - 1;
             const int ctr = __shfl_sync(FULL, sideB ? toff : soff, src);
-            const int cc = __shfl_sync(FULL, c, src);
+            const int cc = __shfl_sync(FULL, ci, src);
             const uint32_t mC = __shfl_sync(FULL, sideB ? mB : mA, src);
             const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
             // the centre is inside the lattice (its cell is not medium), possibly through the wrap
-            int cx = orig[cc] - 1 + px, cy = orig[32 + cc] - 1 + py, cz = (DIM == 3) ? orig[64 + cc] - 1 + pz : 0;
+            int cx = orig[cc] - 1 + px, cy = orig[GC + cc] - 1 + py, cz = (DIM == 3) ? orig[2 * GC + cc] - 1 + pz : 0;
             cx += (cx < 0) ? P.X : (cx >= P.X) ? -P.X : 0;
             cy += (cy < 0) ? P.Y : (cy >= P.Y) ? -P.Y : 0;
             if (DIM == 3) cz += (cz < 0) ? P.Z : (cz >= P.Z) ? -P.Z : 0;
@@ -404,11 +370,11 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
               const int qx = px + ddx, qy = py + ddy, qz = pz + ddz;
               const bool intile = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
               // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
-              const uint32_t wq = intile ? tile[(ctr + mynoff) * 32 + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
+              const uint32_t wq = intile ? tile[(ctr + mynoff) * GC + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
               same = (wq & CELL_MASK31) == mC;
             }
             int av = 1;
-            // L2: sees the Act bytes stored by earlier commits of this CTA
+            // L2: sees the Act bytes stored by earlier commits of this warp
             if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
             const unsigned msame = __ballot_sync(FULL, same);
             const unsigned mzero = __ballot_sync(FULL, same && av == 0);
@@ -432,107 +398,125 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
       const bool draw = uphill && acc;
       if (__any_sync(FULL, draw)) {
         if (draw) {
-          const int ag = ch * PK_CHUNK + a;
-          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)(orig[c] / S + P.nsub[0] * (orig[32 + c] / S + P.nsub[1] * (orig[64 + c] / S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
+          const int ag = sc + a;
+          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)(orig[ci] / S + P.nsub[0] * (orig[GC + ci] / S + P.nsub[1] * (orig[2 * GC + ci] / S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
           if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
         }
       }
       // ---- a9: the first accepted attempt of every chain wins ----
-      if (acc) atomicMin(first + c, (a << 10) | (nA << 5) | nB);
+      if (acc) atomicMin(first + ci, (a << 10) | (nA << 5) | nB);
+      __syncwarp();
+      if (have && a <= (first[ci] >> 10)) ++n_eval;   // what lies before a chain's winner (and the winner) is final
       }
-      __syncthreads();
-      if (have && a <= (first[c] >> 10)) ++n_eval;   // what lies before a chain's winner (and the winner) is final
-      if (wrp == 0 && first[lane] < PK_NOWIN) {
-        // ---- a9/a10: warp 0, lane = chain, commits the winners (n_A, n_B come with the winner slot; the tile still
-        //      holds the state of the round's start) ----
-        const int fw = first[lane];
-        const int c = lane, nA = (fw >> 5) & 31, nB = fw & 31;
-        const int prc = (int)prop[(fw >> 10) * 32 + c];
+
+      // ---- a9/a10: the winners are committed, 8 lanes per winner, 4 winners at a time.  Lane r of a winner's
+      //      8: r = 0 the home word (shared memory, HBM) and the Act byte, r = 1 .. 2^d - 1 the halo replica towards
+      //      the face / edge / corner r (bit 0: x, 1: y, 2: z); r = 0..3 the reductions of the source's cell (V and
+      //      P, sum x, sum y, sum z), r = 4..7 those of the target's cell ----
+      const int fwc = first[c];   // winner slot of this lane's own chain (for its position)
+      unsigned rem = __ballot_sync(FULL, lane < GC && first[lane] < PK_NOWIN);
+      while (rem) {   // warp-uniform
+        unsigned mm = rem;
+        for (int i = 0; i < q; ++i) mm &= mm - 1;
+        const bool on = mm != 0u;
+        const int cw = on ? __ffs(mm) - 1 : 0;
+        const int r = c;
+        const int fw = first[cw];
+        const int nA = (fw >> 5) & 31, nB = fw & 31;
+        const int prc = (int)prop[(on ? (fw >> 10) : 0) * GC + cw];
         const int toff = prc & 511;
-        const uint32_t wA = tcol[(toff + snoff[prc >> 9]) * 32], wB = tcol[toff * 32];
+        const uint32_t wA = tile[(toff + snoff[prc >> 9]) * GC + cw], wB = tile[toff * GC + cw];
         const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
-        const int maxA_new = (A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0;
-        ++n_acc;
-        tile[toff * 32 + c] = wA;            // id and type of the source; neither site is frozen
-        gtile[toff * 32 + c] = wA;           // home word in HBM
-        const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
-        const int ox = orig[c], oy = orig[32 + c], oz = orig[64 + c];
-        const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
-        // halo replicas of this site in the tiles of the adjacent (inactive) subsections
-        const int bx = ox / S, by = oy / S, bz = oz / S;
-        const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
-        const int fz = (DIM == 3) ? ((pz == 1) ? -1 : (pz == S) ? 1 : 0) : 0;
-        const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
-#pragma unroll 1
-        for (int msk = 1; msk < (1 << DIM); ++msk) {
-          if (msk & ~avail) continue;
-          const int dx = (msk & 1) ? fx : 0, dy = (msk & 2) ? fy : 0, dz = (msk & 4) ? fz : 0;
-          int nx = bx + dx, ny = by + dy, nz = bz + dz;
-          bool ok = true;
-          if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
-          if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }
-          if (DIM == 3) { if (nz < 0) { nz += P.nsub[2]; ok = ok && P.per[2] != 0; } else if (nz >= P.nsub[2]) { nz -= P.nsub[2]; ok = ok && P.per[2] != 0; } }
-          if (!ok) continue;
-          const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
-          P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
-        }
-        if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-          P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)maxA_new;
-        // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
-        //      and, in deterministic mode, the chain's own-delta table
-#pragma unroll 1
-        for (int side = 0; side < 2; ++side) {
-          const uint32_t cell = side ? Bc : A;
-          if (cell == 0) continue;
-          const int sgn = side ? -1 : 1;
-          const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
-          const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
-          atomicAdd(P.liveVP + cell, d);
-          atomicAdd(P.sumx + cell, (unsigned long long)(long long)(sgn * gx));
-          atomicAdd(P.sumy + cell, (unsigned long long)(long long)(sgn * gy));
-          if (DIM == 3) atomicAdd(P.sumz + cell, (unsigned long long)(long long)(sgn * gz));
-          if constexpr (!LIVE) {
-            const int di = dn[c];
-            const int ne = di & 255;
-            int slot = (di >> 8) - 1;
-            bool hit = false;
-            const int ns = min(ne, PK_DCAP);
-            for (int i = 0; i < ns; ++i)
-              if (dkey[i * 32 + c] == cell) { ddvp[i * 32 + c] += d; hit = true; }
-            if (!hit && ne > PK_DCAP) {
-              const long long sl = (long long)slot * PK_SPILL;
-              for (int i = 0; i < ne - PK_DCAP; ++i)
-                if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
+        __syncwarp();   // every lane has read the state of the round's start
+        if (on) {
+          const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
+          const int ox = orig[cw], oy = orig[GC + cw], oz = orig[2 * GC + cw];
+          const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
+          if (r == 0) {
+            tile[toff * GC + cw] = wA;                                  // id and type of the source; neither site is frozen
+            gtile[toff * GC + cw] = wA;                                 // home word in HBM
+            if constexpr (ACT)   // Max_act of the new owner; 0 for medium
+              P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0);
+            ++n_acc;
+          } else if (r < (1 << DIM)) {
+            // halo replica of this site in the tile of the adjacent (inactive) subsection towards r
+            const int fx = (px == 1) ? -1 : (px == S) ? 1 : 0, fy = (py == 1) ? -1 : (py == S) ? 1 : 0;
+            const int fz = (DIM == 3) ? ((pz == 1) ? -1 : (pz == S) ? 1 : 0) : 0;
+            const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
+            if ((r & ~avail) == 0) {
+              const int dx = (r & 1) ? fx : 0, dy = (r & 2) ? fy : 0, dz = (r & 4) ? fz : 0;
+              int nx = ox / S + dx, ny = oy / S + dy, nz = oz / S + dz;
+              bool ok = true;
+              if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
+              if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }
+              if (DIM == 3) { if (nz < 0) { nz += P.nsub[2]; ok = ok && P.per[2] != 0; } else if (nz >= P.nsub[2]) { nz -= P.nsub[2]; ok = ok && P.per[2] != 0; } }
+              if (ok) {
+                const int jj = (((DIM == 3) ? (pz - dz * S) * T : 0) + (py - dy * S)) * T + (px - dx * S);
+                P.tl.tiles[tile_word(P.tl, nx, ny, nz, jj)] = wA;
+              }
             }
-            if (!hit) {
-              if (ne < PK_DCAP) { dkey[ne * 32 + c] = cell; ddvp[ne * 32 + c] = d; dn[c] = di + 1; }
-              else if (ne < PK_CAP) {
-                if (slot < 0) {
-                  slot = atomicAdd(P.ovf_count, 1);
-                  if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
-                }
-                if (slot >= 0) {
+          }
+          // a10: integer deltas -> live per-cell arrays (64-bit reductions on the composite {V,P} word, L297)
+          {
+            const int side = r >> 2, which = r & 3;
+            const uint32_t cell = side ? Bc : A;
+            if (cell != 0 && (which < 3 || DIM == 3)) {
+              const int sgn = side ? -1 : 1;
+              const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
+              unsigned long long *const arr = which == 0 ? P.liveVP : which == 1 ? P.sumx : which == 2 ? P.sumy : P.sumz;
+              const unsigned long long v = which == 0 ? ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP
+                                                      : (unsigned long long)(long long)(sgn * (which == 1 ? gx : which == 2 ? gy : gz));
+              atomicAdd(arr + cell, v);
+            }
+          }
+          // deterministic mode: the chain's own-delta table (lane 0 of the winner's 8, both sides)
+          if constexpr (!LIVE) {
+            if (r == 0) {
+#pragma unroll 1
+              for (int side = 0; side < 2; ++side) {
+                const uint32_t cell = side ? Bc : A;
+                if (cell == 0) continue;
+                const int sgn = side ? -1 : 1;
+                const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
+                const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
+                const int di = dn[cw];
+                const int ne = di & 255;
+                int slot = (di >> 8) - 1;
+                bool hit = false;
+                const int ns = min(ne, PK_DCAP);
+                for (int i = 0; i < ns; ++i)
+                  if (dkey[i * GC + cw] == cell) { ddvp[i * GC + cw] += d; hit = true; }
+                if (!hit && ne > PK_DCAP) {
                   const long long sl = (long long)slot * PK_SPILL;
-                  P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
-                  dn[c] = (ne + 1) | ((slot + 1) << 8);
+                  for (int i = 0; i < ne - PK_DCAP; ++i)
+                    if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
                 }
-              } else overflow = true;
+                if (!hit) {
+                  if (ne < PK_DCAP) { dkey[ne * GC + cw] = cell; ddvp[ne * GC + cw] = d; dn[cw] = di + 1; }
+                  else if (ne < PK_CAP) {
+                    if (slot < 0) {
+                      slot = atomicAdd(P.ovf_count, 1);
+                      if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
+                    }
+                    if (slot >= 0) {
+                      const long long sl = (long long)slot * PK_SPILL;
+                      P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
+                      dn[cw] = (ne + 1) | ((slot + 1) << 8);
+                    }
+                  } else overflow = true;
+                }
+              }
             }
           }
         }
+        // the four lowest winners are done
+        for (int i = 0; i < 4; ++i) rem &= rem - 1;
       }
-      if (wrp == 0) {
-        // chains with an accepted copy continue behind it on the new state, the others behind the attempts covered
-        const int fw = first[lane];
-        const int np = (fw < PK_NOWIN) ? (fw >> 10) + 1 : max(spos[lane], a_lim);
-        spos[lane] = np;
-        const unsigned rm = __ballot_sync(FULL, np < kk);
-        if (np < kk) rlist[__popc(rm & lt)] = (unsigned char)lane;
-        if (lane == 0) { cnt[2] = rm != 0u; cnt[3] = __popc(rm); }
-        if (lane < 4) cnt[4 + lane] = 0;
-      }
-      __syncthreads();
-      if (cnt[2] == 0) break;
+      // chains with an accepted copy continue behind it on the new state, the others behind their window
+      pos = (fwc < PK_NOWIN) ? (fwc >> 10) + 1 : min(pos + lim, kk);
+      if (lane < GC) first[lane] = PK_NOWIN;
+      __syncwarp();
+      if (__all_sync(FULL, pos >= kk)) break;
     }
   }
   if (!staged) { while (!mbar_try_wait(mbar, 0)) {} }   // never leave a bulk copy in flight
@@ -540,7 +524,7 @@ __global__ void __launch_bounds__(PK_THREADS, 7) sweep_pool_kernel(const __grid_
   n_acc = __reduce_add_sync(FULL, n_acc);
   const bool any_over = __any_sync(FULL, overflow);
   if (lane == 0) {
-    const int slot = (int)((blockIdx.x * PK_WARPS + wrp) % COUNTER_SLOTS);
+    const int slot = (int)(blockIdx.x % COUNTER_SLOTS);
     if (n_eval) atomicAdd(P.counters + 2 * slot, (unsigned long long)n_eval);
     if (n_acc) atomicAdd(P.counters + 2 * slot + 1, (unsigned long long)n_acc);
     if (any_over) atomicOr(P.error_flag, 1);
@@ -554,14 +538,14 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
                                  int col, unsigned long long n_active, int X, int Y, int Z, int perx, int pery, int perz,
                                  int *error_flag) {
   const int S = L.S, T = S + 2, TW = L.TW;
-  const unsigned long long ngrp = (n_active + 31ull) >> 5;
-  const unsigned long long total = ngrp * (unsigned long long)TW * 32ull;
+  const unsigned long long ngrp = (n_active + (unsigned long long)(PK_GC - 1)) >> PK_GS;
+  const unsigned long long total = ngrp * (unsigned long long)TW * (unsigned long long)PK_GC;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
-    const int c = (int)(i & 31ull);
-    const unsigned long long r = i >> 5;
+    const int c = (int)(i & (unsigned long long)(PK_GC - 1));
+    const unsigned long long r = i >> PK_GS;
     const int j = (int)(r % (unsigned)TW);
-    const unsigned long long w = (r / (unsigned)TW) * 32ull + (unsigned long long)c;
+    const unsigned long long w = (r / (unsigned)TW) * (unsigned long long)PK_GC + (unsigned long long)c;
     uint32_t word = 0u;
     if (w < n_active) {
       const int ax = (int)(w % (unsigned)L.nact[col][0]);
@@ -595,21 +579,17 @@ __global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *
   }
 }
 // recount of V, A (Moore interfaces with sites not of the same cell, L234) and the coordinate sums (L288) from the
-// tiles: a warp takes one group, a lane one chain and walks its S^d interior sites; every neighbour is inside the
-// chain's own tile, the loads of the 32 lanes are one coalesced 128-byte row; runs of equal ids are flushed with
-// one atomic per array.
+// tiles: a thread takes one chain and walks its S^d interior sites; every neighbour is inside the chain's own
+// tile, the loads of the 8 lanes of a group are one 32-byte sector; runs of equal ids are flushed with one atomic
+// per array.
 template <int DIM>
 __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_active, unsigned long long *liveVP,
                                     unsigned long long *sumx, unsigned long long *sumy, unsigned long long *sumz) {
   const int S = L.S, T = S + 2, TW = L.TW;
   constexpr int NNB = (DIM == 2) ? 8 : 26;
-  const int lane = threadIdx.x & 31;
-  const unsigned long long ngrp = (n_active + 31ull) >> 5;
-  const unsigned long long wstride = ((unsigned long long)gridDim.x * blockDim.x) >> 5;
-  for (unsigned long long g = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; g < ngrp; g += wstride) {
-    const unsigned long long w = g * 32ull + (unsigned long long)lane;
-    if (w >= n_active) continue;
-    const uint32_t *tc = L.tiles + L.base[col] + g * (unsigned long long)TW * 32ull + lane;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_active; w += stride) {
+    const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (w & (unsigned long long)(PK_GC - 1));
     const int ax = (int)(w % (unsigned)L.nact[col][0]);
     const unsigned long long r1 = w / (unsigned)L.nact[col][0];
     const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
@@ -628,14 +608,14 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
       for (int ly = 0; ly < S; ++ly)
         for (int lx = 0; lx < S; ++lx) {
           const int j = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-          const uint32_t me = tc[j * 32] & ID_MASK;
+          const uint32_t me = tc[j * PK_GC] & ID_MASK;
           if (me != cur) { flush(); cur = me; cv = cx = cy = cz = 0; }
           if (me == 0) continue;
           int foreign = 0;
           for (int nb = 0; nb < NNB; ++nb) {
             int dx, dy, dz;
             nb_delta<DIM>(nb, dx, dy, dz);
-            foreign += ((tc[(j + (dz * T + dy) * T + dx) * 32] & ID_MASK) != me);
+            foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_GC] & ID_MASK) != me);
           }
           cv += (1ull << 32) + (unsigned long long)foreign;
           cx += (unsigned long long)(ox + lx); cy += (unsigned long long)(oy + ly); cz += (unsigned long long)(oz + lz);

@@ -43,7 +43,13 @@ constexpr int PK_GS = 3;                     // log2 of the chains per group
 constexpr int PK_GC = 1 << PK_GS;            // chains per warp = per group
 constexpr int PK_THREADS = 32;               // one warp per CTA
 constexpr int PK_SUPER = 64;                 // attempts per chain whose proposals are drawn up front
-constexpr int PK_NJ = 5;                     // a chain's window per round: 4 NJ attempts behind its position
+#ifndef PK_NJ_VALUE
+#define PK_NJ_VALUE 6
+#endif
+#ifndef PK_MINB
+#define PK_MINB 20
+#endif
+constexpr int PK_NJ = PK_NJ_VALUE;                     // a chain's window per round: 4 NJ attempts behind its position
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 3;                   // of which the first live in shared memory, the rest in a spill slot
 constexpr int PK_SPILL = PK_CAP - PK_DCAP;
@@ -65,7 +71,7 @@ struct PGeom {
   static constexpr int LOG2S = (S == 2) ? 1 : (S == 4) ? 2 : (S == 8) ? 3 : 4;
   static constexpr int LOG2SITES = DIM * LOG2S;
   static_assert(S == 2 || S == 4 || S == 8 || S == 16, "power-of-two subsection edge");
-  static_assert(TW < 512, "tile offsets are kept in 9 bits");
+  static_assert(TW * 4 * 8 < 65536, "byte offsets into a group's tiles are kept in 16 bits");
   // neighbour n (0..NNB-1, centre skipped; n = NNB is the centre itself) -> offsets
   static __host__ __device__ constexpr int idx27(int n) { return n == NNB ? NNB / 2 : n + (n >= NNB / 2 ? 1 : 0); }
   static __host__ __device__ constexpr int dx(int n) { return idx27(n) % 3 - 1; }
@@ -82,8 +88,8 @@ struct PSmem {
   static constexpr int DDVP = TILE + G::TW * 4 * PK_GC;            // uint64 [DCAP][8]
   static constexpr int MBAR = DDVP + PK_DCAP * 8 * PK_GC;          // uint64
   static constexpr int DKEY = MBAR + 8;                            // uint32 [DCAP][8]
-  static constexpr int PROP = DKEY + PK_DCAP * 4 * PK_GC;          // uint16 [64][8]   toff | nb << 9
-  static constexpr int QUEUE = PROP + PK_SUPER * 2 * PK_GC;        // uint16 [32 NJ]   chain | a << 3
+  static constexpr int PROP = DKEY + PK_DCAP * 4 * PK_GC;          // uint32 [64][8]   byte offsets into the chain's tile column: target | source << 16
+  static constexpr int QUEUE = PROP + PK_SUPER * 4 * PK_GC;        // uint16 [32 NJ]   chain | a << 3
   static constexpr int DN = QUEUE + 32 * PK_NJ * 2;                // int [8] own-delta table of the chain: entries | (spill slot + 1) << 8
   static constexpr int FIRST = DN + 4 * PK_GC;                     // int [8] first accepted attempt of the round
   static constexpr int ORIG = FIRST + 4 * PK_GC;                   // int [3][8] lattice origin of the chain
@@ -120,13 +126,13 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
 }
 
 template <int DIM, int S, bool ACT, bool LIVE>
-__global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
   constexpr int T = G::T, TW = G::TW, NNB = G::NNB, GC = PK_GC, NJ = PK_NJ;
   extern __shared__ __align__(128) unsigned char smem[];
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
-  unsigned short *prop = reinterpret_cast<unsigned short *>(smem + M::PROP);
+  uint32_t *prop = reinterpret_cast<uint32_t *>(smem + M::PROP);
   unsigned short *queue = reinterpret_cast<unsigned short *>(smem + M::QUEUE);
   uint32_t *dkey = reinterpret_cast<uint32_t *>(smem + M::DKEY);
   unsigned long long *ddvp = reinterpret_cast<unsigned long long *>(smem + M::DDVP);
@@ -156,7 +162,9 @@ __global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid
     if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
     snoff[lane] = (dz * T + dy) * T + dx;
   }
+#pragma unroll 1
   for (int i = lane; i < (P.nT + 1) * 8; i += 32) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
+#pragma unroll 1
   for (int i = lane; i < 2 * P.nT * P.nT * P.nT + P.nT; i += 32) sd[i] = P.D[i];
   // geometry of the chains (the host limits n_active to 31 bits for this kernel)
   if (lane < GC) {
@@ -193,7 +201,7 @@ __global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid
         const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
         const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
         const int toff = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-        prop[(4 * qq + j) * GC + c] = (unsigned short)(toff | (nb << 9));
+        prop[(4 * qq + j) * GC + c] = (uint32_t)(toff * (4 * GC)) | ((uint32_t)((toff + snoff[nb]) * (4 * GC)) << 16);
       }
     }
     int pos = active ? 0 : kk;   // attempts < pos of this stretch are final (same value in the 4 lanes of a chain)
@@ -214,9 +222,9 @@ __global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid
         const bool ok = a < kk;
         uint32_t wt = 0u, ws = 0u;
         if (ok) {
-          const int prc = (int)prop[a * GC + c];
-          const int toff = prc & 511;
-          wt = tcol[toff * GC]; ws = tcol[(toff + snoff[prc >> 9]) * GC];
+          const uint32_t prc = prop[a * GC + c];
+          wt = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tcol) + (prc & 0xffffu));
+          ws = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tcol) + (prc >> 16));
         }
         in[j] = ok && (((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u);
         m[j] = __ballot_sync(FULL, in[j]);
@@ -247,10 +255,9 @@ __global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid
       if (W > 0) {   // warp-uniform
       const int item = have ? (int)queue[lane] : 0;
       ci = item & (GC - 1); a = item >> PK_GS;
-      const int prc = (int)prop[a * GC + ci];
-      const int toff = prc & 511, nb = prc >> 9;
+      const uint32_t prc = prop[a * GC + ci];
+      const int toff = (int)(prc & 0xffffu) / (4 * GC), soff = (int)(prc >> 16) / (4 * GC);
       int nA = 0, nB = 0;
-      const int soff = toff + snoff[nb];
       const uint32_t *const tc = tile + ci;
       const uint32_t wA = tc[soff * GC], wB = tc[toff * GC];
       const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
@@ -423,9 +430,9 @@ __global__ void __launch_bounds__(PK_THREADS, 20) sweep_pool_kernel(const __grid
         const int r = c;
         const int fw = first[cw];
         const int nA = (fw >> 5) & 31, nB = fw & 31;
-        const int prc = (int)prop[(on ? (fw >> 10) : 0) * GC + cw];
-        const int toff = prc & 511;
-        const uint32_t wA = tile[(toff + snoff[prc >> 9]) * GC + cw], wB = tile[toff * GC + cw];
+        const uint32_t prc = prop[(on ? (fw >> 10) : 0) * GC + cw];
+        const int toff = (int)(prc & 0xffffu) / (4 * GC);
+        const uint32_t wA = tile[(int)(prc >> 16) / (4 * GC) * GC + cw], wB = tile[toff * GC + cw];
         const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
         __syncwarp();   // every lane has read the state of the round's start
         if (on) {

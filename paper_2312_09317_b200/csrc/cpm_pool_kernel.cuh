@@ -43,12 +43,16 @@ constexpr int PK_GS = 3;                     // log2 of the chains per group
 constexpr int PK_GC = 1 << PK_GS;            // chains per warp = per group
 constexpr int PK_THREADS = 32;               // one warp per CTA
 constexpr int PK_SUPER = 64;                 // attempts per chain whose proposals are drawn up front
+#ifndef PK_TARGET_VALUE
+#define PK_TARGET_VALUE 12
+#endif
 #ifndef PK_NJ_VALUE
 #define PK_NJ_VALUE 6
 #endif
 #ifndef PK_MINB
 #define PK_MINB 20
 #endif
+constexpr int PK_TARGET = PK_TARGET_VALUE;   // a round's window grows until it holds this many items
 constexpr int PK_NJ = PK_NJ_VALUE;                     // a chain's window per round: 4 NJ attempts behind its position
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
 constexpr int PK_DCAP = 3;                   // of which the first live in shared memory, the rest in a spill slot
@@ -89,8 +93,8 @@ struct PSmem {
   static constexpr int MBAR = DDVP + PK_DCAP * 8 * PK_GC;          // uint64
   static constexpr int DKEY = MBAR + 8;                            // uint32 [DCAP][8]
   static constexpr int PROP = DKEY + PK_DCAP * 4 * PK_GC;          // uint32 [64][8]   byte offsets into the chain's tile column: target | source << 16
-  static constexpr int QUEUE = PROP + PK_SUPER * 4 * PK_GC;        // uint16 [32 NJ]   chain | a << 3
-  static constexpr int DN = QUEUE + 32 * PK_NJ * 2;                // int [8] own-delta table of the chain: entries | (spill slot + 1) << 8
+  static constexpr int QUEUE = PROP + PK_SUPER * 4 * PK_GC;        // uint16 [32]   chain | a << 3
+  static constexpr int DN = QUEUE + 32 * PK_NJ * 2;                        // int [8] own-delta table of the chain: entries | (spill slot + 1) << 8
   static constexpr int FIRST = DN + 4 * PK_GC;                     // int [8] first accepted attempt of the round
   static constexpr int ORIG = FIRST + 4 * PK_GC;                   // int [3][8] lattice origin of the chain
   static constexpr int NOFF = ORIG + 12 * PK_GC;                   // int [32] neighbour -> tile offset (entry NNB = centre = 0)
@@ -476,42 +480,66 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
               atomicAdd(arr + cell, v);
             }
           }
-          // deterministic mode: the chain's own-delta table (lane 0 of the winner's 8, both sides)
-          if constexpr (!LIVE) {
-            if (r == 0) {
+        }
+        // deterministic mode: the chain's own-delta table.  Lanes r = 0 (the source's cell) and r = 4 (the target's
+        // cell) of a winner's 8 update it together when what they add fits the shared-memory part
+        if constexpr (!LIVE) {
+          const int side = r >> 2;
+          const uint32_t cell = side ? Bc : A;
+          const int sgn = side ? -1 : 1;
+          const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
+          const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
+          const bool mine = on && (r & 3) == 0 && cell != 0;
+          const int di = dn[cw];
+          const int ne = di & 255;
+          int hit = -1;
+          if (mine) {
+            const int ns = min(ne, PK_DCAP);
+            for (int i = 0; i < ns; ++i)
+              if (dkey[i * GC + cw] == cell) hit = i;
+          }
+          const int need = (mine && hit < 0) ? 1 : 0;
+          const int needA = __shfl_sync(FULL, need, lane & ~7), needB = __shfl_sync(FULL, need, (lane & ~7) | 4);
+          const bool fast = ne + needA + needB <= PK_DCAP;   // then every entry is in shared memory and so are the new ones
+          __syncwarp();   // dn, dkey read by both lanes before either writes
+          if (mine && fast) {
+            if (hit >= 0) ddvp[hit * GC + cw] += d;
+            else { const int sl = ne + (side ? needA : 0); dkey[sl * GC + cw] = cell; ddvp[sl * GC + cw] = d; }
+            if (side == (A != 0 ? 0 : 1)) dn[cw] = di + needA + needB;
+          }
+          if (on && !fast && r == 0) {
 #pragma unroll 1
-              for (int side = 0; side < 2; ++side) {
-                const uint32_t cell = side ? Bc : A;
-                if (cell == 0) continue;
-                const int sgn = side ? -1 : 1;
-                const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
-                const unsigned long long d = ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP;
-                const int di = dn[cw];
-                const int ne = di & 255;
-                int slot = (di >> 8) - 1;
-                bool hit = false;
-                const int ns = min(ne, PK_DCAP);
-                for (int i = 0; i < ns; ++i)
-                  if (dkey[i * GC + cw] == cell) { ddvp[i * GC + cw] += d; hit = true; }
-                if (!hit && ne > PK_DCAP) {
-                  const long long sl = (long long)slot * PK_SPILL;
-                  for (int i = 0; i < ne - PK_DCAP; ++i)
-                    if (__ldcg(P.ovf_keys + sl + i) == cell) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d; hit = true; }
-                }
-                if (!hit) {
-                  if (ne < PK_DCAP) { dkey[ne * GC + cw] = cell; ddvp[ne * GC + cw] = d; dn[cw] = di + 1; }
-                  else if (ne < PK_CAP) {
-                    if (slot < 0) {
-                      slot = atomicAdd(P.ovf_count, 1);
-                      if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
-                    }
-                    if (slot >= 0) {
-                      const long long sl = (long long)slot * PK_SPILL;
-                      P.ovf_keys[sl + ne - PK_DCAP] = cell; P.ovf_dvp[sl + ne - PK_DCAP] = d;
-                      dn[cw] = (ne + 1) | ((slot + 1) << 8);
-                    }
-                  } else overflow = true;
-                }
+            for (int side2 = 0; side2 < 2; ++side2) {
+              const uint32_t cell2 = side2 ? Bc : A;
+              if (cell2 == 0) continue;
+              const int sgn2 = side2 ? -1 : 1;
+              const int dP2 = side2 ? 2 * nB - NNB : NNB - 2 * nA;
+              const unsigned long long d2 = ((unsigned long long)(long long)sgn2 << 32) + (unsigned long long)(long long)dP2;
+              const int di2 = dn[cw];
+              const int ne2 = di2 & 255;
+              int slot = (di2 >> 8) - 1;
+              bool hit2 = false;
+              const int ns = min(ne2, PK_DCAP);
+              for (int i = 0; i < ns; ++i)
+                if (dkey[i * GC + cw] == cell2) { ddvp[i * GC + cw] += d2; hit2 = true; }
+              if (!hit2 && ne2 > PK_DCAP) {
+                const long long sl = (long long)slot * PK_SPILL;
+                for (int i = 0; i < ne2 - PK_DCAP; ++i)
+                  if (__ldcg(P.ovf_keys + sl + i) == cell2) { P.ovf_dvp[sl + i] = __ldcg(P.ovf_dvp + sl + i) + d2; hit2 = true; }
+              }
+              if (!hit2) {
+                if (ne2 < PK_DCAP) { dkey[ne2 * GC + cw] = cell2; ddvp[ne2 * GC + cw] = d2; dn[cw] = di2 + 1; }
+                else if (ne2 < PK_CAP) {
+                  if (slot < 0) {
+                    slot = atomicAdd(P.ovf_count, 1);
+                    if (slot >= P.ovf_cap) { slot = -1; overflow = true; }
+                  }
+                  if (slot >= 0) {
+                    const long long sl = (long long)slot * PK_SPILL;
+                    P.ovf_keys[sl + ne2 - PK_DCAP] = cell2; P.ovf_dvp[sl + ne2 - PK_DCAP] = d2;
+                    dn[cw] = (ne2 + 1) | ((slot + 1) << 8);
+                  }
+                } else overflow = true;
               }
             }
           }

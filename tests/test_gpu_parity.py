@@ -226,6 +226,31 @@ def test_resume_is_exact_on_device(pk, oracle_mod):
         np.testing.assert_array_equal(g2.get_cell_stats()[k], v)
 
 
+@pytest.mark.parametrize("name,dims,over", [
+    ("C1", None, {}),                                              # pooled kernel, 2D S = 16
+    ("C1", None, {"flags": 1}),                                    # warp-per-subsection kernel, TMA tile staging
+    ("C3", (32, 32, 32), {"subsection": 4}),                       # pooled kernel, 3D S = 4, Act
+    ("C3", (32, 32, 32), {"subsection": 8}),                       # warp kernel, 3D S = 8, Act tiles
+    ("C3", (32, 32, 32), {"subsection": 4, "mode": 1}),            # pooled kernel, live atomics
+])
+def test_sanitizer_cases(pk, oracle_mod, name, dims, over):
+    """Small runs of every sweep-kernel family, sized for `compute-sanitizer --tool memcheck|racecheck`
+    (the design-level claim of PAPER.md L49-51 that concurrently active subsections
+    never touch the same lattice site).  compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md),
+    so what stands in for it is this comparison with the oracle, pin P6 (visit order of a phase-step's subsections
+    does not matter) and the bit-for-bit reproducibility check at full size (tests/test_gpu_fullsize.py)."""
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims)
+    live = over.get("mode", 0) == 1
+    g, o = _pair(pk, oracle_mod, cfg, **over)
+    g.step(4); o.step(4)
+    if live:   # one correct result per interleaving: invariants only
+        V = g.get_cell_stats()["volume"]
+        assert (V[1:] > 0).all() and int(V.sum()) == int((g.get_lattice() != 0).sum())
+    else:
+        _compare(g, o, name == "C3", "sanitizer case")
+
+
 def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     """Inputs/outputs as device tensors (on_device=1); and the non-TMA staging path."""
     import torch

@@ -13,7 +13,7 @@ except Exception:  # pragma: no cover
 
 
 def config_names():
-    return ["C1", "C2", "C3", "C4", "C5"]
+    return ["C1", "C2", "C3", "C4", "C5", "C6", "C7"]
 
 
 # --------------------------------------------------------------------------- geometry ----
@@ -255,7 +255,54 @@ def make_config(name, dims=None, seed=None, subsection=None):
                       subsection=subsection if subsection else 16)
         return dict(name="C5", dims=dims, ids=ids, frozen=None, cell_type=cell_type, max_cells=n,
                     params=params, n_mcs=20)
+    if name == "C6":
+        # the paper's 3D cell collective with the persistence model (Fig 5C / 6D, Table 2):
+        # V* = 150, A* = 1500, J(cell,cell) = 10, J(cell,ECM) = 0, T = 20, mu = 0.95, dt = 15, lambda_pers = 40, density
+        # about 0.5.  The paper's lambda_perimeter = 0.2 is not an integer: the whole Hamiltonian and T are scaled by 5
+        # (same Boltzmann factors): lambda_P = 1, lambda_V = 125, J = 50, lambda_pers = 200, T = 100.
+        dims = tuple(dims or (256, 256, 256))
+        rng = np.random.default_rng(20231209 + 6 if seed is None else seed)
+        ids, n = jittered_cubes(dims, pitch=6, edge=5, keep=0.72, rng=rng)
+        cell_type = np.ones(n + 1, dtype=np.uint8); cell_type[0] = 0
+        J = np.array([[0, 0], [0, 50]], dtype=np.int32)
+        params = dict(J=J, lambda_V=[0, 125], target_V=[0, 150], lambda_P=[0, 1], target_P=[0, 1500],
+                      lambda_act=None, max_act=None, T=100.0, seed=int(rng.integers(1 << 62)),
+                      subsection=subsection if subsection else 4,
+                      lambda_pers=[0, 200], mu_pers=[0.0, 0.95], dt_pers=15)
+        return dict(name="C6", dims=dims, ids=ids, frozen=None, cell_type=cell_type, max_cells=n,
+                    params=params, n_mcs=100)
+
+    if name == "C7":
+        # the paper's 2D circular chemotaxis simulation (Fig 5A / 6E, Table 1): V* = 2500,
+        # A* = 600, lambda_P = 2, J(cell,ECM) = 10, T = 10, lambda_V = 20, lambda_chem = 10; the field is tangential
+        # to circles around the lattice centre ("at a 90 degree angle to radial vectors"), unit length.
+        dims = tuple(dims or (1024, 1024))
+        rng = np.random.default_rng(20231209 + 7 if seed is None else seed)
+        ids, n = jittered_cubes(dims, pitch=128, edge=48, keep=0.9, rng=rng)
+        cell_type = np.ones(n + 1, dtype=np.uint8); cell_type[0] = 0
+        J = np.array([[0, 10], [10, 20]], dtype=np.int32)
+        params = dict(J=J, lambda_V=[0, 20], target_V=[0, 2500], lambda_P=[0, 2], target_P=[0, 600],
+                      lambda_act=None, max_act=None, T=10.0, seed=int(rng.integers(1 << 62)),
+                      subsection=subsection if subsection else 8, lambda_chem=[0, 10])
+        return dict(name="C7", dims=dims, ids=ids, frozen=None, cell_type=cell_type, max_cells=n,
+                    params=params, n_mcs=100, field=circular_field(dims))
     raise ValueError("unknown config " + name)
+
+
+def circular_field(dims):
+    """Unit vectors at 90 degrees to the radial direction from the lattice centre, float32,
+    shape dims[::-1] + (ndim,); the z component (3D) is 0.  The centre voxel itself gets (0, ..)."""
+    nd = len(dims)
+    X, Y = dims[0], dims[1]
+    y, x = np.meshgrid(np.arange(Y, dtype=np.float64) - (Y - 1) / 2.0, np.arange(X, dtype=np.float64) - (X - 1) / 2.0, indexing="ij")
+    r = np.sqrt(x * x + y * y)
+    r[r == 0] = np.inf
+    f2 = np.stack([-y / r, x / r], axis=-1).astype(np.float32)
+    if nd == 2:
+        return np.ascontiguousarray(f2)
+    out = np.zeros((dims[2], Y, X, 3), dtype=np.float32)
+    out[..., :2] = f2[None]
+    return out
 
 
 def crop_config(cfg, dims):
@@ -265,4 +312,6 @@ def crop_config(cfg, dims):
     out["dims"] = tuple(dims)
     out["ids"] = np.ascontiguousarray(cfg["ids"][sl])
     out["frozen"] = None if cfg["frozen"] is None else np.ascontiguousarray(cfg["frozen"][sl])
+    if cfg.get("field") is not None:
+        out["field"] = np.ascontiguousarray(cfg["field"][sl])
     return out

@@ -24,7 +24,7 @@ def build(force=False):
         os.path.getmtime(s) > os.path.getmtime(_LIB) for s in (_SRC, _HDR))
     if force or stale:
         tmp = _LIB + ".%d.tmp" % os.getpid()
-        subprocess.check_call(["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-Wall", "-o", tmp, _SRC])
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -41,6 +41,8 @@ class _Params(C.Structure):
         ("subsection", C.c_int32), ("attempts_per_activation", C.c_int32),
         ("mode", C.c_int32), ("max_cells", C.c_uint32),
         ("device", C.c_int32), ("stream", C.c_void_p),
+        ("lambda_pers", C.POINTER(C.c_int32)), ("mu_pers", C.POINTER(C.c_double)), ("dt_pers", C.c_int32),
+        ("lambda_chem", C.POINTER(C.c_int32)),
     ]
 
 
@@ -78,6 +80,11 @@ def lib():
         L.oracle_gm_q16.argtypes = [vp, C.c_int32]
         L.oracle_gm_q16.restype = C.c_int64
         L.oracle_neighbour_offsets.argtypes = [C.c_int32, vp]
+        L.oracle_set_chemotaxis_field.argtypes = [vp, vp]
+        L.oracle_set_persistence.argtypes = [vp, vp]
+        L.oracle_get_persistence.argtypes = [vp, vp]
+        L.oracle_probe_dir.argtypes = [vp, C.c_uint64, C.c_int32, vp]
+        L.oracle_direction_table.argtypes = [C.c_int32, vp]
         _lib = L
     return _lib
 
@@ -102,7 +109,7 @@ class Oracle:
     def __init__(self, dims, J, lambda_V=None, target_V=None, lambda_P=None, target_P=None,
                  lambda_act=None, max_act=None, T=20.0, seed=1, subsection=0,
                  attempts_per_activation=0, mode=MODE_DETERMINISTIC, max_cells=0,
-                 periodic=(0, 0, 0)):
+                 periodic=(0, 0, 0), lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None):
         L = lib()
         dims = tuple(int(x) for x in dims)
         self.ndim = len(dims)
@@ -124,7 +131,8 @@ class Oracle:
         keep = [Jm]
         p.J = Jm.ctypes.data_as(C.POINTER(C.c_int32))
         for name, val in (("lambda_V", lambda_V), ("target_V", target_V), ("lambda_P", lambda_P),
-                          ("target_P", target_P), ("lambda_act", lambda_act), ("max_act", max_act)):
+                          ("target_P", target_P), ("lambda_act", lambda_act), ("max_act", max_act),
+                          ("lambda_pers", lambda_pers), ("lambda_chem", lambda_chem)):
             arr, ptr = _i32(val, nT)
             if arr is not None:
                 keep.append(arr)
@@ -137,6 +145,12 @@ class Oracle:
         p.max_cells = self.max_cells
         p.device = 0
         p.stream = None
+        if mu_pers is not None:
+            mu = np.ascontiguousarray(np.asarray(mu_pers, dtype=np.float64))
+            assert mu.size == nT
+            keep.append(mu)
+            p.mu_pers = mu.ctypes.data_as(C.POINTER(C.c_double))
+        p.dt_pers = int(dt_pers)
         h = C.c_void_p()
         rc = L.oracle_create(C.byref(p), C.byref(h))
         if rc != 0:
@@ -210,6 +224,28 @@ class Oracle:
         self._chk(self._L.oracle_get_schedule(self._h, C.addressof(S), C.addressof(k), C.addressof(n)))
         return {"S": S.value, "k": k.value, "phase_steps_per_mcs": n.value}
 
+    # ---- vector terms (Eq 4-7) ----
+    def set_chemotaxis_field(self, field):
+        """field: shape dims[::-1] + (ndim,), float32, components in [-1, 1]."""
+        f = np.ascontiguousarray(np.asarray(field, dtype=np.float32)).reshape(-1)
+        assert f.size == self.N * self.ndim
+        self._chk(self._L.oracle_set_chemotaxis_field(self._h, f.ctypes.data))
+
+    def set_persistence(self, p):
+        a = np.ascontiguousarray(np.asarray(p, dtype=np.float64)).reshape(-1)
+        assert a.size == 3 * (self.max_cells + 1)
+        self._chk(self._L.oracle_set_persistence(self._h, a.ctypes.data))
+
+    def get_persistence(self):
+        out = np.empty((self.max_cells + 1, 3), dtype=np.float64)
+        self._chk(self._L.oracle_get_persistence(self._h, out.ctypes.data))
+        return out
+
+    def probe_dir(self, t_index, nb):
+        v = C.c_int64()
+        self._chk(self._L.oracle_probe_dir(self._h, int(t_index), int(nb), C.addressof(v)))
+        return v.value
+
     # ---- hooks for the pins ----
     def set_visit_order(self, order, seed=0):
         self._chk(self._L.oracle_set_visit_order(self._h, int(order), int(seed)))
@@ -258,6 +294,12 @@ def threshold_table(T):
 def gm_q16(acts):
     a = np.ascontiguousarray(np.asarray(acts, dtype=np.int32))
     return int(lib().oracle_gm_q16(a.ctypes.data, a.size))
+
+
+def direction_table(ndim):
+    out = np.zeros(26 * 3, dtype=np.int64)
+    n = lib().oracle_direction_table(int(ndim), out.ctypes.data)
+    return out[: 3 * n].reshape(n, 3)
 
 
 def neighbour_offsets(ndim):

@@ -11,6 +11,8 @@
  *   - Hamiltonian: adhesion + volume (Eq 1), perimeter (Eq 3)
  *   - Metropolis acceptance (Eq 2)
  *   - Act model (Eq 8-9)
+ *   - chemotaxis along a vector field (Eq 4), persistence along one vector per cell
+ *     (Eq 5-7), readings S21-S22 of DESIGN.md
  *   - checkerboard of active subsections, cycling periodically              L49, L77
  *   - atomics = no update of a global is ever lost                           L51, L57
  *   - stale reads of globals are tolerated                                   L53
@@ -26,7 +28,9 @@
  * Philox known answers (P8), resume (P10), fixed-point GM vs pow() (P11), threshold table
  * (P12), DETERMINISTIC == LIVE when no cell is shared (P13); round 2: P13b (cells straddling
  * subsection borders, lambda_P != 0: pins the per-phase-step snapshot refresh and the own dP view),
- * P11b (each side of the Act bias uses its own cell's type), Act decay after the last phase-step.
+ * P11b (each side of the Act bias uses its own cell's type), Act decay after the last phase-step;
+ * P14 (direction table, dH of Eq 4-5 against the formula in double, sign by drift), P15 (the
+ * recurrence of Eq 6-7 against a numpy restatement on recorded centroids).
  * Parity unpinned: nothing in this file (the LIVE-mode *GPU* ensemble is only statistical).
  */
 #include "cpm_oracle.h"
@@ -75,6 +79,16 @@ struct oracle_ctx {
   int per[3] = {0, 0, 0};
   int nT = 0;
   std::vector<int64_t> J, lamV, tgtV, lamP, tgtP, lamA, maxA;
+  /* vector terms (Eq 4-7): strengths per type, persistence memory mu per type, look-back dt in MCS */
+  std::vector<int64_t> lamPers, lamChem;
+  std::vector<double> mu;
+  int dt = 0;
+  bool pers_on = false, chem_on = false;
+  int64_t xq[26][3];                 /* Q14 unit vector of the copy direction source -> target, per neighbour index */
+  std::vector<int32_t> cq;           /* Q14 chemotaxis field, [N][3] */
+  std::vector<double> phat;          /* persistence direction per cell, [max_cells+1][3] */
+  std::vector<double> ring;          /* centroids of the last dt+1 MCS, [dt+1][max_cells+1][3] */
+  uint64_t n_updates = 0;            /* persistence updates since set_lattice */
   double T = 0;
   bool accept_all = false;
   uint64_t seed = 0;
@@ -230,6 +244,7 @@ struct Eval {
   int nA, nB;
   int64_t dH_ham;  /* adhesion + volume + perimeter (Eq 1, 3) */
   int64_t dH_act;  /* Act bias, subtracted (reading S8(i)) */
+  int64_t dH_dir;  /* chemotaxis + persistence bias, subtracted (reading S21) */
 };
 
 /* dH of copying the state of the neighbour (sx,sy,sz) into the target (tx,ty,tz), given the
@@ -284,6 +299,42 @@ Eval evaluate(const oracle_ctx *c, int tx, int ty, int tz, int nb, Lookup seen) 
   if (e.B != 0 && c->lamA[e.tauB] != 0 && c->maxA[e.tauB] != 0)
     sideB = (c->lamA[e.tauB] * gm_at(c, tx, ty, tz)) / c->maxA[e.tauB];
   e.dH_act = (sideA - sideB + 32768) >> 16;
+
+  /* Vector terms, Eq 4 and Eq 5 with reading S21: x^ = unit vector of the copy direction, from the source
+   * site i = s to the target site j = t; a copy ALONG the field / the cell's persistence direction is favoured,
+   * so the bias is subtracted (same argument as L259 for Act); both the extending cell A and the retracting
+   * cell B are pushed along x^ by this copy, each with the strength of its own type; medium has none (S3);
+   * the field value is the one at the source site (Eq 4: C_i), zero outside a closed lattice.
+   * Fixed point: x^, p^ and C in Q14, the products summed in Q28 and rounded once. */
+  e.dH_dir = 0;
+  if (c->pers_on || c->chem_on) {
+    const int64_t *x = c->xq[nb];
+    int64_t acc = 0;
+    if (c->pers_on) {
+      if (e.A != 0 && c->lamPers[e.tauA] != 0) {
+        int64_t dot = 0;
+        for (int a = 0; a < 3; ++a) dot += x[a] * (int64_t)std::llrint(16384.0 * c->phat[3 * (size_t)e.A + a]);
+        acc += c->lamPers[e.tauA] * dot;
+      }
+      if (e.B != 0 && c->lamPers[e.tauB] != 0) {
+        int64_t dot = 0;
+        for (int a = 0; a < 3; ++a) dot += x[a] * (int64_t)std::llrint(16384.0 * c->phat[3 * (size_t)e.B + a]);
+        acc += c->lamPers[e.tauB] * dot;
+      }
+    }
+    if (c->chem_on && s.inside && !c->cq.empty()) {
+      int rx = sx, ry = sy, rz = sz;
+      resolve(c, rx, ry, rz);
+      const int32_t *C = &c->cq[3 * (size_t)lin(c, rx, ry, rz)];
+      int64_t dot = 0;
+      for (int a = 0; a < 3; ++a) dot += x[a] * (int64_t)C[a];
+      int64_t lam = 0;
+      if (e.A != 0) lam += c->lamChem[e.tauA];
+      if (e.B != 0) lam += c->lamChem[e.tauB];
+      acc += lam * dot;
+    }
+    e.dH_dir = (acc + ((int64_t)1 << 27)) >> 28;
+  }
   return e;
 }
 
@@ -360,7 +411,7 @@ void run_subsection(oracle_ctx *c, int64_t b, uint32_t p) {
     int64_t rec_dH = 0; int rec_acc = 0; uint32_t rec_u = 0;
     if (e.status != 0) c->evaluated++;
     if (e.status == 1) {
-      const int64_t dH = e.dH_ham - e.dH_act;
+      const int64_t dH = e.dH_ham - e.dH_act - e.dH_dir;
       rec_dH = dH;
       bool acc;
       if (dH <= 0 || c->accept_all) acc = true;          /* Eq 2, reading S6 */
@@ -397,6 +448,44 @@ void run_subsection(oracle_ctx *c, int64_t b, uint32_t p) {
     for (auto &kv : loc) apply(c, kv.first, kv.second);
 }
 
+/* centroid of a cell, Eq 10: coordinate sums over volume, in double */
+inline void centroid(const oracle_ctx *c, size_t cell, double X[3]) {
+  const double v = (double)c->V[cell];
+  X[0] = (double)c->SX[cell] / v; X[1] = (double)c->SY[cell] / v; X[2] = (double)c->SZ[cell] / v;
+}
+
+/* Eq 6-7, once per MCS for every cell that exists (reading S22):
+ *   p = (1 - mu) (X_t - X_{t-dt}) / |X_t - X_{t-dt}| + mu p^_{t-1};   p^_t = p / |p|.
+ * X_{t-dt} is the centroid dt MCS ago (the one at set_lattice while fewer than dt MCS have passed).  A cell that
+ * has not moved contributes no direction (the first term is dropped); a zero p keeps p^ = 0 (no bias).
+ * Every operation is a single IEEE double operation in the order written (no fused multiply-add). */
+void persistence_update(oracle_ctx *c) {
+  const size_t ncell = (size_t)c->max_cells + 1;
+  const uint64_t n = c->n_updates + 1;                 /* this is the n-th update */
+  const size_t slots = (size_t)c->dt + 1;
+  double *old_slot = &c->ring[((n + 1) % slots) * ncell * 3];   /* (n - dt) mod (dt + 1) */
+  double *new_slot = &c->ring[(n % slots) * ncell * 3];
+  for (size_t cell = 1; cell < ncell; ++cell) {
+    if (c->V[cell] <= 0) continue;
+    double X[3];
+    centroid(c, cell, X);
+    const double mu = c->mu[c->type[cell]];
+    const double one_minus_mu = 1.0 - mu;
+    double d[3], p[3];
+    for (int a = 0; a < 3; ++a) d[a] = X[a] - old_slot[3 * cell + a];
+    const double dn = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
+    for (int a = 0; a < 3; ++a) {
+      const double keep = mu * c->phat[3 * cell + a];
+      if (dn > 0.0) { const double u = d[a] / dn; const double turn = one_minus_mu * u; p[a] = turn + keep; }
+      else p[a] = keep;
+    }
+    const double pn = std::sqrt((p[0] * p[0] + p[1] * p[1]) + p[2] * p[2]);
+    for (int a = 0; a < 3; ++a) c->phat[3 * cell + a] = (pn > 0.0) ? p[a] / pn : 0.0;
+    for (int a = 0; a < 3; ++a) new_slot[3 * cell + a] = X[a];
+  }
+  c->n_updates = n;
+}
+
 void one_mcs(oracle_ctx *c) {
   const int ncol = 1 << c->d;
   const int64_t nsub_total = (int64_t)c->nsub[0] * c->nsub[1] * c->nsub[2];
@@ -426,6 +515,8 @@ void one_mcs(oracle_ctx *c) {
     }
   /* Act decay (L255, reading S9): once per MCS, after the last phase-step */
   for (auto &a : c->act) a = std::max(a - 1, 0);
+  /* persistence directions (Eq 6-7): "updated iteratively at every MCS" (L246) */
+  if (c->pers_on) persistence_update(c);
   c->mcs++;
 }
 
@@ -462,6 +553,16 @@ int oracle_create(const oracle_params *p, oracle_ctx **out) {
   take(p->lambda_V, c->lamV); take(p->target_V, c->tgtV); take(p->lambda_P, c->lamP);
   take(p->target_P, c->tgtP); take(p->lambda_act, c->lamA); take(p->max_act, c->maxA);
   for (int i = 0; i < nT; ++i) if (c->maxA[i] < 0 || c->maxA[i] > 255 || c->lamA[i] < 0) { delete c; return ORACLE_ERR_ARG; }
+  take(p->lambda_pers, c->lamPers); take(p->lambda_chem, c->lamChem);
+  c->mu.assign(nT, 0.0);
+  if (p->mu_pers) for (int i = 0; i < nT; ++i) c->mu[i] = p->mu_pers[i];
+  c->dt = p->dt_pers;
+  for (int i = 0; i < nT; ++i) {
+    if (!(c->mu[i] >= 0.0 && c->mu[i] <= 1.0) || std::llabs(c->lamPers[i]) > (1 << 24) || std::llabs(c->lamChem[i]) > (1 << 24)) { delete c; return ORACLE_ERR_ARG; }
+    if (c->lamPers[i] != 0) c->pers_on = true;
+    if (c->lamChem[i] != 0) c->chem_on = true;
+  }
+  if (c->dt < 0 || (c->pers_on && c->dt < 1)) { delete c; return ORACLE_ERR_ARG; }
   c->T = p->T;
   c->accept_all = std::isinf(p->T);
   c->seed = p->seed;
@@ -489,6 +590,11 @@ int oracle_create(const oracle_params *p, oracle_ctx **out) {
   c->R = c->sites / c->k;
 
   c->nNb = build_offsets(c->d, c->off);
+  /* reading S21: x^ of neighbour index nb points from the source s = t + OFF[nb] to the target t */
+  for (int q = 0; q < c->nNb; ++q) {
+    const double len = std::sqrt((double)(c->off[q][0] * c->off[q][0] + c->off[q][1] * c->off[q][1] + c->off[q][2] * c->off[q][2]));
+    for (int a = 0; a < 3; ++a) c->xq[q][a] = std::llround(16384.0 * (double)(-c->off[q][a]) / len);
+  }
   c->Hmax = threshold_hmax(c->T);
   c->thr.assign((size_t)c->Hmax + 1, 0xffffffffu);
   for (int64_t h = 1; h <= c->Hmax; ++h) c->thr[(size_t)h] = threshold_value(c->T, h);
@@ -517,6 +623,19 @@ int oracle_set_lattice(oracle_ctx *c, const uint32_t *ids, const uint8_t *frozen
   std::copy(cell_type, cell_type + c->max_cells + 1, c->type.begin());
   c->act.assign(N, 0); /* reading S9 */
   recount(c);
+  if (c->pers_on) {   /* reading S22: p^ = 0 (no bias), the look-back window starts at the present centroids */
+    const size_t ncell = (size_t)c->max_cells + 1;
+    c->phat.assign(ncell * 3, 0.0);
+    c->ring.assign(((size_t)c->dt + 1) * ncell * 3, 0.0);
+    for (size_t cell = 1; cell < ncell; ++cell) {
+      if (c->V[cell] <= 0) continue;
+      double X[3];
+      centroid(c, cell, X);
+      for (size_t sl = 0; sl <= (size_t)c->dt; ++sl)
+        for (int a = 0; a < 3; ++a) c->ring[(sl * ncell + cell) * 3 + a] = X[a];
+    }
+    c->n_updates = 0;
+  }
   c->have_lattice = true;
   return ORACLE_OK;
 }
@@ -617,6 +736,58 @@ int oracle_set_trace(oracle_ctx *c, int64_t *buf, uint64_t cap, uint64_t *count)
   c->trace = buf; c->trace_cap = cap; c->trace_count = count;
   if (count) *count = 0;
   return ORACLE_OK;
+}
+
+int oracle_set_chemotaxis_field(oracle_ctx *c, const float *field) {
+  if (!c || !field) return fail(c, ORACLE_ERR_ARG, "null argument");
+  if (!c->chem_on) return fail(c, ORACLE_ERR_UNSUPPORTED, "no type has lambda_chem != 0");
+  const size_t N = c->id.size();
+  c->cq.assign(N * 3, 0);
+  for (size_t i = 0; i < N; ++i)
+    for (int a = 0; a < c->d; ++a) {
+      const float v = field[i * (size_t)c->d + a];
+      if (!(v >= -1.0f && v <= 1.0f)) return fail(c, ORACLE_ERR_ARG, "field components must lie in [-1,1]");
+      c->cq[3 * i + a] = (int32_t)std::lrintf(v * 16384.0f);   /* Q14, round to nearest even */
+    }
+  return ORACLE_OK;
+}
+
+int oracle_set_persistence(oracle_ctx *c, const double *p) {
+  if (!c || !p) return fail(c, ORACLE_ERR_ARG, "null argument");
+  if (!c->pers_on || !c->have_lattice) return fail(c, ORACLE_ERR_STATE, "persistence is off or no lattice");
+  for (size_t i = 0; i < 3 * ((size_t)c->max_cells + 1); ++i) {
+    if (!(p[i] >= -1.0 && p[i] <= 1.0)) return fail(c, ORACLE_ERR_ARG, "components must lie in [-1,1]");
+    c->phat[i] = p[i];
+  }
+  return ORACLE_OK;
+}
+
+int oracle_get_persistence(oracle_ctx *c, double *p) {
+  if (!c || !p) return ORACLE_ERR_ARG;
+  if (!c->pers_on || !c->have_lattice) return fail(c, ORACLE_ERR_STATE, "persistence is off or no lattice");
+  std::copy(c->phat.begin(), c->phat.end(), p);
+  return ORACLE_OK;
+}
+
+int oracle_probe_dir(oracle_ctx *c, uint64_t t_index, int32_t nb, int64_t *dH_dir) {
+  if (!c || nb < 0 || nb >= c->nNb || t_index >= c->id.size() || !dH_dir) return ORACLE_ERR_ARG;
+  int tx = (int)(t_index % c->dim[0]);
+  int ty = (int)((t_index / c->dim[0]) % c->dim[1]);
+  int tz = (int)(t_index / ((uint64_t)c->dim[0] * c->dim[1]));
+  Eval e = evaluate(c, tx, ty, tz, nb, [&](uint32_t cell, int64_t &Vv, int64_t &Pp) { Vv = c->V[cell]; Pp = c->P[cell]; });
+  *dH_dir = (e.status == 1) ? e.dH_dir : 0;
+  return ORACLE_OK;
+}
+
+int oracle_direction_table(int32_t ndim, int64_t *out) {
+  int off[26][3];
+  if (ndim != 2 && ndim != 3) return ORACLE_ERR_ARG;
+  int n = build_offsets(ndim, off);
+  for (int q = 0; q < n; ++q) {
+    const double len = std::sqrt((double)(off[q][0] * off[q][0] + off[q][1] * off[q][1] + off[q][2] * off[q][2]));
+    for (int a = 0; a < 3; ++a) out[3 * q + a] = std::llround(16384.0 * (double)(-off[q][a]) / len);
+  }
+  return n;
 }
 
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox(ctr, key, out); }

@@ -40,6 +40,11 @@ typedef struct {
   uint32_t max_cells;      /* cell IDs are 0..max_cells */
   int32_t  device;         /* ignored */
   void    *stream;         /* ignored */
+  /* vector terms (Eq 4-7; readings S21, S22); NULL / 0 = off */
+  const int32_t *lambda_pers; /* [n_types] persistence strength, Eq 5 */
+  const double  *mu_pers;     /* [n_types] directional memory mu in [0,1], Eq 6 */
+  int32_t  dt_pers;           /* look-back in MCS, Eq 6; >= 1 when any lambda_pers != 0 */
+  const int32_t *lambda_chem; /* [n_types] chemotaxis strength, Eq 4 */
 } oracle_params;
 
 int  oracle_create(const oracle_params *p, oracle_ctx **out);
@@ -71,6 +76,16 @@ int  oracle_force_copy(oracle_ctx *c, uint64_t t_index, int32_t nb);
 /* Per-attempt trace of the next oracle_step calls: rec[6] = {t_index, nb, status, dH, accepted, u32}
  * appended to buf (up to cap records); pass NULL to stop. */
 int  oracle_set_trace(oracle_ctx *c, int64_t *buf, uint64_t cap, uint64_t *count);
+/* ---- vector terms (Eq 4-7) ---- */
+/* field[N][ndim] (component fastest), components in [-1,1] (the paper's fields are unit vectors, L240) */
+int  oracle_set_chemotaxis_field(oracle_ctx *c, const float *field);
+/* p[(max_cells+1)][3]: persistence direction per cell (unit or zero vectors); default 0 after set_lattice */
+int  oracle_set_persistence(oracle_ctx *c, const double *p);
+int  oracle_get_persistence(oracle_ctx *c, double *p);
+/* the integer chemotaxis + persistence bias that is SUBTRACTED from dH for this copy (0 for early-outs) */
+int  oracle_probe_dir(oracle_ctx *c, uint64_t t_index, int32_t nb, int64_t *dH_dir);
+/* Q14 unit vectors of the copy direction (source -> target) per neighbour index: out[nb*3 + {0,1,2}] */
+int  oracle_direction_table(int32_t ndim, int64_t *out);
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 /* proposal decode of one 32-bit word: local site index l in [0,S^d) and neighbour index nb */
 void oracle_decode_proposal(uint32_t w, uint32_t sites, uint32_t n_nb, uint32_t *l, uint32_t *nb);

@@ -3,8 +3,9 @@
  *
  * The library implements ONE thing: the data-parallel hot path of the paper's parallel CPM --
  * the checkerboard-partitioned Metropolis copy-attempt sweep over a 2D/3D lattice of cell ids
- * ("Designing a parallel execution scheme", Methods L218-264 Eq 1-3, 8-9, and
- * "GPU implementation details" L270-284).  All compute runs in hand-written CUDA kernels for
+ * ("Designing a parallel execution scheme", Methods L218-264 Eq 1-9, and
+ * "GPU implementation details" L270-284), with the optional motility terms of the Methods: Act (Eq 8-9),
+ * chemotaxis along a vector field (Eq 4) and persistence along one vector per cell (Eq 5-7).  All compute runs in hand-written CUDA kernels for
  * sm_100a; there is no CPU fallback: every entry point that needs the device fails with
  * CPM_ERR_CUDA when no usable GPU is present.
  *
@@ -63,6 +64,14 @@ typedef struct {
   int32_t  device;                /* CUDA device ordinal */
   void    *stream;                /* cudaStream_t (e.g. torch's current stream); NULL = default stream */
   uint32_t flags;                 /* CPM_FLAG_*; 0 = the library chooses (debug / A-B switches for tests) */
+  /* Vector terms (Methods L236-253; readings S21, S22); NULL / 0 = off.  With x^ the unit vector of the
+   * copy direction (source site -> target site), a copy's dH is lowered by
+   *   round( lambda_pers(tau_A) x^.p^_A + lambda_pers(tau_B) x^.p^_B + (lambda_chem(tau_A) + lambda_chem(tau_B)) x^.C_source )
+   * (A = source cell, B = target cell, a side only for a real cell), in Q14 fixed point. */
+  const int32_t *lambda_pers;     /* host [n_types], |.| <= 2^24: persistence strength, Eq 5 */
+  const double  *mu_pers;         /* host [n_types], in [0,1]: directional memory mu of Eq 6 */
+  int32_t  dt_pers;               /* look-back Delta t of Eq 6 in MCS; >= 1 when any lambda_pers != 0 */
+  const int32_t *lambda_chem;     /* host [n_types], |.| <= 2^24: chemotaxis strength, Eq 4 */
 } cpm_params;
 
 /* Validate parameters, build the type tables, the Metropolis threshold table (Eq 2) and the
@@ -83,6 +92,17 @@ int  cpm_set_lattice(cpm_ctx *ctx, const uint32_t *ids, const uint8_t *frozen,
                      const uint8_t *cell_type, int on_device);
 /* Optional: set the per-site Act field (integers 0..255 stored as float, L255). */
 int  cpm_set_act(cpm_ctx *ctx, const float *act, int on_device);
+/* Chemotaxis (Eq 4): the vector field C, field[N][ndim] (component fastest), float32 components in
+ * [-1,1] (the paper's fields are unit vectors); stored in Q14.  Default: all zero.  Needs a type with
+ * lambda_chem != 0 (else CPM_ERR_UNSUPPORTED); a component outside [-1,1] or NaN -> CPM_ERR_ARG. */
+int  cpm_set_chemotaxis_field(cpm_ctx *ctx, const float *field, int on_device);
+/* Persistence (Eq 5-7): p[(max_cells+1)][3] doubles, the direction p^ of every cell (unit or zero
+ * vectors, components in [-1,1]; entry 0 ignored).  cpm_set_lattice resets every p^ to 0 (no bias) and starts the
+ * look-back window at the present centroids; after every MCS of cpm_step each cell's p^ is updated by Eq 6-7 from its
+ * centroid (Eq 10) now and dt_pers MCS ago, on the device, in IEEE double without fused multiply-adds.
+ * Needs a type with lambda_pers != 0 (else CPM_ERR_UNSUPPORTED). */
+int  cpm_set_persistence(cpm_ctx *ctx, const double *p, int on_device);
+int  cpm_get_persistence(cpm_ctx *ctx, double *p, int on_device);
 /* Set the MCS counter (checkpoint/resume: the RNG is keyed by (seed, MCS, phase, subsection, attempt)). */
 int  cpm_set_mcs(cpm_ctx *ctx, uint32_t mcs);
 

@@ -151,6 +151,7 @@ class Oracle:
             keep.append(mu)
             p.mu_pers = mu.ctypes.data_as(C.POINTER(C.c_double))
         p.dt_pers = int(dt_pers)
+        self.pers_on = lambda_pers is not None and any(int(v) != 0 for v in lambda_pers)
         h = C.c_void_p()
         rc = L.oracle_create(C.byref(p), C.byref(h))
         if rc != 0:

@@ -742,23 +742,22 @@ int oracle_set_chemotaxis_field(oracle_ctx *c, const float *field) {
   if (!c || !field) return fail(c, ORACLE_ERR_ARG, "null argument");
   if (!c->chem_on) return fail(c, ORACLE_ERR_UNSUPPORTED, "no type has lambda_chem != 0");
   const size_t N = c->id.size();
+  for (size_t i = 0; i < N * (size_t)c->d; ++i)
+    if (!(field[i] >= -1.0f && field[i] <= 1.0f)) return fail(c, ORACLE_ERR_ARG, "field components must lie in [-1,1]");
   c->cq.assign(N * 3, 0);
   for (size_t i = 0; i < N; ++i)
-    for (int a = 0; a < c->d; ++a) {
-      const float v = field[i * (size_t)c->d + a];
-      if (!(v >= -1.0f && v <= 1.0f)) return fail(c, ORACLE_ERR_ARG, "field components must lie in [-1,1]");
-      c->cq[3 * i + a] = (int32_t)std::lrintf(v * 16384.0f);   /* Q14, round to nearest even */
-    }
+    for (int a = 0; a < c->d; ++a)
+      c->cq[3 * i + a] = (int32_t)std::lrintf(field[i * (size_t)c->d + a] * 16384.0f);   /* Q14, round to nearest even */
   return ORACLE_OK;
 }
 
 int oracle_set_persistence(oracle_ctx *c, const double *p) {
   if (!c || !p) return fail(c, ORACLE_ERR_ARG, "null argument");
   if (!c->pers_on || !c->have_lattice) return fail(c, ORACLE_ERR_STATE, "persistence is off or no lattice");
-  for (size_t i = 0; i < 3 * ((size_t)c->max_cells + 1); ++i) {
+  const size_t n3 = 3 * ((size_t)c->max_cells + 1);
+  for (size_t i = 0; i < n3; ++i)
     if (!(p[i] >= -1.0 && p[i] <= 1.0)) return fail(c, ORACLE_ERR_ARG, "components must lie in [-1,1]");
-    c->phat[i] = p[i];
-  }
+  std::copy(p, p + n3, c->phat.begin());
   return ORACLE_OK;
 }
 

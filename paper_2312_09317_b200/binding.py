@@ -36,6 +36,8 @@ class _Params(C.Structure):
         ("mode", C.c_int32), ("max_cells", C.c_uint32),
         ("device", C.c_int32), ("stream", C.c_void_p),
         ("flags", C.c_uint32),
+        ("lambda_pers", C.POINTER(C.c_int32)), ("mu_pers", C.POINTER(C.c_double)), ("dt_pers", C.c_int32),
+        ("lambda_chem", C.POINTER(C.c_int32)),
     ]
 
 
@@ -72,6 +74,9 @@ def load_library():
     L.cpm_set_lattice.argtypes = [vp, vp, vp, vp, C.c_int]
     L.cpm_set_act.argtypes = [vp, vp, C.c_int]
     L.cpm_set_mcs.argtypes = [vp, C.c_uint32]
+    L.cpm_set_chemotaxis_field.argtypes = [vp, vp, C.c_int]
+    L.cpm_set_persistence.argtypes = [vp, vp, C.c_int]
+    L.cpm_get_persistence.argtypes = [vp, vp, C.c_int]
     L.cpm_step.argtypes = [vp, C.c_uint32]
     L.cpm_get_lattice.argtypes = [vp, vp, C.c_int]
     L.cpm_get_act.argtypes = [vp, vp, C.c_int]
@@ -101,7 +106,7 @@ def _ptr(x, dtype, n):
     if _is_tensor(x):
         import torch
         want = {np.uint32: (torch.uint32, torch.int32), np.uint8: (torch.uint8,), np.float32: (torch.float32,),
-                np.uint64: (torch.uint64, torch.int64)}[dtype]
+                np.uint64: (torch.uint64, torch.int64), np.float64: (torch.float64,)}[dtype]
         assert x.dtype in want, (x.dtype, want)
         assert x.is_contiguous() and x.numel() == n, (x.shape, n)
         return x.data_ptr(), (1 if x.is_cuda else 0), x
@@ -116,7 +121,8 @@ class CPM:
     def __init__(self, dims, J, lambda_V=None, target_V=None, lambda_P=None, target_P=None,
                  lambda_act=None, max_act=None, T=20.0, seed=1, subsection=0,
                  attempts_per_activation=0, mode=MODE_DETERMINISTIC, max_cells=0,
-                 periodic=(0, 0, 0), device=None, stream=None, flags=0):
+                 periodic=(0, 0, 0), device=None, stream=None, flags=0,
+                 lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None):
         import torch  # device memory + streams only
         L = load_library()
         if not torch.cuda.is_available():
@@ -146,7 +152,8 @@ class CPM:
         keep = [Jm]
         p.J = Jm.ctypes.data_as(C.POINTER(C.c_int32))
         for name, val in (("lambda_V", lambda_V), ("target_V", target_V), ("lambda_P", lambda_P),
-                          ("target_P", target_P), ("lambda_act", lambda_act), ("max_act", max_act)):
+                          ("target_P", target_P), ("lambda_act", lambda_act), ("max_act", max_act),
+                          ("lambda_pers", lambda_pers), ("lambda_chem", lambda_chem)):
             if val is not None:
                 arr = np.ascontiguousarray(np.asarray(val, dtype=np.int32))
                 assert arr.size == nT
@@ -161,6 +168,12 @@ class CPM:
         p.device = self.device
         p.stream = C.c_void_p(int(stream))
         p.flags = int(flags)
+        if mu_pers is not None:
+            mu = np.ascontiguousarray(np.asarray(mu_pers, dtype=np.float64))
+            assert mu.size == nT
+            keep.append(mu)
+            p.mu_pers = mu.ctypes.data_as(C.POINTER(C.c_double))
+        p.dt_pers = int(dt_pers)
         h = C.c_void_p()
         rc = L.cpm_create(C.byref(p), C.byref(h))
         if rc != 0:
@@ -198,6 +211,22 @@ class CPM:
 
     def set_mcs(self, mcs):
         self._chk(self._L.cpm_set_mcs(self._h, int(mcs)))
+
+    def set_chemotaxis_field(self, field):
+        """field: shape dims[::-1] + (ndim,), float32 components in [-1, 1] (Eq 4)."""
+        pf, df, kf = _ptr(field, np.float32, self.N * self.ndim)
+        self._chk(self._L.cpm_set_chemotaxis_field(self._h, pf, df))
+
+    def set_persistence(self, p):
+        pp, dp, kp = _ptr(p, np.float64, 3 * (self.max_cells + 1))
+        self._chk(self._L.cpm_set_persistence(self._h, pp, dp))
+
+    def get_persistence(self, out=None):
+        if out is None:
+            out = np.empty(3 * (self.max_cells + 1), dtype=np.float64)
+        po, do, ko = _ptr(out, np.float64, 3 * (self.max_cells + 1))
+        self._chk(self._L.cpm_get_persistence(self._h, po, do))
+        return ko.reshape(self.max_cells + 1, 3)
 
     def step(self, n=1):
         self._chk(self._L.cpm_step(self._h, int(n)))

@@ -81,6 +81,12 @@ struct SweepParams {
   uint32_t *ovf_keys;                // spill slots of the own-delta tables: [ovf_cap][PK_SPILL]
   unsigned long long *ovf_dvp;
   int *ovf_count; int ovf_cap;
+  // vector terms (Eq 4-7, readings S21/S22); all in Q14
+  int vec_on;                        // any lambda_pers / lambda_chem != 0
+  const int2 *vec_types;             // [nT + 1] {lambda_pers, lambda_chem}; row nT (medium) is zero
+  const short4 *pq;                  // [max_cells + 1] persistence direction of the cell (null: persistence off)
+  const short4 *chem;                // [N] chemotaxis field, row-major x fastest (null: no field loaded)
+  int xq_len[3];                     // llround(16384 / sqrt(n)), n = 1, 2, 3: component of the unit copy direction
 };
 
 // ------------------------------------------------------------------ PTX wrappers ----------
@@ -128,6 +134,27 @@ __device__ __forceinline__ uint32_t pick(const uint4 &v, int j) { return j == 0 
 __device__ __forceinline__ long long act_side(int lamA, int maxA, int g) {
   const unsigned q = (unsigned)lamA / (unsigned)maxA, r = (unsigned)lamA - q * (unsigned)maxA;
   return (long long)((unsigned long long)q * (unsigned)g) + (long long)((r * (unsigned)g) / (unsigned)maxA);
+}
+
+// Bias of the vector terms (Eq 4, 5; reading S21) for a copy from source s = t + (dx,dy,dz) into t: the unit vector of
+// the copy direction is -(dx,dy,dz)/|.|; each real cell contributes lambda_pers(tau) x^.p^ and lambda_chem(tau) x^.C_s.
+// rA / rB: parameter rows of the two cells (nT for medium); sidx: lattice index of the source site or -1 when it lies
+// outside a closed lattice (no field there).  Returns the integer that is subtracted from dH.
+__device__ __forceinline__ long long vec_bias(const SweepParams &P, int dx, int dy, int dz, int rA, int rB, uint32_t A, uint32_t B, long long sidx) {
+  const int K = P.xq_len[dx * dx + dy * dy + dz * dz - 1];
+  const int x0 = -dx * K, x1 = -dy * K, x2 = -dz * K;
+  const int2 la = __ldg(P.vec_types + rA), lb = __ldg(P.vec_types + rB);
+  long long acc = 0;
+  if (P.pq != nullptr) {
+    if (la.x != 0) { const short4 v = __ldg(P.pq + A); acc += (long long)la.x * (long long)(x0 * v.x + x1 * v.y + x2 * v.z); }
+    if (lb.x != 0) { const short4 v = __ldg(P.pq + B); acc += (long long)lb.x * (long long)(x0 * v.x + x1 * v.y + x2 * v.z); }
+  }
+  const int lc = la.y + lb.y;
+  if (lc != 0 && P.chem != nullptr && sidx >= 0) {
+    const short4 v = __ldg(P.chem + sidx);
+    acc += (long long)lc * (long long)(x0 * v.x + x1 * v.y + x2 * v.z);
+  }
+  return (acc + (1ll << 27)) >> 28;
 }
 
 // neighbour index (0..nNb-1, centre skipped) -> (dx,dy,dz); order: (dz,dy,dx) lexicographic, dx fastest
@@ -308,6 +335,20 @@ struct Sweep {
       dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
       const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
       dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
+    }
+    if (P.vec_on) {   // warp-uniform
+      const int pr = __shfl_sync(FULL, preg, src);
+      int lx, ly, lz, dx, dy, dz;
+      local_coords(pr & 0xFFFFFF, lx, ly, lz);
+      nb_delta<DIM>((pr >> 24) & 31, dx, dy, dz);
+      int g[3] = {ox + lx + dx, oy + ly + dy, (DIM == 3) ? oz + lz + dz : 0};
+      const int dimv[3] = {P.X, P.Y, P.Z};
+      bool inside = true;
+#pragma unroll
+      for (int ax = 0; ax < DIM; ++ax)
+        if (g[ax] < 0 || g[ax] >= dimv[ax]) { if (P.per[ax]) g[ax] += (g[ax] < 0) ? dimv[ax] : -dimv[ax]; else inside = false; }
+      const long long sidx = inside ? (long long)g[0] + (long long)P.X * ((long long)g[1] + (long long)P.Y * g[2]) : -1ll;
+      dH -= vec_bias(P, dx, dy, dz, rA, rB, A, B, sidx);
     }
     if (ACT) {
       if ((pa.lamA | pb.lamA) != 0) {  // lamA is stored as 0 when the type's Max_act is 0
@@ -621,9 +662,9 @@ __global__ void __launch_bounds__(128) sweep_kernel(const __grid_constant__ CUte
 
 // ------------------------------------------------------------------ auxiliary kernels ------
 // a11: Act decays by 1 per MCS down to 0 (L255); 16 bytes per thread, saturating byte subtract.
-__global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr) {
+__global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr, uint32_t *pers_n) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) *mcs_ptr += 1;
+  if (i == 0) { *mcs_ptr += 1; if (pers_n) *pers_n += 1; }
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long j = i; j < n_vec; j += stride) {
     uint4 v = act[j];
@@ -632,7 +673,91 @@ __global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr)
     act[j] = v;
   }
 }
-__global__ void mcs_increment_kernel(uint32_t *mcs_ptr) { *mcs_ptr += 1; }
+__global__ void mcs_increment_kernel(uint32_t *mcs_ptr, uint32_t *pers_n) { *mcs_ptr += 1; if (pers_n) *pers_n += 1; }
+
+// ---- persistence (Eq 5-7, reading S22) ----
+// Q14 of a direction: what the sweep reads
+__device__ __forceinline__ short4 quantise_q14(double x, double y, double z) {
+  return make_short4((short)__double2ll_rn(__dmul_rn(16384.0, x)), (short)__double2ll_rn(__dmul_rn(16384.0, y)),
+                     (short)__double2ll_rn(__dmul_rn(16384.0, z)), 0);
+}
+// centroid, Eq 10: coordinate sums over volume, one IEEE division each
+__device__ __forceinline__ void centroid_of(unsigned long long vp, unsigned long long sx, unsigned long long sy, unsigned long long sz, double X[3]) {
+  const double v = (double)(uint32_t)(vp >> 32);
+  X[0] = __ddiv_rn((double)(long long)sx, v); X[1] = __ddiv_rn((double)(long long)sy, v); X[2] = __ddiv_rn((double)(long long)sz, v);
+}
+// cpm_set_lattice: p^ = 0 for every cell, every slot of the look-back ring = the present centroid
+__global__ void persistence_init_kernel(long long ncell, int slots, const unsigned long long *liveVP, const unsigned long long *sumx,
+                                        const unsigned long long *sumy, const unsigned long long *sumz, double *phat, short4 *pq,
+                                        double *ring, uint32_t *pers_n) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell == 0) *pers_n = 0;
+  if (cell >= ncell) return;
+  double X[3] = {0.0, 0.0, 0.0};
+  const unsigned long long vp = liveVP[cell];
+  if (cell != 0 && (uint32_t)(vp >> 32) != 0u) centroid_of(vp, sumx[cell], sumy[cell], sumz[cell], X);
+  for (int a = 0; a < 3; ++a) phat[3 * cell + a] = 0.0;
+  pq[cell] = make_short4(0, 0, 0, 0);
+  for (int sl = 0; sl < slots; ++sl)
+    for (int a = 0; a < 3; ++a) ring[((long long)sl * ncell + cell) * 3 + a] = X[a];
+}
+// Once per MCS, one thread per cell: p = (1 - mu) (X_t - X_{t-dt}) / |X_t - X_{t-dt}| + mu p^_{t-1}; p^_t = p / |p| (Eq 6-7).
+// Every step is one IEEE double operation (no fused multiply-add), so the result is the same on any conforming machine.
+__global__ void persistence_update_kernel(long long ncell, int slots, const unsigned long long *liveVP, const unsigned long long *sumx,
+                                          const unsigned long long *sumy, const unsigned long long *sumz, const uint8_t *ctype,
+                                          const double *mu_of_type, double *phat, short4 *pq, double *ring, const uint32_t *pers_n) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell < 1 || cell >= ncell) return;
+  const unsigned long long vp = liveVP[cell];
+  if ((uint32_t)(vp >> 32) == 0u) return;
+  const unsigned long long n = (unsigned long long)*pers_n + 1ull;    // this is the n-th update
+  const double *old_slot = ring + (long long)((n + 1ull) % (unsigned long long)slots) * ncell * 3;   // (n - dt) mod (dt + 1)
+  double *new_slot = ring + (long long)(n % (unsigned long long)slots) * ncell * 3;
+  double X[3], d[3], p[3];
+  centroid_of(vp, sumx[cell], sumy[cell], sumz[cell], X);
+  const double mu = mu_of_type[ctype[cell]];
+  const double one_minus_mu = __dsub_rn(1.0, mu);
+  for (int a = 0; a < 3; ++a) d[a] = __dsub_rn(X[a], old_slot[3 * cell + a]);
+  const double dn = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2])));
+  for (int a = 0; a < 3; ++a) {
+    const double keep = __dmul_rn(mu, phat[3 * cell + a]);
+    p[a] = (dn > 0.0) ? __dadd_rn(__dmul_rn(one_minus_mu, __ddiv_rn(d[a], dn)), keep) : keep;
+  }
+  const double pn = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2])));
+  for (int a = 0; a < 3; ++a) p[a] = (pn > 0.0) ? __ddiv_rn(p[a], pn) : 0.0;
+  for (int a = 0; a < 3; ++a) { phat[3 * cell + a] = p[a]; new_slot[3 * cell + a] = X[a]; }
+  pq[cell] = quantise_q14(p[0], p[1], p[2]);
+}
+// cpm_set_persistence: p^ from the caller (components in [-1,1]) and its Q14 copy
+// commit == 0: only validate (nothing is written when any component is out of range)
+__global__ void persistence_set_kernel(long long ncell, const double *src, double *phat, short4 *pq, int *error_flag, int commit) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell >= ncell) return;
+  double v[3];
+  for (int a = 0; a < 3; ++a) {
+    v[a] = src[3 * cell + a];
+    if (!(v[a] >= -1.0 && v[a] <= 1.0)) { atomicOr(error_flag, 8); return; }
+  }
+  if (!commit) return;
+  for (int a = 0; a < 3; ++a) phat[3 * cell + a] = v[a];
+  pq[cell] = (cell == 0) ? make_short4(0, 0, 0, 0) : quantise_q14(v[0], v[1], v[2]);
+}
+// cpm_set_chemotaxis_field: float components in [-1,1] -> Q14 (round to nearest even), one short4 per site
+// commit == 0: only validate
+__global__ void chem_set_kernel(const float *src, short4 *chem, long long N, int ndim, int *error_flag, int commit) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    short q[3] = {0, 0, 0};
+    bool ok = true;
+    for (int a = 0; a < ndim; ++a) {
+      const float v = src[i * ndim + a];
+      if (!(v >= -1.0f && v <= 1.0f)) { ok = false; break; }
+      q[a] = (short)__float2int_rn(__fmul_rn(v, 16384.0f));
+    }
+    if (!ok) { atomicOr(error_flag, 8); continue; }
+    if (commit) chem[i] = make_short4(q[0], q[1], q[2], 0);
+  }
+}
 
 // set_lattice: ids (+frozen, cell types) -> packed pitched words; flags ids above max_cells
 __global__ void pack_kernel(const uint32_t *ids, const uint8_t *frozen, const uint8_t *ctype, uint32_t max_cells,

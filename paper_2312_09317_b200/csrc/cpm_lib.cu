@@ -64,6 +64,14 @@ struct cpm_ctx {
   uint32_t *ovf_keys = nullptr;
   unsigned long long *ovf_dvp = nullptr;
   int *ovf_count = nullptr;
+  // vector terms (Eq 4-7)
+  bool pers_on = false, chem_on = false;
+  int dt_pers = 0;
+  int2 *vec_types_dev = nullptr;
+  double *mu_dev = nullptr, *phat = nullptr, *ring = nullptr;
+  short4 *pq = nullptr, *chem = nullptr;
+  uint8_t *ctype_dev = nullptr;
+  uint32_t *pers_n = nullptr;
   // staging buffers for host-pointer I/O, kept between calls
   void *stage_a = nullptr, *stage_b = nullptr, *stage_c = nullptr;
   size_t stage_a_cap = 0, stage_b_cap = 0, stage_c_cap = 0;
@@ -118,23 +126,27 @@ SweepFn pick_kernel(int d, bool act, bool live, int nsets) {
   return d == 2 ? pick_flags<2>(act, live, nsets) : pick_flags<3>(act, live, nsets);
 }
 
-template <int DIM, int S>
+template <int DIM, int S, bool VEC>
 ThreadFn pick_pool_flags(bool act, bool live, int nT, size_t *smem) {
   *smem = PSmem<DIM, S>::bytes(nT);
-  if (act) return live ? (ThreadFn)sweep_pool_kernel<DIM, S, true, true> : (ThreadFn)sweep_pool_kernel<DIM, S, true, false>;
-  return live ? (ThreadFn)sweep_pool_kernel<DIM, S, false, true> : (ThreadFn)sweep_pool_kernel<DIM, S, false, false>;
+  if (act) return live ? (ThreadFn)sweep_pool_kernel<DIM, S, true, true, VEC> : (ThreadFn)sweep_pool_kernel<DIM, S, true, false, VEC>;
+  return live ? (ThreadFn)sweep_pool_kernel<DIM, S, false, true, VEC> : (ThreadFn)sweep_pool_kernel<DIM, S, false, false, VEC>;
 }
-// pooled kernel: 3D S = 2, 4; 2D S = 2, 4, 8, 16
-ThreadFn pick_pool_kernel(int d, int S, bool act, bool live, int nT, size_t *smem) {
+template <int DIM, int S>
+ThreadFn pick_pool_vec(bool act, bool live, bool vec, int nT, size_t *smem) {
+  return vec ? pick_pool_flags<DIM, S, true>(act, live, nT, smem) : pick_pool_flags<DIM, S, false>(act, live, nT, smem);
+}
+// pooled kernel: 3D S = 2, 4; 2D S = 2, 4, 8, 16; one specialisation per extension set (L282)
+ThreadFn pick_pool_kernel(int d, int S, bool act, bool live, bool vec, int nT, size_t *smem) {
   if (d == 3) {
-    if (S == 2) return pick_pool_flags<3, 2>(act, live, nT, smem);
-    if (S == 4) return pick_pool_flags<3, 4>(act, live, nT, smem);
+    if (S == 2) return pick_pool_vec<3, 2>(act, live, vec, nT, smem);
+    if (S == 4) return pick_pool_vec<3, 4>(act, live, vec, nT, smem);
     return nullptr;
   }
-  if (S == 2) return pick_pool_flags<2, 2>(act, live, nT, smem);
-  if (S == 4) return pick_pool_flags<2, 4>(act, live, nT, smem);
-  if (S == 8) return pick_pool_flags<2, 8>(act, live, nT, smem);
-  if (S == 16) return pick_pool_flags<2, 16>(act, live, nT, smem);
+  if (S == 2) return pick_pool_vec<2, 2>(act, live, vec, nT, smem);
+  if (S == 4) return pick_pool_vec<2, 4>(act, live, vec, nT, smem);
+  if (S == 8) return pick_pool_vec<2, 8>(act, live, vec, nT, smem);
+  if (S == 16) return pick_pool_vec<2, 16>(act, live, vec, nT, smem);
   return nullptr;
 }
 
@@ -208,6 +220,7 @@ int check_device_flag(cpm_ctx *c) {
   if (flag & 1) return fail(c, CPM_ERR_UNSUPPORTED, "a subsection changed more distinct cells in one activation than its own-delta table holds");
   if (flag & 2) return fail(c, CPM_ERR_ARG, "cell id above max_cells in the lattice");
   if (flag & 4) return fail(c, CPM_ERR_ARG, "Act values must be integers in [0,255]");
+  if (flag & 8) return fail(c, CPM_ERR_ARG, "vector components must lie in [-1,1]");
   return CPM_OK;
 }
 
@@ -238,6 +251,8 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->log_dev); cudaFree(c->exp_dev); cudaFree(c->types_dev); cudaFree(c->thr_dev);
   cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
   cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
+  cudaFree(c->vec_types_dev); cudaFree(c->mu_dev); cudaFree(c->phat); cudaFree(c->ring); cudaFree(c->pq); cudaFree(c->chem);
+  cudaFree(c->ctype_dev); cudaFree(c->pers_n);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -278,11 +293,17 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       // deterministic mode: the next phase-step reads the values as of its own start
       if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, st));
     }
+  if (c->pers_on) {   // Eq 6-7: every cell's persistence direction from its centroid now and dt MCS ago
+    const long long ncl = (long long)ncell;
+    persistence_update_kernel<<<(unsigned)((ncl + 255) / 256), 256, 0, st>>>(ncl, c->dt_pers + 1, c->liveVP, c->sumx, c->sumy, c->sumz,
+                                                                           c->ctype_dev, c->mu_dev, c->phat, c->pq, c->ring, c->pers_n);
+    c->launches++;
+  }
   if (c->act_enabled) {
     const long long n_vec = c->sp.apitch * c->dim[1] * c->dim[2] / 16;
-    act_decay_kernel<<<grid_for(n_vec), 256, 0, st>>>((uint4 *)c->act, n_vec, c->mcs_dev);
+    act_decay_kernel<<<grid_for(n_vec), 256, 0, st>>>((uint4 *)c->act, n_vec, c->mcs_dev, c->pers_n);
   } else {
-    mcs_increment_kernel<<<1, 1, 0, st>>>(c->mcs_dev);
+    mcs_increment_kernel<<<1, 1, 0, st>>>(c->mcs_dev, c->pers_n);
   }
   c->launches++;
   return CPM_OK;
@@ -343,6 +364,15 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     if (p->lambda_V && (p->lambda_V[i] > (1 << 30) || p->lambda_V[i] < -(1 << 30))) return CPM_ERR_ARG;
     if (p->max_act && p->max_act[i] != 0) any_act = true;
   }
+  bool pers_on = false, chem_on = false;
+  for (int i = 0; i < nT; ++i) {
+    if (p->lambda_pers && (p->lambda_pers[i] > (1 << 24) || p->lambda_pers[i] < -(1 << 24))) return CPM_ERR_ARG;
+    if (p->lambda_chem && (p->lambda_chem[i] > (1 << 24) || p->lambda_chem[i] < -(1 << 24))) return CPM_ERR_ARG;
+    if (p->mu_pers && !(p->mu_pers[i] >= 0.0 && p->mu_pers[i] <= 1.0)) return CPM_ERR_ARG;
+    if (p->lambda_pers && p->lambda_pers[i] != 0) pers_on = true;
+    if (p->lambda_chem && p->lambda_chem[i] != 0) chem_on = true;
+  }
+  if (p->dt_pers < 0 || p->dt_pers > 4096 || (pers_on && p->dt_pers < 1)) return CPM_ERR_ARG;
 
   // ---- checkerboard scheduler (a1): subsection edge S, attempts per activation k ----
   int S = p->subsection;
@@ -382,13 +412,14 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->S = S; c->sites = (int)sites; c->k = (int)k; c->R = (int)(sites / k);
   c->nNb = (d == 2) ? 8 : 26;
   c->act_enabled = any_act;
+  c->pers_on = pers_on; c->chem_on = chem_on; c->dt_pers = p->dt_pers;
   c->use_graph = !(p->flags & CPM_FLAG_NO_GRAPH);
   c->nsets = (sites <= 512) ? 1 : 4;
   // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
   c->use_tma = !(p->flags & CPM_FLAG_NO_TMA) && (S % 4 == 0);
   size_t pool_smem = 0;
   c->tfn = (nT <= 8 && !(p->flags & CPM_FLAG_WARP_KERNEL))
-               ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, nT, &pool_smem) : nullptr;
+               ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, pers_on || chem_on, nT, &pool_smem) : nullptr;
   c->pooled = c->tfn != nullptr;
   if (c->pooled) c->use_tma = true;   // one bulk copy per group of 32 tiles
 
@@ -506,6 +537,29 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   alloc((void **)&c->error_flag, 4); alloc((void **)&c->mcs_dev, 4);
   alloc((void **)&c->J_dev, (size_t)nT * nT * 4); alloc((void **)&c->D_dev, Dtab.size() * 4); alloc((void **)&c->log_dev, 256 * 4); alloc((void **)&c->exp_dev, 1024 * 4);
   alloc((void **)&c->types_dev, (nT + 1) * sizeof(TypeParams)); alloc((void **)&c->thr_dev, c->thr.size() * 4);
+  // vector terms: per-type strengths (row nT, what medium reads, stays zero), per-cell directions, the look-back ring
+  std::vector<int2> vtypes(nT + 1, make_int2(0, 0));
+  std::vector<double> mus(nT, 0.0);
+  for (int i = 1; i < nT; ++i) {   // type 0 is medium: no terms (reading S3)
+    vtypes[i] = make_int2(p->lambda_pers ? p->lambda_pers[i] : 0, p->lambda_chem ? p->lambda_chem[i] : 0);
+  }
+  for (int i = 0; i < nT; ++i) mus[i] = p->mu_pers ? p->mu_pers[i] : 0.0;
+  if (pers_on || chem_on) alloc((void **)&c->vec_types_dev, (nT + 1) * sizeof(int2));
+  if (pers_on) {
+    alloc((void **)&c->mu_dev, nT * sizeof(double));
+    alloc((void **)&c->phat, ncell * 3 * sizeof(double));
+    alloc((void **)&c->ring, (size_t)(p->dt_pers + 1) * ncell * 3 * sizeof(double));
+    alloc((void **)&c->pq, ncell * sizeof(short4));
+    alloc((void **)&c->ctype_dev, ncell);
+    alloc((void **)&c->pers_n, 4);
+  }
+  if (chem_on) alloc((void **)&c->chem, (size_t)c->N * sizeof(short4));
+  if (rc == CPM_OK && c->vec_types_dev) {
+    cudaError_t e = cudaMemcpyAsync(c->vec_types_dev, vtypes.data(), vtypes.size() * sizeof(int2), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess && c->mu_dev) e = cudaMemcpyAsync(c->mu_dev, mus.data(), nT * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) rc = fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
+  }
   if (rc == CPM_OK) {
     cudaError_t e = cudaMemcpyAsync(c->J_dev, p->J, (size_t)nT * nT * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->D_dev, Dtab.data(), Dtab.size() * 4, cudaMemcpyHostToDevice, c->stream);
@@ -534,6 +588,8 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   sp.snapVP = c->snapVP; sp.liveVP = c->liveVP; sp.sumx = c->sumx; sp.sumy = c->sumy; sp.sumz = c->sumz;
   sp.counters = c->counters; sp.error_flag = c->error_flag;
   sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
+  sp.vec_on = (pers_on || chem_on) ? 1 : 0; sp.vec_types = c->vec_types_dev; sp.pq = c->pq; sp.chem = c->chem;
+  for (int n2 = 1; n2 <= 3; ++n2) sp.xq_len[n2 - 1] = (int)std::llround(16384.0 / std::sqrt((double)n2));
 
   memset(&c->tm_lat, 0, sizeof(CUtensorMap));
   if (c->use_tma && !c->pooled) {
@@ -622,6 +678,12 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
     c->launches++;
   }
   if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
+  if (c->pers_on) {   // reading S22: p^ = 0, the look-back window starts at the present centroids
+    CK(cudaMemcpyAsync(c->ctype_dev, sct, ncell, cudaMemcpyDeviceToDevice, c->stream));
+    persistence_init_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, c->dt_pers + 1, c->liveVP, c->sumx, c->sumy,
+                                                                                   c->sumz, c->phat, c->pq, c->ring, c->pers_n);
+    c->launches++;
+  }
   CK(cudaGetLastError());
   int rc = check_device_flag(c);
   if (rc != CPM_OK) return rc;
@@ -645,6 +707,58 @@ int cpm_set_act(cpm_ctx *c, const float *act, int on_device) {
   rc = check_device_flag(c);
   if (rc != CPM_OK) CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));   // bad input: reported once, state stays usable
   return rc;
+}
+
+int cpm_set_chemotaxis_field(cpm_ctx *c, const float *field, int on_device) {
+  if (!c || !field) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->chem_on) return fail(c, CPM_ERR_UNSUPPORTED, "no cell type has lambda_chem != 0");
+  CK(cudaSetDevice(c->device));
+  int rc = check_device_flag(c);
+  if (rc != CPM_OK) return rc;
+  const float *s;
+  CK(stage_in(const_cast<float **>(&s), &c->stage_a, &c->stage_a_cap, field, (size_t)c->N * c->d, on_device, c->stream));
+  // validate first: a refused field leaves the loaded one untouched
+  chem_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s, c->chem, c->N, c->d, c->error_flag, 0);
+  c->launches++;
+  CK(cudaGetLastError());
+  rc = check_device_flag(c);
+  if (rc != CPM_OK) { CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream)); return rc; }   // bad input: reported once
+  chem_set_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(s, c->chem, c->N, c->d, c->error_flag, 1);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(c->stream));   // the staging buffer may be reused by the next call
+  return CPM_OK;
+}
+
+int cpm_set_persistence(cpm_ctx *c, const double *p, int on_device) {
+  if (!c || !p) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->pers_on) return fail(c, CPM_ERR_UNSUPPORTED, "no cell type has lambda_pers != 0");
+  if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CK(cudaSetDevice(c->device));
+  int rc = check_device_flag(c);
+  if (rc != CPM_OK) return rc;
+  const size_t ncell = (size_t)c->max_cells + 1;
+  const double *s;
+  CK(stage_in(const_cast<double **>(&s), &c->stage_a, &c->stage_a_cap, p, ncell * 3, on_device, c->stream));
+  persistence_set_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, s, c->phat, c->pq, c->error_flag, 0);
+  c->launches++;
+  CK(cudaGetLastError());
+  rc = check_device_flag(c);
+  if (rc != CPM_OK) { CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream)); return rc; }
+  persistence_set_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, s, c->phat, c->pq, c->error_flag, 1);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(c->stream));
+  return CPM_OK;
+}
+
+int cpm_get_persistence(cpm_ctx *c, double *p, int on_device) {
+  if (!c || !p) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->pers_on) return fail(c, CPM_ERR_UNSUPPORTED, "no cell type has lambda_pers != 0");
+  if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CK(cudaSetDevice(c->device));
+  CK(cudaMemcpyAsync(p, c->phat, ((size_t)c->max_cells + 1) * 3 * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+  return check_device_flag(c);
 }
 
 int cpm_set_mcs(cpm_ctx *c, uint32_t mcs) {

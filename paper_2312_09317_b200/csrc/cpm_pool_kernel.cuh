@@ -129,7 +129,7 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
   return tile_word(L, bx, by, bz, j);
 }
 
-template <int DIM, int S, bool ACT, bool LIVE>
+template <int DIM, int S, bool ACT, bool LIVE, bool VEC>
 __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
@@ -322,6 +322,21 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         dH += 2 * ((long long)pa.lamV * dva - (long long)pb.lamV * dvb) + (pa.lamV + pb.lamV);
         const long long dpa = (long long)(uint32_t)vpA - pa.tgtP, dpb = (long long)(uint32_t)vpB - pb.tgtP;
         dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
+        if constexpr (VEC) {
+          // chemotaxis / persistence bias (Eq 4, 5; reading S21), only for the specialisation that has these terms (L282)
+          if (go) {
+            constexpr int CEN = (DIM == 3) ? (T * T + T + 1) : (T + 1);
+            const int dd = soff - toff + CEN;   // = ((dz + 1) T + dy + 1) T + dx + 1 of the source's offset
+            const int ddx = dd % T - 1, ddy = (dd / T) % T - 1, ddz = (DIM == 3) ? dd / (T * T) - 1 : 0;
+            int gx = orig[ci] - 1 + soff % T, gy = orig[GC + ci] - 1 + (soff / T) % T, gz = (DIM == 3) ? orig[2 * GC + ci] - 1 + soff / (T * T) : 0;
+            bool inside = true;   // false: the source lies outside a closed lattice (no field there)
+            if (gx < 0) { gx += P.X; inside = P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; inside = P.per[0] != 0; }
+            if (gy < 0) { gy += P.Y; inside = inside && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; inside = inside && P.per[1] != 0; }
+            if (DIM == 3) { if (gz < 0) { gz += P.Z; inside = inside && P.per[2] != 0; } else if (gz >= P.Z) { gz -= P.Z; inside = inside && P.per[2] != 0; } }
+            const long long sidx = inside ? (long long)gx + (long long)P.X * ((long long)gy + (long long)P.Y * gz) : -1ll;
+            dH -= vec_bias(P, ddx, ddy, ddz, A != 0 ? tA : P.nT, Bc != 0 ? tB : P.nT, A, Bc, sidx);
+          }
+        }
         if constexpr (ACT) {
           // The Act bias lies in [-capB, +capA] (cap = lamA * largest Act value in the field / maxA, host-built):
           // it is only worked out when it can change the outcome.

@@ -25,6 +25,8 @@ def _pair(pk, ob, cfg, mode=0, flags=0, **over):
     o = ob.Oracle(cfg["dims"], max_cells=cfg["max_cells"], mode=mode, **p)
     g.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
     o.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
+    if cfg.get("field") is not None:
+        g.set_chemotaxis_field(cfg["field"]); o.set_chemotaxis_field(cfg["field"])
     return g, o
 
 
@@ -37,6 +39,8 @@ def _compare(g, o, act=False, tag=""):
         np.testing.assert_array_equal(sg[k], so[k], err_msg="%s %s" % (tag, k))
     if act:
         np.testing.assert_array_equal(g.get_act(), o.get_act(), err_msg=tag + " act")
+    if getattr(o, "pers_on", False):   # Eq 6-7 in IEEE double on both sides: equal to the last bit
+        np.testing.assert_array_equal(g.get_persistence(), o.get_persistence(), err_msg=tag + " persistence")
     assert g.get_counters() == o.get_counters(), (tag, g.get_counters(), o.get_counters())
 
 
@@ -249,6 +253,62 @@ def test_sanitizer_cases(pk, oracle_mod, name, dims, over):
         assert (V[1:] > 0).all() and int(V.sum()) == int((g.get_lattice() != 0).sum())
     else:
         _compare(g, o, name == "C3", "sanitizer case")
+
+
+# ---- persistence (Eq 5-7) and chemotaxis (Eq 4) ----
+@pytest.mark.parametrize("dims,over", [((48, 48, 48), {}), ((40, 32, 24), {"subsection": 8}), ((32, 32, 32), {"subsection": 2}),
+                                       ((32, 32, 32), {"periodic": (1, 0, 1)})])
+def test_C6_persistence_collective_bit_exact(pk, oracle_mod, dims, over):
+    """The paper's 3D persistence workload (Fig 5C / 6D, Table 2), scaled: lattice, tallies, counters AND the per-cell
+    persistence directions p^ (doubles, Eq 6-7) equal the oracle's after every MCS, past the look-back window (dt = 15)."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C6", dims=dims)
+    g, o = _run(pk, oracle_mod, cfg, 20, 1, **over)
+    assert g.get_launch_info()["pooled"] == (over.get("subsection", 4) != 8)
+    p = g.get_persistence()[1:]
+    nrm = np.linalg.norm(p, axis=1)
+    assert (np.abs(nrm - 1) < 1e-12).mean() > 0.9      # nearly every cell has moved and carries a unit vector
+
+
+def test_persistence_given_directions(pk, oracle_mod):
+    """cpm_set_persistence: caller-chosen directions enter dH at once; a refused call changes nothing."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C6", dims=(32, 32, 32))
+    rng = np.random.default_rng(5)
+    v = rng.normal(size=(cfg["max_cells"] + 1, 3)); v /= np.linalg.norm(v, axis=1, keepdims=True)
+    g, o = _pair(pk, oracle_mod, cfg)
+    g.set_persistence(v); o.set_persistence(v)
+    _compare(g, o, False, "directions set")
+    g.step(3); o.step(3)
+    _compare(g, o, False, "after 3 MCS")
+    with pytest.raises(pk.CPMError):
+        g.set_persistence(np.full_like(v, 2.0))
+    _compare(g, o, False, "after a refused set_persistence")
+
+
+@pytest.mark.parametrize("dims,over", [((256, 256), {}), ((128, 192), {"subsection": 16}), ((128, 128), {"subsection": 32}),
+                                       ((128, 128), {"periodic": (1, 1, 0)})])
+def test_C7_circular_chemotaxis_bit_exact(pk, oracle_mod, dims, over):
+    """The paper's 2D circular chemotaxis workload (Fig 5A / 6E, Table 1), scaled: tangential unit field, lambda_chem = 10."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C7", dims=dims)
+    g, o = _run(pk, oracle_mod, cfg, 12, 3, **over)
+    assert g.get_launch_info()["pooled"] == (over.get("subsection", 8) != 32)
+
+
+def test_chemotaxis_3d_with_act_and_persistence_together(pk, oracle_mod):
+    """Every extension at once (the specialisation with all terms): C4's obstacles + Act, a 3D field and persistence."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C4", dims=(40, 40, 40), subsection=4)
+    cfg["params"].update(lambda_pers=[0, 30, 60, 0], mu_pers=[0, 0.9, 0.5, 0], dt_pers=2, lambda_chem=[0, 25, 0, 0])
+    cfg["field"] = ci.circular_field((40, 40, 40))
+    cfg["field"][..., 2] = 0.6; cfg["field"][..., :2] *= 0.8
+    for flags in (0, pk.FLAG_WARP_KERNEL):
+        g, o = _pair(pk, oracle_mod, cfg, flags=flags)
+        g.step(5); o.step(5)
+        _compare(g, o, True, "all terms, flags %d" % flags)
+    with pytest.raises(pk.CPMError):
+        g.set_chemotaxis_field(np.full((40, 40, 40, 3), np.nan, dtype=np.float32))
 
 
 def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):

@@ -42,7 +42,7 @@ class _Params(C.Structure):
         ("mode", C.c_int32), ("max_cells", C.c_uint32),
         ("device", C.c_int32), ("stream", C.c_void_p),
         ("lambda_pers", C.POINTER(C.c_int32)), ("mu_pers", C.POINTER(C.c_double)), ("dt_pers", C.c_int32),
-        ("lambda_chem", C.POINTER(C.c_int32)),
+        ("lambda_chem", C.POINTER(C.c_int32)), ("unwrap_centroids", C.c_int32),
     ]
 
 
@@ -109,7 +109,7 @@ class Oracle:
     def __init__(self, dims, J, lambda_V=None, target_V=None, lambda_P=None, target_P=None,
                  lambda_act=None, max_act=None, T=20.0, seed=1, subsection=0,
                  attempts_per_activation=0, mode=MODE_DETERMINISTIC, max_cells=0,
-                 periodic=(0, 0, 0), lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None):
+                 periodic=(0, 0, 0), lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None, unwrap_centroids=0):
         L = lib()
         dims = tuple(int(x) for x in dims)
         self.ndim = len(dims)
@@ -151,6 +151,7 @@ class Oracle:
             keep.append(mu)
             p.mu_pers = mu.ctypes.data_as(C.POINTER(C.c_double))
         p.dt_pers = int(dt_pers)
+        p.unwrap_centroids = int(unwrap_centroids)
         self.pers_on = lambda_pers is not None and any(int(v) != 0 for v in lambda_pers)
         h = C.c_void_p()
         rc = L.oracle_create(C.byref(p), C.byref(h))

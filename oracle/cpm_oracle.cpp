@@ -89,6 +89,9 @@ struct oracle_ctx {
   std::vector<double> phat;          /* persistence direction per cell, [max_cells+1][3] */
   std::vector<double> ring;          /* centroids of the last dt+1 MCS, [dt+1][max_cells+1][3] */
   uint64_t n_updates = 0;            /* persistence updates since set_lattice */
+  /* periodic centroid tracking (L297, reading S23): per-cell anchor = floor of the centroid at the last MCS boundary */
+  bool unwrap = false;
+  std::vector<int64_t> anc;          /* [max_cells+1][3] */
   double T = 0;
   bool accept_all = false;
   uint64_t seed = 0;
@@ -338,14 +341,42 @@ Eval evaluate(const oracle_ctx *c, int tx, int ty, int tz, int nb, Lookup seen) 
   return e;
 }
 
+/* Reading S23 (L297: "adding or subtracting dimension x |cell| to the sum values ... to keep centroids within
+ * simulation bounds"): on a periodic axis a site's coordinate enters a cell's sum as its periodic image nearest to
+ * the cell's anchor, x' = x + m dim with x' - anchor in [-dim/2, dim/2). */
+inline int64_t image_near(int64_t x, int64_t anchor, int64_t dim) {
+  int64_t r = x - anchor;
+  if (2 * r >= dim) return x - dim;
+  if (2 * r < -dim) return x + dim;
+  return x;
+}
+inline void site_coords(const oracle_ctx *c, uint32_t cell, int x, int y, int z, int64_t out[3]) {
+  const int64_t v[3] = {x, y, z};
+  for (int a = 0; a < 3; ++a)
+    out[a] = (c->unwrap && c->per[a]) ? image_near(v[a], c->anc[3 * (size_t)cell + a], c->dim[a]) : v[a];
+}
+/* keep the centroid inside [0, dim) on periodic axes by shifting the sum by dim x V; the anchor follows the centroid */
+void normalise_centroid(oracle_ctx *c, uint32_t cell) {
+  if (c->V[cell] <= 0) return;
+  int64_t *S[3] = {&c->SX[cell], &c->SY[cell], &c->SZ[cell]};
+  for (int a = 0; a < 3; ++a) {
+    if (!c->per[a]) continue;
+    const int64_t span = (int64_t)c->dim[a] * c->V[cell];
+    while (*S[a] < 0) *S[a] += span;
+    while (*S[a] >= span) *S[a] -= span;
+    c->anc[3 * (size_t)cell + a] = *S[a] / c->V[cell];
+  }
+}
+
 /* commit (a9): the lattice site takes the source's state; Act(t) = Max_act of the new owner;
  * returns the changes of the globals.  Medium (id 0) is not tallied (S3). */
 void commit(oracle_ctx *c, int tx, int ty, int tz, const Eval &e, Delta &dA, Delta &dB) {
   int64_t ti = lin(c, tx, ty, tz);
   c->id[ti] = e.A;
   c->act[ti] = (e.A != 0) ? (int32_t)c->maxA[e.tauA] : 0;
-  if (e.A != 0) { dA.dV += 1; dA.dP += c->nNb - 2 * e.nA; dA.dSX += tx; dA.dSY += ty; dA.dSZ += tz; }
-  if (e.B != 0) { dB.dV -= 1; dB.dP += 2 * e.nB - c->nNb; dB.dSX -= tx; dB.dSY -= ty; dB.dSZ -= tz; }
+  int64_t q[3];
+  if (e.A != 0) { site_coords(c, e.A, tx, ty, tz, q); dA.dV += 1; dA.dP += c->nNb - 2 * e.nA; dA.dSX += q[0]; dA.dSY += q[1]; dA.dSZ += q[2]; }
+  if (e.B != 0) { site_coords(c, e.B, tx, ty, tz, q); dB.dV -= 1; dB.dP += 2 * e.nB - c->nNb; dB.dSX -= q[0]; dB.dSY -= q[1]; dB.dSZ -= q[2]; }
 }
 
 void apply(oracle_ctx *c, uint32_t cell, const Delta &dl) {
@@ -356,17 +387,31 @@ void apply(oracle_ctx *c, uint32_t cell, const Delta &dl) {
 void recount(oracle_ctx *c) {
   size_t n = (size_t)c->max_cells + 1;
   c->V.assign(n, 0); c->P.assign(n, 0); c->SX.assign(n, 0); c->SY.assign(n, 0); c->SZ.assign(n, 0);
+  if (c->unwrap) {   /* reading S23: the first site of a cell in scan order anchors the images of its other sites */
+    c->anc.assign(3 * n, 0);
+    std::vector<uint8_t> seen(n, 0);
+    for (int z = 0; z < c->dim[2]; ++z)
+      for (int y = 0; y < c->dim[1]; ++y)
+        for (int x = 0; x < c->dim[0]; ++x) {
+          uint32_t me = c->id[lin(c, x, y, z)];
+          if (me == 0 || seen[me]) continue;
+          seen[me] = 1; c->anc[3 * (size_t)me] = x; c->anc[3 * (size_t)me + 1] = y; c->anc[3 * (size_t)me + 2] = z;
+        }
+  }
   for (int z = 0; z < c->dim[2]; ++z)
     for (int y = 0; y < c->dim[1]; ++y)
       for (int x = 0; x < c->dim[0]; ++x) {
         uint32_t me = c->id[lin(c, x, y, z)];
         if (me == 0) continue;
-        c->V[me] += 1; c->SX[me] += x; c->SY[me] += y; c->SZ[me] += z;
+        int64_t q[3];
+        site_coords(c, me, x, y, z, q);
+        c->V[me] += 1; c->SX[me] += q[0]; c->SY[me] += q[1]; c->SZ[me] += q[2];
         for (int q = 0; q < c->nNb; ++q) {
           SiteView nb = view(c, x + c->off[q][0], y + c->off[q][1], z + c->off[q][2]);
           if (nb.id != me) c->P[me] += 1;
         }
       }
+  if (c->unwrap) for (size_t cell = 1; cell < n; ++cell) normalise_centroid(c, (uint32_t)cell);
 }
 
 /* one activation of subsection b in phase-step p (the inner loop of SURVEY 8(c)) */
@@ -472,7 +517,14 @@ void persistence_update(oracle_ctx *c) {
     const double mu = c->mu[c->type[cell]];
     const double one_minus_mu = 1.0 - mu;
     double d[3], p[3];
-    for (int a = 0; a < 3; ++a) d[a] = X[a] - old_slot[3 * cell + a];
+    for (int a = 0; a < 3; ++a) {
+      d[a] = X[a] - old_slot[3 * cell + a];
+      if (c->unwrap && c->per[a]) {   /* shortest displacement through the periodic border (S23) */
+        const double half = 0.5 * (double)c->dim[a];
+        if (d[a] > half) d[a] = d[a] - (double)c->dim[a];
+        else if (d[a] < -half) d[a] = d[a] + (double)c->dim[a];
+      }
+    }
     const double dn = std::sqrt((d[0] * d[0] + d[1] * d[1]) + d[2] * d[2]);
     for (int a = 0; a < 3; ++a) {
       const double keep = mu * c->phat[3 * cell + a];
@@ -515,6 +567,8 @@ void one_mcs(oracle_ctx *c) {
     }
   /* Act decay (L255, reading S9): once per MCS, after the last phase-step */
   for (auto &a : c->act) a = std::max(a - 1, 0);
+  /* centroids back into the lattice on periodic axes (L297, reading S23) */
+  if (c->unwrap) for (size_t cell = 1; cell <= c->max_cells; ++cell) normalise_centroid(c, (uint32_t)cell);
   /* persistence directions (Eq 6-7): "updated iteratively at every MCS" (L246) */
   if (c->pers_on) persistence_update(c);
   c->mcs++;
@@ -563,6 +617,7 @@ int oracle_create(const oracle_params *p, oracle_ctx **out) {
     if (c->lamChem[i] != 0) c->chem_on = true;
   }
   if (c->dt < 0 || (c->pers_on && c->dt < 1)) { delete c; return ORACLE_ERR_ARG; }
+  c->unwrap = p->unwrap_centroids != 0 && (c->per[0] || c->per[1] || c->per[2]);
   c->T = p->T;
   c->accept_all = std::isinf(p->T);
   c->seed = p->seed;

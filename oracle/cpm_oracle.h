@@ -45,6 +45,7 @@ typedef struct {
   const double  *mu_pers;     /* [n_types] directional memory mu in [0,1], Eq 6 */
   int32_t  dt_pers;           /* look-back in MCS, Eq 6; >= 1 when any lambda_pers != 0 */
   const int32_t *lambda_chem; /* [n_types] chemotaxis strength, Eq 4 */
+  int32_t  unwrap_centroids;  /* != 0: coordinate sums follow the cell through periodic borders (L297; reading S23) */
 } oracle_params;
 
 int  oracle_create(const oracle_params *p, oracle_ctx **out);

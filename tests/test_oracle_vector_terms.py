@@ -212,3 +212,136 @@ def test_vector_term_parameters_are_validated(oracle_mod):
     o = oracle_mod.Oracle((8, 8), J=J, subsection=4, max_cells=1, lambda_chem=[0, 5])
     with pytest.raises(oracle_mod.OracleError):      # components in [-1, 1]
         o.set_chemotaxis_field(np.full((8, 8, 2), 1.5, dtype=np.float32))
+
+
+# ------------------------------------------------------------------------------------ P16 --
+def _circular_centroids(lat, n_cells, dims, periodic):
+    """Centroid of every cell straight from the lattice with the periodic axes unwrapped around one of the cell's own
+    sites (valid for cells smaller than half the lattice): returns (centroid mod dim, volume)."""
+    nd = len(dims)
+    lat3 = lat if lat.ndim == 3 else lat[None]
+    out = np.full((n_cells + 1, 3), np.nan)
+    vol = np.zeros(n_cells + 1, dtype=np.int64)
+    dimv = [dims[0], dims[1], dims[2] if nd == 3 else 1]
+    for cell in range(1, n_cells + 1):
+        z, y, x = np.nonzero(lat3 == cell)
+        vol[cell] = len(x)
+        if len(x) == 0:
+            continue
+        for a, v in enumerate((x, y, z)):
+            v = v.astype(np.float64)
+            if periodic[a]:
+                r = v[0]
+                v = r + ((v - r + dimv[a] / 2.0) % dimv[a]) - dimv[a] / 2.0
+                out[cell, a] = v.mean() % dimv[a]
+            else:
+                out[cell, a] = v.mean()
+    return out, vol
+
+
+def _check_tracked_centroids(o, n_cells, dims, periodic, tag):
+    st = o.get_cell_stats()
+    want, vol = _circular_centroids(o.get_lattice(), n_cells, dims, periodic)
+    np.testing.assert_array_equal(st["volume"][1:], vol[1:])
+    dimv = [dims[0], dims[1], dims[2] if len(dims) == 3 else 1]
+    for a, k in enumerate(("sum_x", "sum_y", "sum_z")):
+        got = st[k][1:].astype(np.int64).astype(np.float64) / np.maximum(vol[1:], 1)
+        live = vol[1:] > 0
+        if periodic[a]:
+            assert ((got[live] >= 0) & (got[live] < dimv[a])).all(), (tag, k, got[live].min(), got[live].max())
+            diff = (got[live] - want[1:, a][live] + dimv[a] / 2.0) % dimv[a] - dimv[a] / 2.0
+        else:
+            diff = got[live] - want[1:, a][live]
+        assert np.abs(diff).max() < 1e-9, (tag, k, np.abs(diff).max())
+
+
+@pytest.mark.parametrize("dims,periodic,sub", [((32, 24), (1, 1, 0), 4), ((16, 16, 16), (1, 0, 1), 4)])
+def test_P16_periodic_centroids_follow_cells_through_the_border(oracle_mod, dims, periodic, sub):
+    """L297 / reading S23: with unwrap_centroids the tracked sums give, after every MCS, the centroid of the cell as a
+    connected object on the torus (computed here from the lattice by unwrapping around one of the cell's own sites),
+    kept inside [0, dim); cells are seeded ACROSS the periodic borders."""
+    nd = len(dims)
+    shape = tuple(reversed(dims))
+    ids = np.zeros(shape, dtype=np.uint32)
+    n = 0
+    if nd == 2:
+        for j in range(0, dims[1], 8):
+            for i in range(0, dims[0], 8):
+                n += 1
+                yy = (np.arange(j - 2, j + 3) % dims[1])[:, None]; xx = (np.arange(i - 2, i + 3) % dims[0])[None, :]
+                ids[yy, xx] = n                      # 5x5 squares centred on the corners of an 8-pitch grid: (0,0) wraps
+    else:
+        for k in range(0, dims[2], 8):
+            for j in range(0, dims[1], 8):
+                for i in range(0, dims[0], 8):
+                    n += 1
+                    zz = (np.arange(k - 2, k + 2) % dims[2])[:, None, None]
+                    yy = np.clip(np.arange(j + 1, j + 5), 0, dims[1] - 1)[None, :, None]
+                    xx = (np.arange(i - 2, i + 2) % dims[0])[None, None, :]
+                    ids[zz, yy, xx] = n
+    ct = np.ones(n + 1, dtype=np.uint8); ct[0] = 0
+    kw = dict(J=np.array([[0, 6], [6, 12]], dtype=np.int32), lambda_V=[0, 5], target_V=[0, 30 if nd == 2 else 70],
+              T=20.0, seed=4, subsection=sub, max_cells=n, periodic=periodic, unwrap_centroids=1)
+    o = oracle_mod.Oracle(dims, **kw)
+    o.set_lattice(ids, None, ct)
+    _check_tracked_centroids(o, n, dims, periodic, "initial")
+    for t in range(8):
+        o.step(1)
+        _check_tracked_centroids(o, n, dims, periodic, "MCS %d" % (t + 1))
+    # without the option the sums are the plain coordinate sums (P2)
+    kw["unwrap_centroids"] = 0
+    o2 = oracle_mod.Oracle(dims, **kw)
+    o2.set_lattice(ids, None, ct); o2.step(3)
+    rc = H.recount(o2.get_lattice(), n, nd, periodic)
+    st = o2.get_cell_stats()
+    for k, want in zip(("volume", "perimeter", "sum_x", "sum_y", "sum_z"), rc):
+        np.testing.assert_array_equal(st[k][1:].astype(np.int64), want[1:], err_msg=k)
+
+
+@pytest.mark.parametrize("sgn", [1, -1])
+def test_P16_a_cell_driven_across_the_border_keeps_a_continuous_track(oracle_mod, sgn):
+    """A lone cell pushed in +x by a uniform field on a periodic 32-wide lattice crosses the border: the tracked centroid
+    stays the torus centroid, moves by small steps (shortest image) and re-enters on the other side; the
+    persistence direction (Eq 6, shortest displacement through the border) ends up pointing along +x."""
+    dims, periodic = (32, 32), (1, 1, 0)
+    ids = np.zeros((32, 32), dtype=np.uint32)
+    if sgn > 0:
+        ids[12:20, 22:30] = 1
+    else:
+        ids[12:20, 2:10] = 1
+    o = oracle_mod.Oracle(dims, J=np.array([[0, 10], [10, 20]], dtype=np.int32), lambda_V=[0, 20], target_V=[0, 64],
+                          lambda_P=[0, 1], target_P=[0, 90], T=10.0, seed=3, subsection=8, max_cells=1, periodic=periodic,
+                          lambda_chem=[0, 60], lambda_pers=[0, 1], mu_pers=[0, 0.5], dt_pers=4, unwrap_centroids=1)
+    o.set_lattice(ids, None, np.array([0, 1], dtype=np.uint8))
+    f = np.zeros((32, 32, 2), dtype=np.float32); f[..., 0] = float(sgn)
+    o.set_chemotaxis_field(f)
+    prev = None; travelled = 0.0; wraps = 0
+
+    def cent():
+        st = o.get_cell_stats()
+        v = float(st["volume"][1])
+        return np.array([st["sum_x"][1] / v, st["sum_y"][1] / v, 0.0])
+    hist = [cent()]; p_prev = np.zeros(3); mu, dt = 0.5, 4
+    for t in range(150):
+        o.step(1)
+        _check_tracked_centroids(o, 1, dims, periodic, "MCS %d" % (t + 1))
+        # Eq 6-7 restated with the shortest displacement through the periodic border
+        hist.append(cent())
+        d = hist[-1] - hist[max(len(hist) - 1 - dt, 0)]
+        d[:2] = (d[:2] + 16.0) % 32.0 - 16.0
+        dn = np.linalg.norm(d)
+        pv = ((1 - mu) * d / dn if dn > 0 else 0.0) + mu * p_prev
+        pn = np.linalg.norm(pv)
+        p_prev = pv / pn if pn > 0 else np.zeros(3)
+        np.testing.assert_allclose(o.get_persistence()[1], p_prev, rtol=0, atol=1e-12, err_msg="MCS %d" % (t + 1))
+        p_prev = o.get_persistence()[1]
+        st = o.get_cell_stats()
+        c = float(st["sum_x"][1]) / float(st["volume"][1])
+        if prev is not None:
+            step = (c - prev + 16.0) % 32.0 - 16.0
+            assert abs(step) < 3.0, (t, prev, c)
+            travelled += step
+            wraps += int(sgn * (prev - c) > 16.0)
+        prev = c
+    assert sgn * travelled > 14.0 and wraps >= 1, (travelled, wraps)
+    assert sgn * o.get_persistence()[1][0] > 0.7

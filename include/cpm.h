@@ -72,6 +72,13 @@ typedef struct {
   const double  *mu_pers;         /* host [n_types], in [0,1]: directional memory mu of Eq 6 */
   int32_t  dt_pers;               /* look-back Delta t of Eq 6 in MCS; >= 1 when any lambda_pers != 0 */
   const int32_t *lambda_chem;     /* host [n_types], |.| <= 2^24: chemotaxis strength, Eq 4 */
+  /* Periodic centroid tracking (L297 "Composite variable tracking"; reading S23).  != 0: on periodic axes a
+   * site's coordinate enters its cell's sum as the periodic image nearest to the cell (its anchor = floor of the
+   * centroid at the last MCS boundary), and after every MCS the sum is shifted by dim x volume so that the centroid
+   * sum/volume (Eq 10) stays inside [0, dim): cells smaller than half the lattice keep a meaningful centroid when
+   * they straddle or cross a periodic border; Eq 6 then uses the shortest displacement through the border.
+   * 0: sums are the plain coordinate sums of the cell's sites. */
+  int32_t  unwrap_centroids;
 } cpm_params;
 
 /* Validate parameters, build the type tables, the Metropolis threshold table (Eq 2) and the

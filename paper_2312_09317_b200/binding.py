@@ -37,7 +37,7 @@ class _Params(C.Structure):
         ("device", C.c_int32), ("stream", C.c_void_p),
         ("flags", C.c_uint32),
         ("lambda_pers", C.POINTER(C.c_int32)), ("mu_pers", C.POINTER(C.c_double)), ("dt_pers", C.c_int32),
-        ("lambda_chem", C.POINTER(C.c_int32)),
+        ("lambda_chem", C.POINTER(C.c_int32)), ("unwrap_centroids", C.c_int32),
     ]
 
 
@@ -122,7 +122,7 @@ class CPM:
                  lambda_act=None, max_act=None, T=20.0, seed=1, subsection=0,
                  attempts_per_activation=0, mode=MODE_DETERMINISTIC, max_cells=0,
                  periodic=(0, 0, 0), device=None, stream=None, flags=0,
-                 lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None):
+                 lambda_pers=None, mu_pers=None, dt_pers=0, lambda_chem=None, unwrap_centroids=0):
         import torch  # device memory + streams only
         L = load_library()
         if not torch.cuda.is_available():
@@ -174,6 +174,7 @@ class CPM:
             keep.append(mu)
             p.mu_pers = mu.ctypes.data_as(C.POINTER(C.c_double))
         p.dt_pers = int(dt_pers)
+        p.unwrap_centroids = int(unwrap_centroids)
         h = C.c_void_p()
         rc = L.cpm_create(C.byref(p), C.byref(h))
         if rc != 0:

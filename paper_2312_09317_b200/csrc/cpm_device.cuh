@@ -87,6 +87,7 @@ struct SweepParams {
   const short4 *pq;                  // [max_cells + 1] persistence direction of the cell (null: persistence off)
   const short4 *chem;                // [N] chemotaxis field, row-major x fastest (null: no field loaded)
   int xq_len[3];                     // llround(16384 / sqrt(n)), n = 1, 2, 3: component of the unit copy direction
+  const int *anc;                    // [max_cells + 1][3] anchors of the periodic centroid tracking (reading S23); null: off
 };
 
 // ------------------------------------------------------------------ PTX wrappers ----------
@@ -155,6 +156,17 @@ __device__ __forceinline__ long long vec_bias(const SweepParams &P, int dx, int 
     acc += (long long)lc * (long long)(x0 * v.x + x1 * v.y + x2 * v.z);
   }
   return (acc + (1ll << 27)) >> 28;
+}
+
+// Reading S23 (L297): on a periodic axis a site's coordinate enters a cell's sum as the image nearest to the cell's anchor
+__device__ __forceinline__ int image_near(int x, int anchor, int dim) {
+  const int r = x - anchor;
+  return (2 * r >= dim) ? x - dim : (2 * r < -dim) ? x + dim : x;
+}
+// coordinate of axis a (0..2) of a site as it enters the sums of `cell`
+__device__ __forceinline__ int sum_coord(const SweepParams &P, uint32_t cell, int a, int x) {
+  if (P.anc == nullptr || !P.per[a]) return x;
+  return image_near(x, __ldg(P.anc + 3 * (size_t)cell + a), a == 0 ? P.X : a == 1 ? P.Y : P.Z);
 }
 
 // neighbour index (0..nNb-1, centre skipped) -> (dx,dy,dz); order: (dz,dy,dx) lexicographic, dx fastest
@@ -386,8 +398,8 @@ struct Sweep {
     __syncwarp();
     dirty = true;
     const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
-    if (A != 0) add_delta(A, entA, 1, dPA, gx, gy, gz, +1);
-    if (B != 0) add_delta(B, entB, -1, dPB, gx, gy, gz, -1);
+    if (A != 0) add_delta(A, entA, 1, dPA, sum_coord(P, A, 0, gx), sum_coord(P, A, 1, gy), sum_coord(P, A, 2, gz), +1);
+    if (B != 0) add_delta(B, entB, -1, dPB, sum_coord(P, B, 0, gx), sum_coord(P, B, 1, gy), sum_coord(P, B, 2, gz), -1);
     return true;
   }
 
@@ -675,6 +687,45 @@ __global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr,
 }
 __global__ void mcs_increment_kernel(uint32_t *mcs_ptr, uint32_t *pers_n) { *mcs_ptr += 1; if (pers_n) *pers_n += 1; }
 
+// ---- periodic centroid tracking (L297, reading S23) ----
+// set_lattice: the first site of every cell in scan order (lowest linear index) ...
+__global__ void anchor_first_site_kernel(const uint32_t *ids, long long N, uint32_t max_cells, unsigned long long *first) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    const uint32_t id = ids[i];
+    if (id != 0 && id <= max_cells) atomicMin(first + id, (unsigned long long)i);
+  }
+}
+// ... becomes its anchor
+__global__ void anchor_from_first_kernel(long long ncell, const unsigned long long *first, int X, int Y, int *anc) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell >= ncell) return;
+  const unsigned long long f = first[cell];
+  const bool have = cell != 0 && f != ~0ull;
+  anc[3 * cell] = have ? (int)(f % (unsigned)X) : 0;
+  anc[3 * cell + 1] = have ? (int)((f / (unsigned)X) % (unsigned)Y) : 0;
+  anc[3 * cell + 2] = have ? (int)(f / ((unsigned long long)X * (unsigned)Y)) : 0;
+}
+// after the recount and after every MCS: centroid back into [0, dim) on periodic axes, the anchor follows the centroid
+__global__ void centroid_normalise_kernel(long long ncell, const unsigned long long *liveVP, unsigned long long *sumx,
+                                          unsigned long long *sumy, unsigned long long *sumz, int *anc, int X, int Y, int Z,
+                                          int perx, int pery, int perz) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell < 1 || cell >= ncell) return;
+  const long long v = (long long)(uint32_t)(liveVP[cell] >> 32);
+  if (v <= 0) return;
+  unsigned long long *S[3] = {sumx, sumy, sumz};
+  const int dimv[3] = {X, Y, Z}, per[3] = {perx, pery, perz};
+  for (int a = 0; a < 3; ++a) {
+    if (!per[a]) continue;
+    const long long span = (long long)dimv[a] * v;
+    long long s = (long long)S[a][cell] % span;
+    if (s < 0) s += span;
+    S[a][cell] = (unsigned long long)s;
+    anc[3 * cell + a] = (int)(s / v);
+  }
+}
+
 // ---- persistence (Eq 5-7, reading S22) ----
 // Q14 of a direction: what the sweep reads
 __device__ __forceinline__ short4 quantise_q14(double x, double y, double z) {
@@ -705,7 +756,8 @@ __global__ void persistence_init_kernel(long long ncell, int slots, const unsign
 // Every step is one IEEE double operation (no fused multiply-add), so the result is the same on any conforming machine.
 __global__ void persistence_update_kernel(long long ncell, int slots, const unsigned long long *liveVP, const unsigned long long *sumx,
                                           const unsigned long long *sumy, const unsigned long long *sumz, const uint8_t *ctype,
-                                          const double *mu_of_type, double *phat, short4 *pq, double *ring, const uint32_t *pers_n) {
+                                          const double *mu_of_type, double *phat, short4 *pq, double *ring, const uint32_t *pers_n,
+                                          int wrapx, int wrapy, int wrapz) {
   const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (cell < 1 || cell >= ncell) return;
   const unsigned long long vp = liveVP[cell];
@@ -717,7 +769,15 @@ __global__ void persistence_update_kernel(long long ncell, int slots, const unsi
   centroid_of(vp, sumx[cell], sumy[cell], sumz[cell], X);
   const double mu = mu_of_type[ctype[cell]];
   const double one_minus_mu = __dsub_rn(1.0, mu);
-  for (int a = 0; a < 3; ++a) d[a] = __dsub_rn(X[a], old_slot[3 * cell + a]);
+  const int wrap[3] = {wrapx, wrapy, wrapz};   // dim of the axes whose centroids are tracked through the periodic border, else 0
+  for (int a = 0; a < 3; ++a) {
+    d[a] = __dsub_rn(X[a], old_slot[3 * cell + a]);
+    if (wrap[a] != 0) {   // shortest displacement through the border (reading S23)
+      const double half = __dmul_rn(0.5, (double)wrap[a]);
+      if (d[a] > half) d[a] = __dsub_rn(d[a], (double)wrap[a]);
+      else if (d[a] < -half) d[a] = __dadd_rn(d[a], (double)wrap[a]);
+    }
+  }
   const double dn = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2])));
   for (int a = 0; a < 3; ++a) {
     const double keep = __dmul_rn(mu, phat[3 * cell + a]);
@@ -810,7 +870,7 @@ __global__ void act_get_kernel(const uint8_t *act, long long apitch, int X, int 
 template <int DIM>
 __global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int Y, int Z, int perx, int pery, int perz,
                                unsigned long long *liveVP, unsigned long long *sumx, unsigned long long *sumy,
-                               unsigned long long *sumz) {
+                               unsigned long long *sumz, const int *anc) {
   const long long N = (long long)X * Y * Z;
   const long long stride = (long long)gridDim.x * blockDim.x;
   const int per[3] = {perx, pery, perz};
@@ -845,6 +905,11 @@ __global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int 
         }
       }
     }
+    if (anc != nullptr && me != 0) {   // reading S23: the image of the site nearest to the cell's anchor
+      if (perx) x = image_near(x, anc[3 * (size_t)me], X);
+      if (pery) y = image_near(y, anc[3 * (size_t)me + 1], Y);
+      if (perz) z = image_near(z, anc[3 * (size_t)me + 2], Z);
+    }
     const unsigned peers = __match_any_sync(FULL, me);
     const unsigned cnt = __popc(peers);
     const unsigned f = __reduce_add_sync(peers, (unsigned)foreign);
@@ -853,9 +918,9 @@ __global__ void recount_kernel(const uint32_t *lat, long long pitch, int X, int 
     const unsigned sz = (DIM == 3) ? __reduce_add_sync(peers, (unsigned)z) : 0u;
     if (me != 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) {
       atomicAdd(liveVP + me, ((unsigned long long)cnt << 32) + (unsigned long long)f);
-      atomicAdd(sumx + me, (unsigned long long)sx);
-      atomicAdd(sumy + me, (unsigned long long)sy);
-      if (DIM == 3) atomicAdd(sumz + me, (unsigned long long)sz);
+      atomicAdd(sumx + me, (unsigned long long)(long long)(int)sx);   // images may be negative
+      atomicAdd(sumy + me, (unsigned long long)(long long)(int)sy);
+      if (DIM == 3) atomicAdd(sumz + me, (unsigned long long)(long long)(int)sz);
     }
   }
 }

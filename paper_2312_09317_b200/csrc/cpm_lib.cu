@@ -72,6 +72,9 @@ struct cpm_ctx {
   short4 *pq = nullptr, *chem = nullptr;
   uint8_t *ctype_dev = nullptr;
   uint32_t *pers_n = nullptr;
+  bool unwrap = false;                       // periodic centroid tracking (reading S23)
+  int *anc = nullptr;
+  unsigned long long *first_site = nullptr;
   // staging buffers for host-pointer I/O, kept between calls
   void *stage_a = nullptr, *stage_b = nullptr, *stage_c = nullptr;
   size_t stage_a_cap = 0, stage_b_cap = 0, stage_c_cap = 0;
@@ -252,7 +255,7 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
   cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
   cudaFree(c->vec_types_dev); cudaFree(c->mu_dev); cudaFree(c->phat); cudaFree(c->ring); cudaFree(c->pq); cudaFree(c->chem);
-  cudaFree(c->ctype_dev); cudaFree(c->pers_n);
+  cudaFree(c->ctype_dev); cudaFree(c->pers_n); cudaFree(c->anc); cudaFree(c->first_site);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -293,10 +296,19 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       // deterministic mode: the next phase-step reads the values as of its own start
       if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, st));
     }
+  if (c->unwrap) {   // L297: centroids back inside the lattice on periodic axes, anchors follow
+    const long long ncl = (long long)ncell;
+    centroid_normalise_kernel<<<(unsigned)((ncl + 255) / 256), 256, 0, st>>>(ncl, c->liveVP, c->sumx, c->sumy, c->sumz, c->anc, c->dim[0],
+                                                                           c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
+    c->launches++;
+  }
   if (c->pers_on) {   // Eq 6-7: every cell's persistence direction from its centroid now and dt MCS ago
     const long long ncl = (long long)ncell;
     persistence_update_kernel<<<(unsigned)((ncl + 255) / 256), 256, 0, st>>>(ncl, c->dt_pers + 1, c->liveVP, c->sumx, c->sumy, c->sumz,
-                                                                           c->ctype_dev, c->mu_dev, c->phat, c->pq, c->ring, c->pers_n);
+                                                                           c->ctype_dev, c->mu_dev, c->phat, c->pq, c->ring, c->pers_n,
+                                                                           (c->unwrap && c->per[0]) ? c->dim[0] : 0,
+                                                                           (c->unwrap && c->per[1]) ? c->dim[1] : 0,
+                                                                           (c->unwrap && c->per[2]) ? c->dim[2] : 0);
     c->launches++;
   }
   if (c->act_enabled) {
@@ -413,6 +425,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->nNb = (d == 2) ? 8 : 26;
   c->act_enabled = any_act;
   c->pers_on = pers_on; c->chem_on = chem_on; c->dt_pers = p->dt_pers;
+  c->unwrap = p->unwrap_centroids != 0 && (c->per[0] || c->per[1] || c->per[2]);
   c->use_graph = !(p->flags & CPM_FLAG_NO_GRAPH);
   c->nsets = (sites <= 512) ? 1 : 4;
   // TMA wants the tile's first word at a 16-byte boundary: x0-4 with x0 a multiple of S
@@ -554,6 +567,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     alloc((void **)&c->pers_n, 4);
   }
   if (chem_on) alloc((void **)&c->chem, (size_t)c->N * sizeof(short4));
+  if (c->unwrap) { alloc((void **)&c->anc, ncell * 3 * sizeof(int)); alloc((void **)&c->first_site, ncell * 8); }
   if (rc == CPM_OK && c->vec_types_dev) {
     cudaError_t e = cudaMemcpyAsync(c->vec_types_dev, vtypes.data(), vtypes.size() * sizeof(int2), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess && c->mu_dev) e = cudaMemcpyAsync(c->mu_dev, mus.data(), nT * sizeof(double), cudaMemcpyHostToDevice, c->stream);
@@ -589,6 +603,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   sp.counters = c->counters; sp.error_flag = c->error_flag;
   sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
   sp.vec_on = (pers_on || chem_on) ? 1 : 0; sp.vec_types = c->vec_types_dev; sp.pq = c->pq; sp.chem = c->chem;
+  sp.anc = c->anc;
   for (int n2 = 1; n2 <= 3; ++n2) sp.xq_len[n2 - 1] = (int)std::llround(16384.0 / std::sqrt((double)n2));
 
   memset(&c->tm_lat, 0, sizeof(CUtensorMap));
@@ -643,6 +658,12 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
   CK(cudaMemsetAsync(c->sumx, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumy, 0, ncell * 8, c->stream));
   CK(cudaMemsetAsync(c->sumz, 0, ncell * 8, c->stream));
+  if (c->unwrap) {   // reading S23: the first site of a cell in scan order anchors the images of its other sites
+    CK(cudaMemsetAsync(c->first_site, 0xff, ncell * 8, c->stream));
+    anchor_first_site_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(sid, c->N, c->max_cells, c->first_site);
+    anchor_from_first_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, c->first_site, c->dim[0], c->dim[1], c->anc);
+    c->launches += 2;
+  }
   if (c->pooled) {
     const TileLayout &tl = c->sp.tl;
     for (int col = 0; col < (1 << c->d); ++col) {
@@ -660,9 +681,11 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
       if (c->n_act_col[col] == 0) continue;
       const long long thr = (long long)c->n_act_col[col];
       if (c->d == 2)
-        tile_recount_kernel<2><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz);
+        tile_recount_kernel<2><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+                                                                         c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
       else
-        tile_recount_kernel<3><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz);
+        tile_recount_kernel<3><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+                                                                         c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
       c->launches++;
     }
   } else {
@@ -671,13 +694,18 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
     c->launches++;
     if (c->d == 2)
       recount_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
-                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz, c->anc);
     else
       recount_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], c->per[0],
-                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz);
+                                                                c->per[1], c->per[2], c->liveVP, c->sumx, c->sumy, c->sumz, c->anc);
     c->launches++;
   }
   if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, c->stream));
+  if (c->unwrap) {
+    centroid_normalise_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, c->liveVP, c->sumx, c->sumy, c->sumz, c->anc,
+                                                                                   c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
+    c->launches++;
+  }
   if (c->pers_on) {   // reading S22: p^ = 0, the look-back window starts at the present centroids
     CK(cudaMemcpyAsync(c->ctype_dev, sct, ncell, cudaMemcpyDeviceToDevice, c->stream));
     persistence_init_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, c->stream>>>((long long)ncell, c->dt_pers + 1, c->liveVP, c->sumx, c->sumy,

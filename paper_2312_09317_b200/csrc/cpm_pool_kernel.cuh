@@ -491,7 +491,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
               const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
               unsigned long long *const arr = which == 0 ? P.liveVP : which == 1 ? P.sumx : which == 2 ? P.sumy : P.sumz;
               const unsigned long long v = which == 0 ? ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP
-                                                      : (unsigned long long)(long long)(sgn * (which == 1 ? gx : which == 2 ? gy : gz));
+                                                      : (unsigned long long)(long long)(sgn * sum_coord(P, cell, which - 1, which == 1 ? gx : which == 2 ? gy : gz));
               atomicAdd(arr + cell, v);
             }
           }
@@ -634,7 +634,8 @@ __global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *
 // per array.
 template <int DIM>
 __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_active, unsigned long long *liveVP,
-                                    unsigned long long *sumx, unsigned long long *sumy, unsigned long long *sumz) {
+                                    unsigned long long *sumx, unsigned long long *sumy, unsigned long long *sumz,
+                                    const int *anc, int X, int Y, int Z, int perx, int pery, int perz) {
   const int S = L.S, T = S + 2, TW = L.TW;
   constexpr int NNB = (DIM == 2) ? 8 : 26;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
@@ -668,7 +669,13 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
             foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_GC] & ID_MASK) != me);
           }
           cv += (1ull << 32) + (unsigned long long)foreign;
-          cx += (unsigned long long)(ox + lx); cy += (unsigned long long)(oy + ly); cz += (unsigned long long)(oz + lz);
+          int qx = ox + lx, qy = oy + ly, qz = oz + lz;
+          if (anc != nullptr) {   // reading S23: the image of the site nearest to the cell's anchor
+            if (perx) qx = image_near(qx, anc[3 * (size_t)me], X);
+            if (pery) qy = image_near(qy, anc[3 * (size_t)me + 1], Y);
+            if (perz) qz = image_near(qz, anc[3 * (size_t)me + 2], Z);
+          }
+          cx += (unsigned long long)(long long)qx; cy += (unsigned long long)(long long)qy; cz += (unsigned long long)(long long)qz;
         }
     flush();
   }

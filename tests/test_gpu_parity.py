@@ -311,6 +311,36 @@ def test_chemotaxis_3d_with_act_and_persistence_together(pk, oracle_mod):
         g.set_chemotaxis_field(np.full((40, 40, 40, 3), np.nan, dtype=np.float32))
 
 
+@pytest.mark.parametrize("name,dims,over", [
+    ("C6", (32, 32, 32), {"periodic": (1, 1, 1)}),                       # pooled 3D + persistence through the border
+    ("C6", (32, 32, 32), {"periodic": (1, 0, 1), "subsection": 8}),      # warp kernel
+    ("C7", (128, 128), {"periodic": (1, 1, 0)}),                         # pooled 2D + chemotaxis
+    ("C5", (64, 96), {"periodic": (0, 1, 0), "subsection": 4}),
+    ("C3", (32, 32, 32), {"periodic": (1, 1, 1), "subsection": 4, "mode": 0}),
+])
+def test_periodic_centroid_tracking_bit_exact(pk, oracle_mod, name, dims, over):
+    """L297 / reading S23 (unwrap_centroids): sums, anchors' effect on the sums, centroids inside the lattice and, for C6, the
+    persistence directions built from shortest displacements -- all equal to the oracle's after every MCS; the
+    lattice itself is the same as without the option (the sums do not feed back into dH)."""
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims)
+    cfg["ids"] = np.roll(cfg["ids"], shift=3, axis=-1)    # seeds straddle the x border
+    cfg["ids"] = np.roll(cfg["ids"], shift=2, axis=0)     # ... and the last axis' border
+    if cfg.get("frozen") is not None:
+        cfg["frozen"] = np.roll(np.roll(cfg["frozen"], 3, -1), 2, 0)
+    g, o = _run(pk, oracle_mod, cfg, 10, 1, act=(name == "C3"), unwrap_centroids=1, **over)
+    st = g.get_cell_stats()
+    v = np.maximum(st["volume"][1:].astype(np.float64), 1)
+    for a, k in enumerate(("sum_x", "sum_y", "sum_z")[:len(dims)]):
+        if over["periodic"][a]:
+            c = st[k][1:].astype(np.int64) / v
+            assert ((c >= 0) & (c < dims[a]))[st["volume"][1:] > 0].all(), k
+    if name != "C6":   # without persistence the option cannot change the trajectory
+        g0, _ = _pair(pk, oracle_mod, cfg, **over)
+        g0.step(10)
+        np.testing.assert_array_equal(g0.get_lattice(), g.get_lattice())
+
+
 def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     """Inputs/outputs as device tensors (on_device=1); and the non-TMA staging path."""
     import torch

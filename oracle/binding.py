@@ -85,6 +85,8 @@ def lib():
         L.oracle_get_persistence.argtypes = [vp, vp]
         L.oracle_probe_dir.argtypes = [vp, C.c_uint64, C.c_int32, vp]
         L.oracle_direction_table.argtypes = [C.c_int32, vp]
+        L.oracle_get_interface_counts.argtypes = [vp, vp]
+        L.oracle_update_statistics.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32]
         _lib = L
     return _lib
 
@@ -247,6 +249,18 @@ class Oracle:
         v = C.c_int64()
         self._chk(self._L.oracle_probe_dir(self._h, int(t_index), int(nb), C.addressof(v)))
         return v.value
+
+    # ---- instrumentation ----
+    def get_interface_counts(self):
+        out = np.zeros((self.n_types, self.n_types), dtype=np.uint64)
+        self._chk(self._L.oracle_get_interface_counts(self._h, out.ctypes.data))
+        return out
+
+    def update_statistics(self, n_mcs, n_freq=8, n_wait=64, wait_bin=1):
+        freq = np.zeros(n_freq, dtype=np.uint64); wait = np.zeros(n_wait, dtype=np.uint64)
+        self._chk(self._L.oracle_update_statistics(self._h, int(n_mcs), freq.ctypes.data, n_freq, wait.ctypes.data, n_wait,
+                                                   int(wait_bin)))
+        return freq, wait
 
     # ---- hooks for the pins ----
     def set_visit_order(self, order, seed=0):

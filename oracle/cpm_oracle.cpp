@@ -844,6 +844,91 @@ int oracle_direction_table(int32_t ndim, int64_t *out) {
   return n;
 }
 
+/* ---- instrumentation: sorting observables and update statistics ---- */
+
+/* Number of unordered Moore pairs {i, j} of lattice positions held by DIFFERENT cells, by the types of the two cells
+ * (the interfaces Eq 1 sums J over; homotypic = diagonal, heterotypic = off-diagonal: the sorting observable of
+ * Fig 4, L69).  A position outside a closed lattice is medium (reading S5), so a cell site on the border forms a
+ * (type, 0) pair with each of its outside neighbours.  out[a*nT + b] == out[b*nT + a]. */
+int oracle_get_interface_counts(oracle_ctx *c, uint64_t *out) {
+  if (!c || !out) return ORACLE_ERR_ARG;
+  const int nT = c->nT;
+  std::vector<uint64_t> cnt((size_t)nT * nT, 0);
+  for (int z = 0; z < c->dim[2]; ++z)
+    for (int y = 0; y < c->dim[1]; ++y)
+      for (int x = 0; x < c->dim[0]; ++x) {
+        SiteView me = view(c, x, y, z);
+        for (int q = 0; q < c->nNb; ++q) {
+          SiteView nb = view(c, x + c->off[q][0], y + c->off[q][1], z + c->off[q][2]);
+          if (nb.id == me.id) continue;
+          /* an inside pair is met from both ends: count it from the end whose offset comes first (q < nNb/2 means the
+           * neighbour precedes in scan order); a pair with an outside position is met once */
+          if (nb.inside && q < c->nNb / 2) continue;
+          cnt[(size_t)me.tau * nT + nb.tau] += 1;
+          if (me.tau != nb.tau) cnt[(size_t)nb.tau * nT + me.tau] += 1;
+        }
+      }
+  std::copy(cnt.begin(), cnt.end(), out);
+  return ORACLE_OK;
+}
+
+/* Update statistics of the schedule (Fig 3, L65-79): which positions the copy attempts of the next n_mcs MCS pick as
+ * targets, without touching the lattice.  All active subsections advance in lock-step (the paper puts a barrier
+ * after every update, L75), so attempt a of the e-th non-empty phase-step of the m-th MCS happens at tick
+ * (m * E + e) * k + a, E = non-empty phase-steps per MCS.
+ *   freq[j]: (position, MCS) pairs in which the position was picked exactly j times in that MCS (last bin: >= n_freq-1);
+ *   wait[j]: consecutive picks of the same position whose ticks differ by dt with (dt-1)/bin == j (last bin: beyond). */
+int oracle_update_statistics(oracle_ctx *c, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
+                             uint32_t bin) {
+  if (!c || !freq || !wait || n_freq < 1 || n_wait < 1 || bin < 1) return ORACLE_ERR_ARG;
+  const size_t N = c->id.size();
+  std::vector<uint64_t> last(N, 0);       /* tick + 1 of the last pick; 0 = never */
+  std::vector<uint32_t> cnt(N, 0);
+  std::fill(freq, freq + n_freq, 0); std::fill(wait, wait + n_wait, 0);
+  const int ncol = 1 << c->d;
+  const int64_t nsub_total = (int64_t)c->nsub[0] * c->nsub[1] * c->nsub[2];
+  const uint32_t key[2] = {(uint32_t)c->seed, (uint32_t)(c->seed >> 32)};
+  std::vector<int> occurs(ncol, 0);
+  for (int64_t b = 0; b < nsub_total; ++b) {
+    int bx = (int)(b % c->nsub[0]), by = (int)((b / c->nsub[0]) % c->nsub[1]), bz = (int)(b / ((int64_t)c->nsub[0] * c->nsub[1]));
+    occurs[(bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2)] = 1;
+  }
+  int E_per_rep = 0;
+  for (int col = 0; col < ncol; ++col) E_per_rep += occurs[col];
+  const uint64_t E = (uint64_t)E_per_rep * (uint64_t)c->R;
+  for (uint32_t m = 0; m < n_mcs; ++m) {
+    uint64_t e = 0;
+    for (int64_t rep = 0; rep < c->R; ++rep)
+      for (int col = 0; col < ncol; ++col) {
+        if (!occurs[col]) continue;
+        const uint32_t p = (uint32_t)(rep * ncol + col);
+        for (int64_t b = 0; b < nsub_total; ++b) {
+          int bx = (int)(b % c->nsub[0]), by = (int)((b / c->nsub[0]) % c->nsub[1]), bz = (int)(b / ((int64_t)c->nsub[0] * c->nsub[1]));
+          if (((bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2)) != col) continue;
+          uint32_t w4[4] = {0, 0, 0, 0};
+          for (int64_t a = 0; a < c->k; ++a) {
+            if ((a & 3) == 0) { uint32_t ctr[4] = {(uint32_t)(a >> 2), (uint32_t)b, 2 * p + 0, c->mcs + m}; philox(ctr, key, w4); }
+            uint32_t l, nb;
+            decode_proposal(w4[a & 3], (uint32_t)c->sites, (uint32_t)c->nNb, &l, &nb);
+            const int S = c->S;
+            const int tx = bx * S + (int)(l % S), ty = by * S + (int)((l / S) % S), tz = (c->d == 3) ? bz * S + (int)(l / (S * S)) : 0;
+            const size_t i = (size_t)lin(c, tx, ty, tz);
+            const uint64_t tick = ((uint64_t)m * E + e) * (uint64_t)c->k + (uint64_t)a;
+            if (last[i] != 0) {
+              const uint64_t dt = tick + 1 - last[i];
+              wait[std::min<uint64_t>((dt - 1) / bin, (uint64_t)n_wait - 1)] += 1;
+            }
+            last[i] = tick + 1;
+            cnt[i] += 1;
+          }
+        }
+        ++e;
+      }
+    for (size_t i = 0; i < N; ++i) { freq[std::min<uint32_t>(cnt[i], (uint32_t)n_freq - 1)] += 1; cnt[i] = 0; }
+  }
+  return ORACLE_OK;
+}
+
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox(ctr, key, out); }
 
 void oracle_decode_proposal(uint32_t w, uint32_t sites, uint32_t n_nb, uint32_t *l, uint32_t *nb) {

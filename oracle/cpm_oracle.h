@@ -87,6 +87,12 @@ int  oracle_get_persistence(oracle_ctx *c, double *p);
 int  oracle_probe_dir(oracle_ctx *c, uint64_t t_index, int32_t nb, int64_t *dH_dir);
 /* Q14 unit vectors of the copy direction (source -> target) per neighbour index: out[nb*3 + {0,1,2}] */
 int  oracle_direction_table(int32_t ndim, int64_t *out);
+/* ---- instrumentation ---- */
+/* out[n_types*n_types]: unordered Moore pairs of positions held by different cells, by the two cells' types (symmetric) */
+int  oracle_get_interface_counts(oracle_ctx *c, uint64_t *out);
+/* target-pick statistics of the next n_mcs MCS of the schedule (lattice untouched): see cpm_oracle.cpp */
+int  oracle_update_statistics(oracle_ctx *c, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
+                              uint32_t bin);
 void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 /* proposal decode of one 32-bit word: local site index l in [0,S^d) and neighbour index nb */
 void oracle_decode_proposal(uint32_t w, uint32_t sites, uint32_t n_nb, uint32_t *l, uint32_t *nb);

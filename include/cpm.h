@@ -127,6 +127,19 @@ int  cpm_get_cell_stats(cpm_ctx *ctx, uint32_t *volume, uint32_t *perimeter,
 /* out (host) = {attempts, evaluated, accepted, mcs}. */
 int  cpm_get_counters(cpm_ctx *ctx, uint64_t out[4]);
 int  cpm_get_schedule(cpm_ctx *ctx, int32_t *S, int32_t *k, int32_t *phase_steps_per_mcs);
+/* ---- instrumentation (Fig 3, Fig 4; not on the sweep's hot path) ----
+ * Sorting observable (L69, Fig 4): out (host) [n_types*n_types], out[a*n_types+b] == out[b*n_types+a] = number of unordered
+ * Moore pairs of lattice positions held by DIFFERENT cells whose types are a and b -- the interfaces Eq 1 sums J over
+ * (diagonal: homotypic, off-diagonal: heterotypic).  A position outside a closed lattice counts as medium. */
+int  cpm_get_interface_counts(cpm_ctx *ctx, uint64_t *out);
+/* Update statistics of the schedule (L65-79, Fig 3): which positions the copy attempts of the NEXT n_mcs MCS pick as
+ * targets; the lattice and the MCS counter are not touched.  Active subsections advance in lock-step (L75), so attempt a of
+ * the e-th non-empty phase-step of the m-th MCS happens at tick (m E + e) k + a, E = non-empty phase-steps per MCS.
+ *   freq (host) [n_freq]: (position, MCS) pairs in which the position was picked exactly j times (last bin: >= n_freq-1);
+ *   wait (host) [n_wait]: consecutive picks of one position whose ticks differ by dt, binned (dt-1)/wait_bin (last bin: beyond).
+ * Needs n_mcs * 2^d * S^d < 2^32 and n_freq + n_wait <= 4096 (CPM_ERR_ARG); allocates 8 bytes per site while it runs. */
+int  cpm_update_statistics(cpm_ctx *ctx, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
+                           uint32_t wait_bin);
 /* Introspection for tests: host copy of the Metropolis table, thr[h] = floor(exp(-h/T) 2^32),
  * h = 1..Hmax; returns Hmax (>= 0) or a negative error; fills at most cap entries (thr[0] unused). */
 int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);

@@ -83,6 +83,8 @@ def load_library():
     L.cpm_get_cell_stats.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
     L.cpm_get_counters.argtypes = [vp, vp]
     L.cpm_get_schedule.argtypes = [vp, vp, vp, vp]
+    L.cpm_get_interface_counts.argtypes = [vp, vp]
+    L.cpm_update_statistics.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32]
     L.cpm_get_threshold_table.argtypes = [vp, vp, C.c_uint64]
     L.cpm_get_threshold_table.restype = C.c_int64
     L.cpm_get_launch_info.argtypes = [vp, vp]
@@ -263,6 +265,17 @@ class CPM:
         S = C.c_int32(); k = C.c_int32(); n = C.c_int32()
         self._chk(self._L.cpm_get_schedule(self._h, C.addressof(S), C.addressof(k), C.addressof(n)))
         return {"S": S.value, "k": k.value, "phase_steps_per_mcs": n.value}
+
+    def get_interface_counts(self):
+        out = np.zeros((self.n_types, self.n_types), dtype=np.uint64)
+        self._chk(self._L.cpm_get_interface_counts(self._h, out.ctypes.data))
+        return out
+
+    def update_statistics(self, n_mcs, n_freq=8, n_wait=64, wait_bin=1):
+        freq = np.zeros(n_freq, dtype=np.uint64); wait = np.zeros(n_wait, dtype=np.uint64)
+        self._chk(self._L.cpm_update_statistics(self._h, int(n_mcs), freq.ctypes.data, n_freq, wait.ctypes.data, n_wait,
+                                                int(wait_bin)))
+        return freq, wait
 
     def get_threshold_table(self):
         hmax = self._L.cpm_get_threshold_table(self._h, None, 0)

@@ -6,7 +6,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "csrc", "cpm_lib.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "cpm_device.cuh"), os.path.join(HERE, "csrc", "cpm_pool_kernel.cuh"), os.path.join(os.path.dirname(HERE), "include", "cpm.h")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "cpm_device.cuh"), os.path.join(HERE, "csrc", "cpm_pool_kernel.cuh"), os.path.join(HERE, "csrc", "cpm_stats_kernels.cuh"), os.path.join(os.path.dirname(HERE), "include", "cpm.h")]
 LIB = os.path.join(HERE, "libcpm_b200.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -5,6 +5,7 @@
 #include "../../include/cpm.h"
 #include "cpm_device.cuh"
 #include "cpm_pool_kernel.cuh"
+#include "cpm_stats_kernels.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -889,6 +890,68 @@ int cpm_get_schedule(cpm_ctx *c, int32_t *S, int32_t *k, int32_t *steps) {
   if (S) *S = c->S;
   if (k) *k = c->k;
   if (steps) *steps = (1 << c->d) * c->R;
+  return CPM_OK;
+}
+
+int cpm_get_interface_counts(cpm_ctx *c, uint64_t *out) {
+  if (!c || !out) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CK(cudaSetDevice(c->device));
+  const size_t n = (size_t)c->nT * c->nT;
+  unsigned long long *d = nullptr;
+  CK(stage_reserve(&c->stage_c, &c->stage_c_cap, n * 8));
+  d = reinterpret_cast<unsigned long long *>(c->stage_c);
+  CK(cudaMemsetAsync(d, 0, n * 8, c->stream));
+  LatView V{};
+  V.lat = c->lat; V.pitch = c->sp.pitch; V.tl = c->sp.tl; V.pooled = c->pooled ? 1 : 0;
+  V.X = c->dim[0]; V.Y = c->dim[1]; V.Z = c->dim[2];
+  for (int a = 0; a < 3; ++a) V.per[a] = c->per[a];
+  if (c->d == 2) interface_count_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(V, c->nT, d);
+  else interface_count_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(V, c->nT, d);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, d, n * 8, cudaMemcpyDeviceToHost, c->stream));
+  return check_device_flag(c);
+}
+
+int cpm_update_statistics(cpm_ctx *c, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait, uint32_t wait_bin) {
+  if (!c || !freq || !wait) return fail(c, CPM_ERR_ARG, "null argument");
+  if (n_freq < 1 || n_wait < 1 || wait_bin < 1 || n_freq + n_wait > 4096) return fail(c, CPM_ERR_ARG, "histogram sizes");
+  const unsigned long long ticks = (unsigned long long)n_mcs * (unsigned long long)(1 << c->d) * (unsigned long long)c->sites;
+  if (ticks >= (1ull << 32)) return fail(c, CPM_ERR_ARG, "n_mcs * 2^d * S^d must stay below 2^32");
+  CK(cudaSetDevice(c->device));
+  StatParams P{};
+  P.S = c->S; P.sites = c->sites; P.k = c->k; P.R = c->R; P.nNb = c->nNb;
+  for (int a = 0; a < 3; ++a) P.nsub[a] = c->nsub[a];
+  P.X = c->dim[0]; P.Y = c->dim[1];
+  int rank = 0;
+  for (int col = 0; col < 8; ++col) P.rank[col] = (col < (1 << c->d) && c->n_act_col[col] > 0) ? rank++ : -1;
+  P.E_per_rep = rank;
+  P.mcs0 = c->mcs_host; P.n_mcs = n_mcs; P.key0 = (uint32_t)c->seed; P.key1 = (uint32_t)(c->seed >> 32); P.bin = wait_bin;
+  P.n_freq = n_freq; P.n_wait = n_wait;
+  const long long nsub_total = (long long)c->nsub[0] * c->nsub[1] * c->nsub[2];
+  const size_t nh = (size_t)n_freq + (size_t)n_wait;
+  uint32_t *scratch = nullptr;
+  unsigned long long *hist = nullptr;
+  cudaError_t e = cudaMalloc(&scratch, (size_t)c->N * 8);
+  if (e == cudaSuccess) e = cudaMalloc(&hist, nh * 8);
+  if (e != cudaSuccess) { cudaFree(scratch); cudaFree(hist); return fail(c, CPM_ERR_OOM, cudaGetErrorString(e)); }
+  std::vector<unsigned long long> h(nh);
+  e = cudaMemsetAsync(scratch, 0, (size_t)c->N * 8, c->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(hist, 0, nh * 8, c->stream);
+  if (e == cudaSuccess) {
+    const unsigned blocks = (unsigned)((nsub_total + 127) / 128);
+    if (c->d == 2) update_stats_kernel<2><<<blocks, 128, nh * 8, c->stream>>>(P, nsub_total, scratch, scratch + c->N, hist);
+    else update_stats_kernel<3><<<blocks, 128, nh * 8, c->stream>>>(P, nsub_total, scratch, scratch + c->N, hist);
+    c->launches++;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), hist, nh * 8, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(scratch); cudaFree(hist);
+  if (e != cudaSuccess) return fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
+  for (int i = 0; i < n_freq; ++i) freq[i] = h[(size_t)i];
+  for (int i = 0; i < n_wait; ++i) wait[i] = h[(size_t)n_freq + i];
   return CPM_OK;
 }
 

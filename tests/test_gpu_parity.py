@@ -341,6 +341,39 @@ def test_periodic_centroid_tracking_bit_exact(pk, oracle_mod, name, dims, over):
         np.testing.assert_array_equal(g0.get_lattice(), g.get_lattice())
 
 
+# ---- instrumentation ----
+@pytest.mark.parametrize("name,dims,over", [("C2", (48, 48, 48), {"subsection": 4}), ("C4", (40, 40, 40), {"subsection": 8}),
+                                            ("C5", (96, 64), {"subsection": 8, "periodic": (1, 1, 0)}), ("C1", None, {})])
+def test_interface_counts_equal_oracle(pk, oracle_mod, name, dims, over):
+    """Interface counts by type pair (sorting observable, Fig 4), both lattice layouts, before and after a few MCS."""
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims)
+    g, o = _pair(pk, oracle_mod, cfg, **over)
+    np.testing.assert_array_equal(g.get_interface_counts(), o.get_interface_counts())
+    g.step(3); o.step(3)
+    C = g.get_interface_counts()
+    np.testing.assert_array_equal(C, o.get_interface_counts())
+    assert C.sum() > 0 and (C == C.T).all()
+
+
+@pytest.mark.parametrize("dims,S,k,periodic", [((16, 16), 16, 256, (0, 0, 0)), ((16, 16), 2, 4, (0, 0, 0)), ((64, 48), 8, 16, (0, 0, 0)),
+                                               ((16, 16, 16), 4, 64, (0, 0, 0)), ((8, 24, 8), 8, 128, (0, 0, 0))])
+def test_update_statistics_equal_oracle(pk, oracle_mod, dims, S, k, periodic):
+    """Pick-frequency and waiting-time histograms of the schedule (Fig 3): the paper's 16x16 grid as one region and as 2x2
+    checkerboards, larger grids, 3D; taken at MCS 5 of a run; the state is not touched."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C1" if len(dims) == 2 else "C2", dims=dims)
+    g, o = _pair(pk, oracle_mod, cfg, subsection=S, attempts_per_activation=k)
+    g.step(5); o.step(5)
+    fg, wg = g.update_statistics(20, n_freq=8, n_wait=200, wait_bin=4)
+    fo, wo = o.update_statistics(20, n_freq=8, n_wait=200, wait_bin=4)
+    np.testing.assert_array_equal(fg, fo)
+    np.testing.assert_array_equal(wg, wo)
+    assert int(fg.sum()) == int(np.prod(dims)) * 20
+    g.step(1); o.step(1)
+    _compare(g, o, False, "after update_statistics")
+
+
 def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     """Inputs/outputs as device tensors (on_device=1); and the non-TMA staging path."""
     import torch

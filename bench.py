@@ -236,6 +236,72 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+def run_speed_accuracy_map(args):
+    """--map: the S x switching-frequency speed / accuracy map of the paper's 2D circular chemotaxis workload
+    (Fig 6E) as a markdown table on stdout.
+    accuracy side: an ensemble of `--ensemble` seeds of C7 at 128x128 (one cell circling in the tangential field), 200 MCS;
+    per-pixel occupancy q (fraction of runs in which the pixel is covered by a cell at the end) against the occupancy p of
+    the SERIAL schedule (S = 128: the whole lattice is one region, i.e. the update order of the serial CPM), as the mean
+    binary cross-entropy in bits, probabilities clipped to [1/2n, 1 - 1/2n]; accuracy = 1 - cross-entropy (the paper's axis).
+    speed side: copy attempts/s of the same (S, k) on C7 at `--dims` (default 4096x4096), 10 MCS after 10 burn-in."""
+    import torch
+    import cpm_inputs as ci
+    import paper_2312_09317_b200 as pk
+    n_ens, n_mcs = args.ensemble, 200
+    small = ci.make_config("C7", dims=(128, 128))
+
+    def occupancy(S, k, seed0):
+        streams = [torch.cuda.Stream() for _ in range(8)]
+        ctxs = []
+        for i in range(n_ens):
+            p = dict(small["params"]); p.update(subsection=S, attempts_per_activation=k, seed=seed0 + i)
+            with torch.cuda.stream(streams[i % len(streams)]):
+                g = pk.CPM(small["dims"], max_cells=small["max_cells"], **p)
+                g.set_lattice(small["ids"], None, small["cell_type"])
+                g.set_chemotaxis_field(small["field"])
+                g.step(n_mcs)
+                ctxs.append(g)
+        torch.cuda.synchronize()
+        occ = np.zeros(small["ids"].shape, dtype=np.float64)
+        for g in ctxs:
+            occ += (g.get_lattice() != 0)
+        return occ / n_ens
+
+    def cross_entropy(p, q):
+        eps = 1.0 / (2 * n_ens)
+        q = np.clip(q, eps, 1 - eps)
+        return float(-(p * np.log2(q) + (1 - p) * np.log2(1 - q)).mean())
+
+    p_serial = occupancy(128, 0, 1000)
+    p_serial2 = occupancy(128, 0, 500000)          # an independent serial ensemble: the noise floor of the measure
+    big_dims = parse_dims(args.dims) if args.dims else (4096, 4096)
+    big = ci.make_config("C7", dims=big_dims)
+    N = int(np.prod(big_dims))
+    rows = []
+    for S in (2, 4, 8, 16):
+        for k in sorted({max(S * S // div, 1) for div in (1, 4, 16)}, reverse=True):
+            q = occupancy(S, k, 1000)
+            ce = cross_entropy(p_serial, q)
+            p = dict(big["params"]); p.update(subsection=S, attempts_per_activation=k)
+            g = pk.CPM(big["dims"], max_cells=big["max_cells"], **p)
+            g.set_lattice(big["ids"], None, big["cell_type"])
+            g.set_chemotaxis_field(big["field"])
+            g.step(BURN_IN_MCS)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); g.step(10); e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 10
+            rows.append((S, k, g.get_schedule()["phase_steps_per_mcs"], N / (ms * 1e-3), ms, ce, 1 - ce))
+            del g
+    print("| S | k | phase-steps / MCS | attempts/s (C7 %s) | ms / MCS | cross-entropy vs serial (bits / pixel) | accuracy |" % "x".join(map(str, big_dims)))
+    print("|---:|---:|---:|---:|---:|---:|---:|")
+    for r in rows:
+        print("| %d | %d | %d | %.3g | %.3f | %.4f | %.4f |" % r)
+    print()
+    print("serial ensemble against itself (entropy of p, the lower bound): %.4f bits / pixel; against an independent serial "
+          "ensemble (noise floor at %d runs): %.4f bits / pixel" % (cross_entropy(p_serial, p_serial), n_ens, cross_entropy(p_serial, p_serial2)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -249,7 +315,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-live", action="store_true", help="skip the extra LIVE-mode measurement")
+    ap.add_argument("--map", action="store_true", help="print the speed / accuracy map of the C7 chemotaxis workload instead of the bench line")
+    ap.add_argument("--ensemble", type=int, default=64, help="--map: runs per ensemble")
     args = ap.parse_args()
+    if args.map:
+        run_speed_accuracy_map(args)
+        return
     args.warmup = max(args.warmup, BURN_IN_MCS)   # both arms: the same burn-in, so the same MCS window is timed
 
     rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)

@@ -202,6 +202,32 @@ def test_2d_shapes_boundaries(pk, oracle_mod, dims, S, periodic):
     _run(pk, oracle_mod, cfg, 8, 2, periodic=periodic)
 
 
+@pytest.mark.parametrize("S,flags", [(8, 0), (16, 0), (8, 1), (32, 0)])
+def test_2d_act_both_kernels(pk, oracle_mod, S, flags):
+    """The Act extension in 2D (BASELINE's 2D configs have none): pooled kernel S = 8, 16; warp kernel S = 8 (forced), 32."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C5", dims=(96, 64), subsection=S)
+    cfg["params"]["lambda_act"] = [0, 150, 90]; cfg["params"]["max_act"] = [0, 30, 12]
+    g, o = _run(pk, oracle_mod, cfg, 8, 2, act=True, flags=flags)
+    assert g.get_launch_info()["pooled"] == (flags == 0 and S <= 16)
+    assert g.get_act().max() > 0
+
+
+def test_nine_types_fall_back_to_the_warp_kernel(pk, oracle_mod):
+    """More than 8 cell types (reading R3): the pooled kernel's 5-bit type field is not used, the warp kernel runs instead."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C2", dims=(32, 32, 32), subsection=4)
+    rng = np.random.default_rng(12)
+    nT = 9
+    J = rng.integers(5, 31, size=(nT, nT)); J = (np.triu(J) + np.triu(J, 1).T).astype(np.int32)
+    ct = rng.integers(1, nT, size=cfg["max_cells"] + 1).astype(np.uint8); ct[0] = 0
+    cfg["cell_type"] = ct
+    cfg["params"].update(J=J, lambda_V=[0] + [25] * 8, target_V=[0] + [500] * 8, lambda_P=[0] + [2] * 8,
+                         target_P=[0] + [cfg["params"]["target_P"][1]] * 8)
+    g, o = _run(pk, oracle_mod, cfg, 4, 2)
+    assert not g.get_launch_info()["pooled"]
+
+
 @pytest.mark.parametrize("S", [8, 4])
 def test_negative_J_and_extreme_temperatures(pk, oracle_mod, S):
     """Negative adhesion energies occur in the paper (J_cell,FRC down to -3000, L194-201)."""
@@ -420,12 +446,13 @@ def test_graph_and_plain_launches_agree(pk, oracle_mod, name, dims):
     assert g.get_launch_info()["sweep_launches"] == gp.get_launch_info()["sweep_launches"] == gt.get_launch_info()["sweep_launches"] == 6 * per_mcs
 
 
-def test_live_mode_equals_deterministic_while_no_cell_is_shared(pk, oracle_mod):
-    """P13 on the GPU: inside the precondition the paper-faithful LIVE kernel must reproduce the
-    deterministic oracle bit for bit (config 1 starts inside it)."""
+@pytest.mark.parametrize("flags", [0, 1])
+def test_live_mode_equals_deterministic_while_no_cell_is_shared(pk, oracle_mod, flags):
+    """P13 on the GPU: inside the precondition the paper-faithful LIVE kernel (pooled kernel, and the warp-per-subsection
+    kernel with CPM_FLAG_WARP_KERNEL) must reproduce the deterministic oracle bit for bit (config 1 starts inside it)."""
     import cpm_inputs as ci
     cfg = ci.make_config("C1")
-    gl = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], mode=pk.MODE_LIVE_ATOMICS, **cfg["params"])
+    gl = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], mode=pk.MODE_LIVE_ATOMICS, flags=flags, **cfg["params"])
     gl.set_lattice(cfg["ids"], None, cfg["cell_type"])
     od = oracle_mod.Oracle(cfg["dims"], max_cells=cfg["max_cells"], mode=0, **cfg["params"])
     od.set_lattice(cfg["ids"], None, cfg["cell_type"])
@@ -477,7 +504,7 @@ def test_act_msd_ensemble_live_mode(pk, oracle_mod):
     """Act-model cell mean-squared displacement in LIVE mode within 2% relative of the oracle
     (north_star); centroids from the integer sums (Eq 10)."""
     import cpm_inputs as ci
-    cfg = ci.make_config("C3", dims=(64, 64, 64))
+    cfg = ci.make_config("C3", dims=(128, 128, 128))   # ~ 200 motile cells per run
 
     def msd(s):
         st0 = s.get_cell_stats()
@@ -493,10 +520,9 @@ def test_act_msd_ensemble_live_mode(pk, oracle_mod):
         g, o = _pair(pk, oracle_mod, cfg, mode=1, seed=77 + seed)
         vg.append(msd(g)); vo.append(msd(o))
     mg, mo = np.mean(vg), np.mean(vo)
-    # 8 seeds x 27 cells: the standard error of the mean is itself a few percent, so the bound is
-    # 2% plus 3 standard errors of the difference
-    se = np.sqrt(np.var(vg) / 8 + np.var(vo) / 8)
-    assert abs(mg - mo) <= 0.02 * mo + 3 * se, (mg, mo, se)
+    # both sides draw the same random numbers and differ only in the interleaving of the atomics, so their
+    # trajectories stay close: the north_star's plain 2 % holds without a sampling-error allowance
+    assert abs(mg - mo) <= 0.02 * mo, (mg, mo, vg, vo)
 
 
 def test_errors_are_reported(pk):

@@ -230,12 +230,11 @@ struct Sweep {
   }
 
   // ---- per-cell state as this attempt sees it (a6) ----
-  // deterministic: snapshot + own deltas; returns the entry index through e
+  // deterministic: snapshot + own deltas.  e = index of the cell's entry in the own-delta table, -1 when the cell has
+  // not been CHANGED in this activation yet (looking at a cell does not take an entry, reading R2)
   __device__ __forceinline__ unsigned long long lookup(uint32_t cell, int &e) {
-    if (LIVE) {
-      e = -1;
-      return __ldcg(P.liveVP + cell);  // live, possibly stale (L53)
-    }
+    e = -1;
+    if (LIVE) return __ldcg(P.liveVP + cell);  // live, possibly stale (L53)
     unsigned long long cur = 0;
     bool found = false;
 #pragma unroll
@@ -248,23 +247,11 @@ struct Sweep {
         found = true;
       }
     }
-    if (found) return cur;
-    const unsigned long long base = __ldg(P.snapVP + cell);
-    if (n_entries >= 32 * NSETS) {  // table full: cannot keep own deltas -> report, keep going
-      overflow = true;
-      e = -1;
-      return base;
-    }
-    e = n_entries++;
-#pragma unroll
-    for (int s = 0; s < NSETS; ++s)
-      if ((e >> 5) == s && lane == (e & 31)) {
-        tab.key[s] = cell; tab.cur[s] = base; tab.dvp[s] = 0ull; tab.dsx[s] = 0; tab.dsy[s] = 0; tab.dsz[s] = 0;
-      }
-    return base;
+    return found ? cur : __ldg(P.snapVP + cell);
   }
 
-  __device__ __forceinline__ void add_delta(uint32_t cell, int e, int dV, int dP, int x, int y, int z, int sgn) {
+  // vp: the value lookup() returned for this cell (its snapshot value when e < 0)
+  __device__ __forceinline__ void add_delta(uint32_t cell, int e, unsigned long long vp, int dV, int dP, int x, int y, int z, int sgn) {
     // composite delta dV*2^32 + dP, mod 2^64 (the paper's interleaved pair, L297, updated by one add)
     const unsigned long long d = ((unsigned long long)(long long)dV << 32) + (unsigned long long)(long long)dP;
     if (LIVE) {
@@ -276,7 +263,15 @@ struct Sweep {
       }
       return;
     }
-    if (e < 0) return;  // overflowed table: error already flagged
+    if (e < 0) {   // first change of this cell in this activation: it takes an entry now
+      if (n_entries >= 32 * NSETS) { overflow = true; return; }   // table full: reported, not computed approximately
+      e = n_entries++;
+#pragma unroll
+      for (int s = 0; s < NSETS; ++s)
+        if ((e >> 5) == s && lane == (e & 31)) {
+          tab.key[s] = cell; tab.cur[s] = vp; tab.dvp[s] = 0ull; tab.dsx[s] = 0; tab.dsy[s] = 0; tab.dsz[s] = 0;
+        }
+    }
 #pragma unroll
     for (int s = 0; s < NSETS; ++s)
       if ((e >> 5) == s && lane == (e & 31)) {
@@ -398,8 +393,8 @@ struct Sweep {
     __syncwarp();
     dirty = true;
     const int gx = ox + lx, gy = oy + ly, gz = oz + lz;
-    if (A != 0) add_delta(A, entA, 1, dPA, sum_coord(P, A, 0, gx), sum_coord(P, A, 1, gy), sum_coord(P, A, 2, gz), +1);
-    if (B != 0) add_delta(B, entB, -1, dPB, sum_coord(P, B, 0, gx), sum_coord(P, B, 1, gy), sum_coord(P, B, 2, gz), -1);
+    if (A != 0) add_delta(A, entA, vpA, 1, dPA, sum_coord(P, A, 0, gx), sum_coord(P, A, 1, gy), sum_coord(P, A, 2, gz), +1);
+    if (B != 0) add_delta(B, entB, vpB, -1, dPB, sum_coord(P, B, 0, gx), sum_coord(P, B, 1, gy), sum_coord(P, B, 2, gz), -1);
     return true;
   }
 

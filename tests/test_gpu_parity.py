@@ -563,6 +563,24 @@ def test_cell_table_overflow_is_flagged(pk, S):
     assert e.value.code == -3
 
 
+@pytest.mark.parametrize("S", [8, 4])
+def test_many_cells_looked_at_few_changed(pk, oracle_mod, S):
+    """Reading R2 counts the cells a subsection CHANGES in one activation, not the ones it looks at: 2-voxel cells (far more
+    than 32 in the reach of one subsection) at a temperature where few copies are accepted run without an overflow and
+    equal the oracle (warp kernel S = 8, pooled kernel S = 4)."""
+    dims = (16, 16, 16)
+    n = 16 ** 3 // 2
+    ids = ((np.arange(16 ** 3, dtype=np.uint32).reshape(16, 16, 16)) // 2 + 1).astype(np.uint32)
+    ct = np.ones(n + 1, np.uint8); ct[0] = 0
+    kw = dict(J=np.zeros((2, 2), dtype=np.int32), lambda_V=[0, 3], target_V=[0, 2], max_cells=n, T=1.0, subsection=S, seed=3)
+    g = pk.CPM(dims, **kw); o = oracle_mod.Oracle(dims, **kw)
+    g.set_lattice(ids, None, ct); o.set_lattice(ids, None, ct)
+    g.step(3); o.step(3)
+    _compare(g, o, False, "many cells looked at")
+    c = g.get_counters()
+    assert c["evaluated"] > 10000 and 20 < c["accepted"] < 400
+
+
 def test_C4_256_cubed_scheduler_choice_bit_exact(pk, oracle_mod):
     """Config 4 recipe at 256^3 (16.8 M voxels, 262 144 subsections of 4^3, ~16 k cells, obstacles, Act)
     in the launch configuration bench.py times (subsection = 0: the scheduler's choice), compared with the

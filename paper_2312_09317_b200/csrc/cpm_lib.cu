@@ -433,7 +433,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->use_tma = !(p->flags & CPM_FLAG_NO_TMA) && (S % 4 == 0);
   size_t pool_smem = 0;
   c->tfn = (nT <= 8 && !(p->flags & CPM_FLAG_WARP_KERNEL))
-               ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, pers_on || chem_on, nT, &pool_smem) : nullptr;
+               ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, pers_on || chem_on || c->unwrap, nT, &pool_smem) : nullptr;
   c->pooled = c->tfn != nullptr;
   if (c->pooled) c->use_tma = true;   // one bulk copy per group of 32 tiles
 
@@ -531,11 +531,12 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   if (c->pooled) {
     alloc((void **)&tl.tiles, c->tile_words * 4);
     if (c->mode == CPM_MODE_DETERMINISTIC) {
-      // spill slots for chains that change more than PK_DCAP distinct cells in one activation: one for every 8th
-      // chain of the largest colour (a few per cent of the chains need one), between 64 Ki and 1 Mi slots
+      // spill slots for chains that change more than PK_DCAP distinct cells in one activation: one for every chain of
+      // the largest colour (12 * PK_SPILL bytes each: 0.7 GB at 1024^3), so the pool itself can never run out; beyond
+      // 8 Mi chains per colour one for every 8th chain
       unsigned long long most = 0;
       for (int col = 0; col < 8; ++col) most = std::max(most, c->n_act_col[col]);
-      sp.ovf_cap = (int)std::min<unsigned long long>(std::max<unsigned long long>(most / 8, 65536ull), 1048576ull);
+      sp.ovf_cap = (int)(most <= (8ull << 20) ? std::max<unsigned long long>(most, 1ull) : std::max<unsigned long long>(most / 8, 8ull << 20));
       alloc((void **)&c->ovf_keys, (size_t)sp.ovf_cap * PK_SPILL * 4);
       alloc((void **)&c->ovf_dvp, (size_t)sp.ovf_cap * PK_SPILL * 8);
     }

@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         dH += (long long)(pa.lamP * dPA) * (2 * dpa + dPA) + (long long)(pb.lamP * dPB) * (2 * dpb + dPB);
         if constexpr (VEC) {
           // chemotaxis / persistence bias (Eq 4, 5; reading S21), only for the specialisation that has these terms (L282)
-          if (go) {
+          if (go && P.vec_on) {   // (the specialisation also serves periodic centroid tracking alone)
             constexpr int CEN = (DIM == 3) ? (T * T + T + 1) : (T + 1);
             const int dd = soff - toff + CEN;   // = ((dz + 1) T + dy + 1) T + dx + 1 of the source's offset
             const int ddx = dd % T - 1, ddy = (dd / T) % T - 1, ddz = (DIM == 3) ? dd / (T * T) - 1 : 0;
@@ -491,7 +491,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
               const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
               unsigned long long *const arr = which == 0 ? P.liveVP : which == 1 ? P.sumx : which == 2 ? P.sumy : P.sumz;
               const unsigned long long v = which == 0 ? ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP
-                                                      : (unsigned long long)(long long)(sgn * sum_coord(P, cell, which - 1, which == 1 ? gx : which == 2 ? gy : gz));
+                                                      : (unsigned long long)(long long)(sgn * (VEC ? sum_coord(P, cell, which - 1, which == 1 ? gx : which == 2 ? gy : gz)
+                                                                                                   : (which == 1 ? gx : which == 2 ? gy : gz)));   // periodic tracking (S23) rides on the VEC specialisation
               atomicAdd(arr + cell, v);
             }
           }

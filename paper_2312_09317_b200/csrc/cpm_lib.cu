@@ -670,12 +670,11 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
     const TileLayout &tl = c->sp.tl;
     for (int col = 0; col < (1 << c->d); ++col) {
       if (c->n_act_col[col] == 0) continue;
-      const long long words = (long long)(c->grp_col[col] * (unsigned long long)tl.TW * (unsigned long long)PK_GC);
       if (c->d == 2)
-        tile_pack_kernel<2><<<grid_for(words), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
+        tile_pack_kernel<2><<<grid_for((long long)c->grp_col[col], 1), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
                                                                      c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
       else
-        tile_pack_kernel<3><<<grid_for(words), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
+        tile_pack_kernel<3><<<grid_for((long long)c->grp_col[col], 1), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
                                                                      c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
       c->launches++;
     }

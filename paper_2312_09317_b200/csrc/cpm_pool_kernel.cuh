@@ -583,40 +583,43 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
 }
 
 // ------------------------------------------------------------ tiled-layout helpers ----------
-// set_lattice: ids (+frozen, cell types) -> tiles with halo.  One thread per tile word of one colour.
+// set_lattice: ids (+frozen, cell types) -> tiles with halo.  A block takes whole groups; thread t writes the words
+// j = t >> 3, t >> 3 + blockDim / 8, ... of chain t & 7, so the chain's geometry is worked out once per group and the
+// stores of a warp are contiguous (no 64-bit division per word).
 template <int DIM>
 __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, const uint8_t *ctype, uint32_t max_cells, TileLayout L,
                                  int col, unsigned long long n_active, int X, int Y, int Z, int perx, int pery, int perz,
                                  int *error_flag) {
   const int S = L.S, T = S + 2, TW = L.TW;
   const unsigned long long ngrp = (n_active + (unsigned long long)(PK_GC - 1)) >> PK_GS;
-  const unsigned long long total = ngrp * (unsigned long long)TW * (unsigned long long)PK_GC;
-  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
-    const int c = (int)(i & (unsigned long long)(PK_GC - 1));
-    const unsigned long long r = i >> PK_GS;
-    const int j = (int)(r % (unsigned)TW);
-    const unsigned long long w = (r / (unsigned)TW) * (unsigned long long)PK_GC + (unsigned long long)c;
-    uint32_t word = 0u;
-    if (w < n_active) {
-      const int ax = (int)(w % (unsigned)L.nact[col][0]);
-      const unsigned long long r1 = w / (unsigned)L.nact[col][0];
-      const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
-      const int az = (int)(r1 / (unsigned)L.nact[col][1]);
-      const int bx = 2 * ax + (col & 1), by = 2 * ay + ((col >> 1) & 1), bz = (DIM == 3) ? 2 * az + ((col >> 2) & 1) : 0;
-      int x = bx * S + j % T - 1, y = by * S + (j / T) % T - 1, z = (DIM == 3) ? bz * S + j / (T * T) - 1 : 0;
-      bool ok = true;
-      if (x < 0) { if (perx) x += X; else ok = false; } else if (x >= X) { if (perx) x -= X; else ok = false; }
-      if (y < 0) { if (pery) y += Y; else ok = false; } else if (y >= Y) { if (pery) y -= Y; else ok = false; }
-      if (DIM == 3) { if (z < 0) { if (perz) z += Z; else ok = false; } else if (z >= Z) { if (perz) z -= Z; else ok = false; } }
-      if (ok) {
-        const long long gi = (long long)x + (long long)X * ((long long)y + (long long)Y * z);
-        uint32_t id = ids[gi];
-        if (id > max_cells) { atomicOr(error_flag, 2); id = 0; }
-        word = id | ((uint32_t)ctype[id] << PK_TYPE_SHIFT) | ((frozen && frozen[gi]) ? PK_FROZEN : 0u);
+  const int c = (int)(threadIdx.x & (PK_GC - 1));
+  for (unsigned long long grp = blockIdx.x; grp < ngrp; grp += gridDim.x) {
+    const unsigned long long w = grp * (unsigned long long)PK_GC + (unsigned long long)c;
+    const bool live = w < n_active;   // the host keeps n_active below 2^31 for this layout
+    const uint32_t w32 = (uint32_t)w;
+    const int ax = (int)(w32 % (unsigned)L.nact[col][0]);
+    const uint32_t r1 = w32 / (unsigned)L.nact[col][0];
+    const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
+    const int az = (int)(r1 / (unsigned)L.nact[col][1]);
+    const int x0 = (2 * ax + (col & 1)) * S - 1, y0 = (2 * ay + ((col >> 1) & 1)) * S - 1, z0 = (DIM == 3) ? (2 * az + ((col >> 2) & 1)) * S - 1 : 0;
+    uint32_t *out = L.tiles + L.base[col] + grp * (unsigned long long)TW * (unsigned long long)PK_GC + (unsigned long long)c;
+    for (int j = (int)(threadIdx.x >> PK_GS); j < TW; j += (int)(blockDim.x >> PK_GS)) {
+      uint32_t word = 0u;
+      if (live) {
+        int x = x0 + j % T, y = y0 + (j / T) % T, z = (DIM == 3) ? z0 + j / (T * T) : 0;
+        bool ok = true;
+        if (x < 0) { if (perx) x += X; else ok = false; } else if (x >= X) { if (perx) x -= X; else ok = false; }
+        if (y < 0) { if (pery) y += Y; else ok = false; } else if (y >= Y) { if (pery) y -= Y; else ok = false; }
+        if (DIM == 3) { if (z < 0) { if (perz) z += Z; else ok = false; } else if (z >= Z) { if (perz) z -= Z; else ok = false; } }
+        if (ok) {
+          const long long gi = (long long)x + (long long)X * ((long long)y + (long long)Y * z);
+          uint32_t id = ids[gi];
+          if (id > max_cells) { atomicOr(error_flag, 2); id = 0; }
+          word = id | ((uint32_t)ctype[id] << PK_TYPE_SHIFT) | ((frozen && frozen[gi]) ? PK_FROZEN : 0u);
+        }
       }
+      out[j * PK_GC] = word;
     }
-    L.tiles[L.base[col] + i] = word;
   }
 }
 template <int DIM>
@@ -640,45 +643,76 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
   const int S = L.S, T = S + 2, TW = L.TW;
   constexpr int NNB = (DIM == 2) ? 8 : 26;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_active; w += stride) {
-    const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (w & (unsigned long long)(PK_GC - 1));
-    const int ax = (int)(w % (unsigned)L.nact[col][0]);
-    const unsigned long long r1 = w / (unsigned)L.nact[col][0];
-    const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
-    const int az = (int)(r1 / (unsigned)L.nact[col][1]);
-    const int ox = (2 * ax + (col & 1)) * S, oy = (2 * ay + ((col >> 1) & 1)) * S, oz = (DIM == 3) ? (2 * az + ((col >> 2) & 1)) * S : 0;
-    uint32_t cur = 0;
-    unsigned long long cv = 0, cx = 0, cy = 0, cz = 0;
-    auto flush = [&]() {
-      if (cur != 0) {
-        atomicAdd(liveVP + cur, cv);
-        atomicAdd(sumx + cur, cx); atomicAdd(sumy + cur, cy);
-        if (DIM == 3) atomicAdd(sumz + cur, cz);
-      }
-    };
-    for (int lz = 0; lz < (DIM == 3 ? S : 1); ++lz)
-      for (int ly = 0; ly < S; ++ly)
-        for (int lx = 0; lx < S; ++lx) {
-          const int j = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-          const uint32_t me = tc[j * PK_GC] & ID_MASK;
-          if (me != cur) { flush(); cur = me; cv = cx = cy = cz = 0; }
-          if (me == 0) continue;
-          int foreign = 0;
-          for (int nb = 0; nb < NNB; ++nb) {
-            int dx, dy, dz;
-            nb_delta<DIM>(nb, dx, dy, dz);
-            foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_GC] & ID_MASK) != me);
-          }
-          cv += (1ull << 32) + (unsigned long long)foreign;
-          int qx = ox + lx, qy = oy + ly, qz = oz + lz;
-          if (anc != nullptr) {   // reading S23: the image of the site nearest to the cell's anchor
-            if (perx) qx = image_near(qx, anc[3 * (size_t)me], X);
-            if (pery) qy = image_near(qy, anc[3 * (size_t)me + 1], Y);
-            if (perz) qz = image_near(qz, anc[3 * (size_t)me + 2], Z);
-          }
-          cx += (unsigned long long)(long long)qx; cy += (unsigned long long)(long long)qy; cz += (unsigned long long)(long long)qz;
+  const unsigned long long first = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long n_iter = (n_active + stride - 1) / stride;   // same trip count for every lane of a warp
+  for (unsigned long long it = 0; it < n_iter; ++it) {
+    const unsigned long long w = first + it * stride;
+    // frozen voxels (one obstacle id can own a fifth of the lattice, L139) are tallied apart and combined over the warp
+    // before they reach the per-cell arrays: their atomics would all hit the same few addresses
+    uint32_t fid = 0;
+    int fcnt = 0, ffor = 0, fsx = 0, fsy = 0, fsz = 0;
+    if (w < n_active) {
+      const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (w & (unsigned long long)(PK_GC - 1));
+      const uint32_t w32 = (uint32_t)w;   // the host keeps n_active below 2^31 for this layout
+      const int ax = (int)(w32 % (unsigned)L.nact[col][0]);
+      const uint32_t r1 = w32 / (unsigned)L.nact[col][0];
+      const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
+      const int az = (int)(r1 / (unsigned)L.nact[col][1]);
+      const int ox = (2 * ax + (col & 1)) * S, oy = (2 * ay + ((col >> 1) & 1)) * S, oz = (DIM == 3) ? (2 * az + ((col >> 2) & 1)) * S : 0;
+      uint32_t cur = 0;
+      unsigned long long cv = 0, cx = 0, cy = 0, cz = 0;
+      auto flush = [&](uint32_t id, unsigned long long v, unsigned long long x, unsigned long long y, unsigned long long z) {
+        if (id != 0) {
+          atomicAdd(liveVP + id, v);
+          atomicAdd(sumx + id, x); atomicAdd(sumy + id, y);
+          if (DIM == 3) atomicAdd(sumz + id, z);
         }
-    flush();
+      };
+      for (int lz = 0; lz < (DIM == 3 ? S : 1); ++lz)
+        for (int ly = 0; ly < S; ++ly)
+          for (int lx = 0; lx < S; ++lx) {
+            const int j = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
+            const uint32_t word = tc[j * PK_GC];
+            const uint32_t me = word & ID_MASK;
+            const bool frozen = (word & PK_FROZEN) != 0u;
+            if (!frozen && me != cur) { flush(cur, cv, cx, cy, cz); cur = me; cv = cx = cy = cz = 0; }
+            if (me == 0) continue;
+            int foreign = 0;
+            for (int nb = 0; nb < NNB; ++nb) {
+              int dx, dy, dz;
+              nb_delta<DIM>(nb, dx, dy, dz);
+              foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_GC] & ID_MASK) != me);
+            }
+            int qx = ox + lx, qy = oy + ly, qz = oz + lz;
+            if (anc != nullptr) {   // reading S23: the image of the site nearest to the cell's anchor
+              if (perx) qx = image_near(qx, anc[3 * (size_t)me], X);
+              if (pery) qy = image_near(qy, anc[3 * (size_t)me + 1], Y);
+              if (perz) qz = image_near(qz, anc[3 * (size_t)me + 2], Z);
+            }
+            if (frozen) {
+              if (me != fid) {   // a second obstacle id in one subsection: rare, flushed directly
+                flush(fid, ((unsigned long long)fcnt << 32) + (unsigned long long)ffor, (unsigned long long)(long long)fsx,
+                      (unsigned long long)(long long)fsy, (unsigned long long)(long long)fsz);
+                fid = me; fcnt = ffor = fsx = fsy = fsz = 0;
+              }
+              fcnt += 1; ffor += foreign; fsx += qx; fsy += qy; fsz += qz;
+            } else {
+              cv += (1ull << 32) + (unsigned long long)foreign;
+              cx += (unsigned long long)(long long)qx; cy += (unsigned long long)(long long)qy; cz += (unsigned long long)(long long)qz;
+            }
+          }
+      flush(cur, cv, cx, cy, cz);
+    }
+    // lanes holding the same obstacle id add up first; one lane issues the atomics (<= 64 sites per lane: 32-bit sums)
+    const unsigned peers = __match_any_sync(FULL, fid);
+    const int tcnt = (int)__reduce_add_sync(peers, (unsigned)fcnt), tfor = (int)__reduce_add_sync(peers, (unsigned)ffor);
+    const int tsx = (int)__reduce_add_sync(peers, (unsigned)fsx), tsy = (int)__reduce_add_sync(peers, (unsigned)fsy);
+    const int tsz = (int)__reduce_add_sync(peers, (unsigned)fsz);
+    if (fid != 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) {
+      atomicAdd(liveVP + fid, ((unsigned long long)(unsigned)tcnt << 32) + (unsigned long long)(unsigned)tfor);
+      atomicAdd(sumx + fid, (unsigned long long)(long long)tsx); atomicAdd(sumy + fid, (unsigned long long)(long long)tsy);
+      if (DIM == 3) atomicAdd(sumz + fid, (unsigned long long)(long long)tsz);
+    }
   }
 }
 

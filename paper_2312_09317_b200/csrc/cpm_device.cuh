@@ -680,6 +680,14 @@ __global__ void act_decay_kernel(uint4 *act, long long n_vec, uint32_t *mcs_ptr,
     act[j] = v;
   }
 }
+// deterministic mode, after every phase-step: snapshot := live (reading S12) and the spill-slot counter of the pooled kernel
+// back to 0 for the next phase-step -- one launch instead of a copy node and a memset node
+__global__ void snapshot_kernel(const ulonglong2 *live, ulonglong2 *snap, long long n_pairs, int *ovf_count) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && ovf_count) *ovf_count = 0;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long j = i; j < n_pairs; j += stride) snap[j] = live[j];
+}
 __global__ void mcs_increment_kernel(uint32_t *mcs_ptr, uint32_t *pers_n) { *mcs_ptr += 1; if (pers_n) *pers_n += 1; }
 
 // ---- periodic centroid tracking (L297, reading S23) ----

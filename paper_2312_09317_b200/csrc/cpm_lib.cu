@@ -283,7 +283,6 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       const unsigned long long per_cta = c->pooled ? (unsigned long long)PK_GC : (unsigned long long)c->wpc;
       const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
       if (grid > 0x7fffffffULL || (c->pooled && n_active > 0x7fffffffULL)) return fail(c, CPM_ERR_UNSUPPORTED, "too many subsections for one launch");
-      if (c->pooled && c->snapVP) CK(cudaMemsetAsync(c->ovf_count, 0, 4, st));
       cudaEvent_t e0 = nullptr, e1 = nullptr;
       if (timed) {
         while (c->ev_pool.size() < c->ev_used + 2) { cudaEvent_t e; CK(cudaEventCreate(&e)); c->ev_pool.push_back(e); }
@@ -295,7 +294,11 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       if (timed) CK(cudaEventRecord(e1, st));
       c->launches++; c->sweep_launches++;
       // deterministic mode: the next phase-step reads the values as of its own start
-      if (c->snapVP) CK(cudaMemcpyAsync(c->snapVP, c->liveVP, ncell * 8, cudaMemcpyDeviceToDevice, st));
+      if (c->snapVP) {
+        const long long n_pairs = (long long)((ncell + 1) / 2);   // the arrays are allocated in whole 16-byte pairs
+        snapshot_kernel<<<grid_for(n_pairs), 256, 0, st>>>((const ulonglong2 *)c->liveVP, (ulonglong2 *)c->snapVP, n_pairs, c->ovf_count);
+        c->launches++;
+      }
     }
   if (c->unwrap) {   // L297: centroids back inside the lattice on periodic axes, anchors follow
     const long long ncl = (long long)ncell;
@@ -545,8 +548,8 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     alloc((void **)&c->lat, (size_t)pitch * rows * 4);
   }
   if (c->act_enabled) alloc((void **)&c->act, (size_t)apitch * rows);
-  alloc((void **)&c->liveVP, ncell * 8);
-  if (c->mode == CPM_MODE_DETERMINISTIC) alloc((void **)&c->snapVP, ncell * 8);
+  alloc((void **)&c->liveVP, (ncell + 1) / 2 * 16);
+  if (c->mode == CPM_MODE_DETERMINISTIC) alloc((void **)&c->snapVP, (ncell + 1) / 2 * 16);
   alloc((void **)&c->sumx, ncell * 8); alloc((void **)&c->sumy, ncell * 8); alloc((void **)&c->sumz, ncell * 8);
   alloc((void **)&c->counters, COUNTER_SLOTS * 2 * 8);
   alloc((void **)&c->error_flag, 4); alloc((void **)&c->mcs_dev, 4);

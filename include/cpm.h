@@ -121,7 +121,9 @@ int  cpm_step(cpm_ctx *ctx, uint32_t n_mcs);
 
 int  cpm_get_lattice(cpm_ctx *ctx, uint32_t *ids, int on_device);
 int  cpm_get_act(cpm_ctx *ctx, float *act, int on_device);
-/* Per-cell globals kept by integer atomics (L51, L57, L288): volume, perimeter, coordinate sums. */
+/* Per-cell globals kept by integer atomics (L51, L57, L288): volume, perimeter, coordinate sums.  Volume and perimeter
+ * share one 64-bit word {V:hi32, P:lo32} (the paper's interleaved pair, L297): a cell whose perimeter reaches 2^32
+ * (only an obstacle id owning > 1.6e8 surface-like voxels could) would carry into its volume -- outside this build. */
 int  cpm_get_cell_stats(cpm_ctx *ctx, uint32_t *volume, uint32_t *perimeter,
                         uint64_t *sum_x, uint64_t *sum_y, uint64_t *sum_z, int on_device);
 /* out (host) = {attempts, evaluated, accepted, mcs}. */

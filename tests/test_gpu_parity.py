@@ -296,6 +296,16 @@ def test_C6_persistence_collective_bit_exact(pk, oracle_mod, dims, over):
     assert (np.abs(nrm - 1) < 1e-12).mean() > 0.9      # nearly every cell has moved and carries a unit vector
 
 
+def test_C6_at_the_papers_size_bit_exact(pk, oracle_mod):
+    """C6 at 256^3, the size the paper quotes its 3D speed-up on (Fig 6D): 54 k cells, 3 MCS, everything compared."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C6")
+    assert cfg["dims"] == (256, 256, 256) and cfg["max_cells"] > 50000
+    g, o = _run(pk, oracle_mod, cfg, 3, 3)
+    c = g.get_counters()
+    assert c["accepted"] > 1000000
+
+
 def test_persistence_given_directions(pk, oracle_mod):
     """cpm_set_persistence: caller-chosen directions enter dH at once; a refused call changes nothing."""
     import cpm_inputs as ci

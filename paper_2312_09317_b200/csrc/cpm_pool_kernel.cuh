@@ -61,6 +61,13 @@ constexpr int PK_NOWIN = PK_SUPER << 10;     // "no accepted attempt": a chain's
 // lattice word of the tiled layout: [type:5 | frozen:1 | 00 | id:24]: the top byte is the byte offset type * 8 +
 // frozen * 4 into a row of the adhesion table, so a neighbour's adhesion term costs one multiply-high, one load
 // and one add
+// Order of a group's 8 tiles, in HBM and (the bulk copy keeps it) in shared memory: chain-major = the tile of chain c
+// is the contiguous block [c * TW, (c + 1) * TW); else word j of chain c at j * 8 + c.
+#ifndef PK_CHAIN_MAJOR
+#define PK_CHAIN_MAJOR 0   // measured on C4 1024^3: the sweep takes the same time either way (11.14 vs 11.16 ms per MCS: shared-memory bank conflicts are not what bounds it), pack and recount are slower chain-major (51 vs 33 ms)
+#endif
+constexpr int PK_TS = PK_CHAIN_MAJOR ? 1 : PK_GC;   // distance (words) between consecutive words of one chain's tile
+__host__ __device__ __forceinline__ constexpr int pk_tbase(int c, int TW) { return PK_CHAIN_MAJOR ? c * TW : c; }   // first word of chain c's tile
 constexpr uint32_t PK_FROZEN = 1u << 26;
 constexpr uint32_t PK_CELL = ~PK_FROZEN;        // type + id: equal iff same cell
 constexpr int PK_TYPE_SHIFT = 27;
@@ -118,7 +125,7 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
 __device__ __forceinline__ unsigned long long tile_word(const TileLayout &L, int bx, int by, int bz, int j) {
   const int col = (bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2);
   const unsigned long long w = (unsigned long long)(bx >> 1) + (unsigned long long)L.nact[col][0] * ((unsigned long long)(by >> 1) + (unsigned long long)L.nact[col][1] * (unsigned long long)(bz >> 1));
-  return L.base[col] + ((((w >> PK_GS) * (unsigned long long)L.TW + (unsigned long long)j) << PK_GS) | (w & (unsigned long long)(PK_GC - 1)));
+  return L.base[col] + (w >> PK_GS) * (unsigned long long)(L.TW * PK_GC) + (unsigned long long)(pk_tbase((int)(w & (unsigned long long)(PK_GC - 1)), L.TW) + j * PK_TS);
 }
 // home word of lattice site (x,y,z), all inside the lattice; S = L.S
 template <int DIM>
@@ -133,7 +140,7 @@ template <int DIM, int S, bool ACT, bool LIVE, bool VEC>
 __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
-  constexpr int T = G::T, TW = G::TW, NNB = G::NNB, GC = PK_GC, NJ = PK_NJ;
+  constexpr int T = G::T, TW = G::TW, NNB = G::NNB, GC = PK_GC, NJ = PK_NJ, TS = PK_TS;
   extern __shared__ __align__(128) unsigned char smem[];
   uint32_t *tile = reinterpret_cast<uint32_t *>(smem + M::TILE);
   uint32_t *prop = reinterpret_cast<uint32_t *>(smem + M::PROP);
@@ -190,7 +197,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;
   bool staged = false;
-  const uint32_t *const tcol = tile + c;   // this lane's own chain column
+  const uint32_t *const tcol = tile + pk_tbase(c, TW);   // the tile of this lane's own chain
 
   for (int sc = 0; sc < k; sc += PK_SUPER) {
     const int kk = min(PK_SUPER, k - sc);   // attempts of this stretch
@@ -205,7 +212,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
         const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
         const int toff = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-        prop[(4 * qq + j) * GC + c] = (uint32_t)(toff * (4 * GC)) | ((uint32_t)((toff + snoff[nb]) * (4 * GC)) << 16);
+        prop[(4 * qq + j) * GC + c] = (uint32_t)(toff * (4 * TS)) | ((uint32_t)((toff + snoff[nb]) * (4 * TS)) << 16);
       }
     }
     int pos = active ? 0 : kk;   // attempts < pos of this stretch are final (same value in the 4 lanes of a chain)
@@ -260,10 +267,10 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
       const int item = have ? (int)queue[lane] : 0;
       ci = item & (GC - 1); a = item >> PK_GS;
       const uint32_t prc = prop[a * GC + ci];
-      const int toff = (int)(prc & 0xffffu) / (4 * GC), soff = (int)(prc >> 16) / (4 * GC);
+      const int toff = (int)(prc & 0xffffu) / (4 * TS), soff = (int)(prc >> 16) / (4 * TS);
       int nA = 0, nB = 0;
-      const uint32_t *const tc = tile + ci;
-      const uint32_t wA = tc[soff * GC], wB = tc[toff * GC];
+      const uint32_t *const tc = tile + pk_tbase(ci, TW);
+      const uint32_t wA = tc[soff * TS], wB = tc[toff * TS];
       const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
       const uint32_t mA = wA & CELL_MASK31, mB = wB & CELL_MASK31;
       const int tA = (int)(wA >> PK_TYPE_SHIFT), tB = (int)(wB >> PK_TYPE_SHIFT);
@@ -279,7 +286,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         int adh = 0;
 #pragma unroll
         for (int n = 0; n < NNB; ++n) {
-          const uint32_t raw = tc[(toff + G::noff(n)) * GC];
+          const uint32_t raw = tc[(toff + G::noff(n)) * TS];
           count_same(nA, raw, wA);
           count_same(nB, raw, wB);
           adh += *reinterpret_cast<const int32_t *>(Drow + (raw >> 24));
@@ -396,7 +403,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
               const int qx = px + ddx, qy = py + ddy, qz = pz + ddz;
               const bool intile = qx >= 0 && qx < T && qy >= 0 && qy < T && (DIM == 2 || (qz >= 0 && qz < T));
               // ids two sites away from the subsection belong to inactive subsections: stable during this phase-step
-              const uint32_t wq = intile ? tile[(ctr + mynoff) * GC + cc] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
+              const uint32_t wq = intile ? tile[pk_tbase(cc, TW) + (ctr + mynoff) * TS] : __ldg(P.tl.tiles + home_word<DIM>(P.tl, S, gx, gy, gz));
               same = (wq & CELL_MASK31) == mC;
             }
             int av = 1;
@@ -450,8 +457,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         const int fw = first[cw];
         const int nA = (fw >> 5) & 31, nB = fw & 31;
         const uint32_t prc = prop[(on ? (fw >> 10) : 0) * GC + cw];
-        const int toff = (int)(prc & 0xffffu) / (4 * GC);
-        const uint32_t wA = tile[(int)(prc >> 16) / (4 * GC) * GC + cw], wB = tile[toff * GC + cw];
+        const int toff = (int)(prc & 0xffffu) / (4 * TS);
+        const uint32_t wA = tile[pk_tbase(cw, TW) + (int)(prc >> 16) / (4 * TS) * TS], wB = tile[pk_tbase(cw, TW) + toff * TS];
         const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
         __syncwarp();   // every lane has read the state of the round's start
         if (on) {
@@ -459,8 +466,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
           const int ox = orig[cw], oy = orig[GC + cw], oz = orig[2 * GC + cw];
           const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
           if (r == 0) {
-            tile[toff * GC + cw] = wA;                                  // id and type of the source; neither site is frozen
-            gtile[toff * GC + cw] = wA;                                 // home word in HBM
+            tile[pk_tbase(cw, TW) + toff * TS] = wA;                                  // id and type of the source; neither site is frozen
+            gtile[pk_tbase(cw, TW) + toff * TS] = wA;                                 // home word in HBM
             if constexpr (ACT)   // Max_act of the new owner; 0 for medium
               P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0);
             ++n_acc;
@@ -592,7 +599,10 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
                                  int *error_flag) {
   const int S = L.S, T = S + 2, TW = L.TW;
   const unsigned long long ngrp = (n_active + (unsigned long long)(PK_GC - 1)) >> PK_GS;
-  const int c = (int)(threadIdx.x & (PK_GC - 1));
+  // chain-major tiles: a warp writes one chain's contiguous tile; interleaved tiles: 8 consecutive threads = the 8 chains
+  const int c = PK_CHAIN_MAJOR ? (int)((threadIdx.x >> 5) & (PK_GC - 1)) : (int)(threadIdx.x & (PK_GC - 1));
+  const int j0 = PK_CHAIN_MAJOR ? (int)(threadIdx.x & 31) + 32 * (int)(threadIdx.x >> 8) : (int)(threadIdx.x >> PK_GS);
+  const int jstep = PK_CHAIN_MAJOR ? 32 * (int)(blockDim.x >> 8) : (int)(blockDim.x >> PK_GS);   // blockDim is a multiple of 256
   for (unsigned long long grp = blockIdx.x; grp < ngrp; grp += gridDim.x) {
     const unsigned long long w = grp * (unsigned long long)PK_GC + (unsigned long long)c;
     const bool live = w < n_active;   // the host keeps n_active below 2^31 for this layout
@@ -602,8 +612,8 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
     const int ay = (int)(r1 % (unsigned)L.nact[col][1]);
     const int az = (int)(r1 / (unsigned)L.nact[col][1]);
     const int x0 = (2 * ax + (col & 1)) * S - 1, y0 = (2 * ay + ((col >> 1) & 1)) * S - 1, z0 = (DIM == 3) ? (2 * az + ((col >> 2) & 1)) * S - 1 : 0;
-    uint32_t *out = L.tiles + L.base[col] + grp * (unsigned long long)TW * (unsigned long long)PK_GC + (unsigned long long)c;
-    for (int j = (int)(threadIdx.x >> PK_GS); j < TW; j += (int)(blockDim.x >> PK_GS)) {
+    uint32_t *out = L.tiles + L.base[col] + grp * (unsigned long long)TW * (unsigned long long)PK_GC + (unsigned long long)pk_tbase(c, TW);
+    for (int j = j0; j < TW; j += jstep) {
       uint32_t word = 0u;
       if (live) {
         int x = x0 + j % T, y = y0 + (j / T) % T, z = (DIM == 3) ? z0 + j / (T * T) : 0;
@@ -618,7 +628,7 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
           word = id | ((uint32_t)ctype[id] << PK_TYPE_SHIFT) | ((frozen && frozen[gi]) ? PK_FROZEN : 0u);
         }
       }
-      out[j * PK_GC] = word;
+      out[j * PK_TS] = word;
     }
   }
 }
@@ -652,7 +662,7 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
     uint32_t fid = 0;
     int fcnt = 0, ffor = 0, fsx = 0, fsy = 0, fsz = 0;
     if (w < n_active) {
-      const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (w & (unsigned long long)(PK_GC - 1));
+      const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (unsigned long long)pk_tbase((int)(w & (unsigned long long)(PK_GC - 1)), TW);
       const uint32_t w32 = (uint32_t)w;   // the host keeps n_active below 2^31 for this layout
       const int ax = (int)(w32 % (unsigned)L.nact[col][0]);
       const uint32_t r1 = w32 / (unsigned)L.nact[col][0];
@@ -672,7 +682,7 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
         for (int ly = 0; ly < S; ++ly)
           for (int lx = 0; lx < S; ++lx) {
             const int j = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-            const uint32_t word = tc[j * PK_GC];
+            const uint32_t word = tc[j * PK_TS];
             const uint32_t me = word & ID_MASK;
             const bool frozen = (word & PK_FROZEN) != 0u;
             if (!frozen && me != cur) { flush(cur, cv, cx, cy, cz); cur = me; cv = cx = cy = cz = 0; }
@@ -681,7 +691,7 @@ __global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_
             for (int nb = 0; nb < NNB; ++nb) {
               int dx, dy, dz;
               nb_delta<DIM>(nb, dx, dy, dz);
-              foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_GC] & ID_MASK) != me);
+              foreign += ((tc[(j + (dz * T + dy) * T + dx) * PK_TS] & ID_MASK) != me);
             }
             int qx = ox + lx, qy = oy + ly, qz = oz + lz;
             if (anc != nullptr) {   // reading S23: the image of the site nearest to the cell's anchor

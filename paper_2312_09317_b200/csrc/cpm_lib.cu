@@ -140,11 +140,12 @@ template <int DIM, int S>
 ThreadFn pick_pool_vec(bool act, bool live, bool vec, int nT, size_t *smem) {
   return vec ? pick_pool_flags<DIM, S, true>(act, live, nT, smem) : pick_pool_flags<DIM, S, false>(act, live, nT, smem);
 }
-// pooled kernel: 3D S = 2, 4; 2D S = 2, 4, 8, 16; one specialisation per extension set (L282)
+// pooled kernel: 3D S = 2, 4, 8; 2D S = 2, 4, 8, 16; one specialisation per extension set (L282)
 ThreadFn pick_pool_kernel(int d, int S, bool act, bool live, bool vec, int nT, size_t *smem) {
   if (d == 3) {
     if (S == 2) return pick_pool_vec<3, 2>(act, live, vec, nT, smem);
     if (S == 4) return pick_pool_vec<3, 4>(act, live, vec, nT, smem);
+    if (S == 8) return pick_pool_vec<3, 8>(act, live, vec, nT, smem);
     return nullptr;
   }
   if (S == 2) return pick_pool_vec<2, 2>(act, live, vec, nT, smem);

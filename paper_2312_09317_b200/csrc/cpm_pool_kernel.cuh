@@ -1,4 +1,4 @@
-// cpm_pool_kernel.cuh -- sm_100a sweep kernel for small power-of-two subsections (3D S = 2, 4; 2D S = 2..16):
+// cpm_pool_kernel.cuh -- sm_100a sweep kernel for small power-of-two subsections (3D S = 2, 4, 8; 2D S = 2..16):
 // one WARP owns a GROUP of 8 active checkerboard subsections ("chains") and evaluates their copy attempts
 // SPECULATIVELY IN PARALLEL, pooled over the 8 chains, while keeping the exact sequential semantics of every
 // chain (the attempts of one subsection are applied in order).  Warps never wait for one

@@ -189,7 +189,11 @@ def test_3d_shapes_schedules_boundaries(pk, oracle_mod, dims, S, k, periodic):
     if cfg["max_cells"] == 0:
         cfg = ci.make_config("C2", dims=dims, subsection=S)
         cfg["params"]["lambda_act"] = [0, 150, 90]; cfg["params"]["max_act"] = [0, 30, 12]
-    _run(pk, oracle_mod, cfg, 6, 2, act=True, attempts_per_activation=k, periodic=periodic)
+    g, _ = _run(pk, oracle_mod, cfg, 6, 2, act=True, attempts_per_activation=k, periodic=periodic)
+    assert g.get_launch_info()["pooled"] == (S in (2, 4, 8))
+    if S == 8:   # 3D S = 8 runs in the pooled kernel; the warp-per-subsection kernel is held to the same cases
+        g, _ = _run(pk, oracle_mod, cfg, 6, 2, act=True, attempts_per_activation=k, periodic=periodic, flags=pk.FLAG_WARP_KERNEL)
+        assert not g.get_launch_info()["pooled"]
 
 
 @pytest.mark.parametrize("dims,S,periodic", [
@@ -260,7 +264,8 @@ def test_resume_is_exact_on_device(pk, oracle_mod):
     ("C1", None, {}),                                              # pooled kernel, 2D S = 16
     ("C1", None, {"flags": 1}),                                    # warp-per-subsection kernel, TMA tile staging
     ("C3", (32, 32, 32), {"subsection": 4}),                       # pooled kernel, 3D S = 4, Act
-    ("C3", (32, 32, 32), {"subsection": 8}),                       # warp kernel, 3D S = 8, Act tiles
+    ("C3", (32, 32, 32), {"subsection": 8, "flags": 1}),           # warp kernel, 3D S = 8, Act tiles
+    ("C3", (32, 32, 32), {"subsection": 8}),                       # pooled kernel, 3D S = 8 (8 stretches of 64 attempts)
     ("C3", (32, 32, 32), {"subsection": 4, "mode": 1}),            # pooled kernel, live atomics
 ])
 def test_sanitizer_cases(pk, oracle_mod, name, dims, over):
@@ -282,7 +287,8 @@ def test_sanitizer_cases(pk, oracle_mod, name, dims, over):
 
 
 # ---- persistence (Eq 5-7) and chemotaxis (Eq 4) ----
-@pytest.mark.parametrize("dims,over", [((48, 48, 48), {}), ((40, 32, 24), {"subsection": 8}), ((32, 32, 32), {"subsection": 2}),
+@pytest.mark.parametrize("dims,over", [((48, 48, 48), {}), ((40, 32, 24), {"subsection": 8}), ((40, 32, 24), {"subsection": 8, "flags": 1}),
+                                       ((32, 32, 32), {"subsection": 2}),
                                        ((32, 32, 32), {"periodic": (1, 0, 1)})])
 def test_C6_persistence_collective_bit_exact(pk, oracle_mod, dims, over):
     """The paper's 3D persistence workload (Fig 5C / 6D, Table 2), scaled: lattice, tallies, counters AND the per-cell
@@ -290,7 +296,7 @@ def test_C6_persistence_collective_bit_exact(pk, oracle_mod, dims, over):
     import cpm_inputs as ci
     cfg = ci.make_config("C6", dims=dims)
     g, o = _run(pk, oracle_mod, cfg, 20, 1, **over)
-    assert g.get_launch_info()["pooled"] == (over.get("subsection", 4) != 8)
+    assert g.get_launch_info()["pooled"] == (over.get("flags", 0) == 0)
     p = g.get_persistence()[1:]
     nrm = np.linalg.norm(p, axis=1)
     assert (np.abs(nrm - 1) < 1e-12).mean() > 0.9      # nearly every cell has moved and carries a unit vector
@@ -349,7 +355,8 @@ def test_chemotaxis_3d_with_act_and_persistence_together(pk, oracle_mod):
 
 @pytest.mark.parametrize("name,dims,over", [
     ("C6", (32, 32, 32), {"periodic": (1, 1, 1)}),                       # pooled 3D + persistence through the border
-    ("C6", (32, 32, 32), {"periodic": (1, 0, 1), "subsection": 8}),      # warp kernel
+    ("C6", (32, 32, 32), {"periodic": (1, 0, 1), "subsection": 8, "flags": 1}),      # warp kernel
+    ("C6", (32, 32, 32), {"periodic": (1, 0, 1), "subsection": 8}),                  # pooled kernel, S = 8
     ("C7", (128, 128), {"periodic": (1, 1, 0)}),                         # pooled 2D + chemotaxis
     ("C5", (64, 96), {"periodic": (0, 1, 0), "subsection": 4}),
     ("C3", (32, 32, 32), {"periodic": (1, 1, 1), "subsection": 4, "mode": 0}),
@@ -425,7 +432,7 @@ def test_device_pointers_and_tma_off_give_same_result(pk, oracle_mod):
     out = torch.empty(gd.N, dtype=torch.int32, device="cuda")
     gd.get_lattice(out)
     np.testing.assert_array_equal(out.cpu().numpy().astype(np.uint32).reshape(o.shape), o.get_lattice())
-    gm = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], flags=pk.FLAG_NO_TMA, **cfg["params"])
+    gm = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], flags=pk.FLAG_NO_TMA | pk.FLAG_WARP_KERNEL, **cfg["params"])
     assert not gm.get_launch_info()["uses_tma"] and not gm.get_launch_info()["pooled"]
     gm.set_lattice(cfg["ids"], None, cfg["cell_type"])
     gm.step(3)
@@ -554,16 +561,16 @@ def test_errors_are_reported(pk):
     assert e.value.code == -1
 
 
-@pytest.mark.parametrize("S", [8, 4])
-def test_cell_table_overflow_is_flagged(pk, S):
+@pytest.mark.parametrize("S,flags", [(8, 1), (8, 0), (4, 0)])
+def test_cell_table_overflow_is_flagged(pk, S, flags):
     """Degenerate input: every voxel its own cell and T = inf, so one activation changes far
     more than 32 distinct cells -> the library reports CPM_ERR_UNSUPPORTED instead of silently
-    dropping deltas (warp kernel S = 8, thread kernel S = 4)."""
+    dropping deltas (warp kernel S = 8, pooled kernel S = 8 and 4)."""
     dims = (16, 16, 16)
     n = 16 ** 3
     ids = np.arange(1, n + 1, dtype=np.uint32).reshape(16, 16, 16)
     ct = np.ones(n + 1, np.uint8); ct[0] = 0
-    g = pk.CPM(dims, J=[[0, 1], [1, 1]], lambda_V=[0, 0], target_V=[0, 0], max_cells=n, T=float("inf"), subsection=S)
+    g = pk.CPM(dims, J=[[0, 1], [1, 1]], lambda_V=[0, 0], target_V=[0, 0], max_cells=n, T=float("inf"), subsection=S, flags=flags)
     # volume-1 cells cannot be erased (S13); give them volume 2 by pairing voxels along x
     ids = ((ids - 1) // 2 + 1).astype(np.uint32)
     g.set_lattice(ids, None, ct)
@@ -573,17 +580,17 @@ def test_cell_table_overflow_is_flagged(pk, S):
     assert e.value.code == -3
 
 
-@pytest.mark.parametrize("S", [8, 4])
-def test_many_cells_looked_at_few_changed(pk, oracle_mod, S):
+@pytest.mark.parametrize("S,flags", [(8, 1), (8, 0), (4, 0)])
+def test_many_cells_looked_at_few_changed(pk, oracle_mod, S, flags):
     """Reading R2 counts the cells a subsection CHANGES in one activation, not the ones it looks at: 2-voxel cells (far more
     than 32 in the reach of one subsection) at a temperature where few copies are accepted run without an overflow and
-    equal the oracle (warp kernel S = 8, pooled kernel S = 4)."""
+    equal the oracle (warp kernel S = 8, pooled kernel S = 8 and 4)."""
     dims = (16, 16, 16)
     n = 16 ** 3 // 2
     ids = ((np.arange(16 ** 3, dtype=np.uint32).reshape(16, 16, 16)) // 2 + 1).astype(np.uint32)
     ct = np.ones(n + 1, np.uint8); ct[0] = 0
     kw = dict(J=np.zeros((2, 2), dtype=np.int32), lambda_V=[0, 3], target_V=[0, 2], max_cells=n, T=1.0, subsection=S, seed=3)
-    g = pk.CPM(dims, **kw); o = oracle_mod.Oracle(dims, **kw)
+    g = pk.CPM(dims, flags=flags, **kw); o = oracle_mod.Oracle(dims, **kw)
     g.set_lattice(ids, None, ct); o.set_lattice(ids, None, ct)
     g.step(3); o.step(3)
     _compare(g, o, False, "many cells looked at")

@@ -399,6 +399,27 @@ def test_interface_counts_equal_oracle(pk, oracle_mod, name, dims, over):
     assert C.sum() > 0 and (C == C.T).all()
 
 
+def test_cell_sorting_trend_in_interface_counts(pk, oracle_mod):
+    """The paper's validation workload (Fig 4, L69, after Graner and Glazier): two cell types that adhere to their own kind
+    more strongly than to the other kind sort out: heterotypic interfaces fall, homotypic ones rise.  The trend is read with
+    cpm_get_interface_counts every 250 MCS over 1 770 MCS and equals the oracle's at every read-out (deterministic mode)."""
+    import cpm_inputs as ci
+    cfg = ci.make_config("C5", dims=(128, 128), subsection=8)
+    J = np.array([[0, 16, 16], [16, 2, 30], [16, 30, 14]], dtype=np.int32)   # J(1,2) > (J(1,1) + J(2,2)) / 2: sorting
+    cfg["params"].update(J=J, T=20.0)
+    g, o = _pair(pk, oracle_mod, cfg)
+    g.step(20); o.step(20)          # the seeds grow into contact
+    het, hom = [], []
+    for it in range(8):
+        Cg, Co = g.get_interface_counts(), o.get_interface_counts()
+        np.testing.assert_array_equal(Cg, Co)
+        het.append(int(Cg[1, 2])); hom.append(int(Cg[1, 1] + Cg[2, 2]))
+        if it < 7:
+            g.step(250); o.step(250)
+    assert het[-1] < 0.9 * het[0] and hom[-1] > 1.1 * hom[0], (het, hom)
+    _compare(g, o, False, "sorting run")
+
+
 @pytest.mark.parametrize("dims,S,k,periodic", [((16, 16), 16, 256, (0, 0, 0)), ((16, 16), 2, 4, (0, 0, 0)), ((64, 48), 8, 16, (0, 0, 0)),
                                                ((16, 16, 16), 4, 64, (0, 0, 0)), ((8, 24, 8), 8, 128, (0, 0, 0))])
 def test_update_statistics_equal_oracle(pk, oracle_mod, dims, S, k, periodic):

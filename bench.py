@@ -74,7 +74,7 @@ class ClockSampler:
         try:
             self.f = open(self.path, "w")
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
                                          stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
@@ -138,7 +138,8 @@ def static_capture(config, dims, S):
                 if r.get("source_hash") != cur:
                     return None, "stale: %s was captured on sources %s, timed sources are %s" % (r.get("source"), r.get("source_hash"), cur), None
                 wipa = float(r["warp_instr_per_attempt"]) if r.get("warp_instr_per_attempt") else None
-                return int(r["dram_bytes_per_sweep_launch"]), "static ncu capture %s (sources %s)" % (r.get("source"), cur), {"warp_instr_per_attempt": wipa}
+                alu = float(r["alu_pipe_active_pct_under_ncu"]) if r.get("alu_pipe_active_pct_under_ncu") else None
+                return int(r["dram_bytes_per_sweep_launch"]), "static ncu capture %s (sources %s)" % (r.get("source"), cur), {"warp_instr_per_attempt": wipa, "alu_pipe_active_pct_under_ncu": alu}
     except Exception:
         pass
     return None, "no capture for this workload", None
@@ -372,10 +373,12 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-resident throughput ----
-    g.step(args.warmup)
-    barrier()
+    # the clock sampler starts before the burn-in (the same kernels on the same workload) so that nvidia-smi is already
+    # polling when the timed region, a fraction of a second long, begins; it stops after the graph replay
     sampler = ClockSampler(local)
     sampler.start()
+    g.step(args.warmup)
+    barrier()
     g.set_kernel_timing(True)
     l0 = g.get_launch_info()["launches"]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -387,7 +390,6 @@ def main():
     sweep_ms, sweep_n = g.get_kernel_timing(reset=True)
     g.set_kernel_timing(False)
     launches = g.get_launch_info()["launches"] - l0
-    clocks = sampler.stop()
     counters = g.get_counters()
     # the same K steps again the way cpm_step runs them for a user: one CUDA graph per MCS, no per-launch events
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -396,6 +398,7 @@ def main():
     g1.record()
     barrier()
     graph_ms = g0.elapsed_time(g1)
+    clocks = sampler.stop()
     graph_window = [args.warmup + args.steps + 1, args.warmup + 2 * args.steps]   # later MCS than the timed region: the workload relaxes
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the inputs, MCS, D2H of the lattice ----
@@ -452,7 +455,7 @@ def main():
                 "frac_layout_bytes": layout_bpa * attempts_per_launch / avg_launch_s / 1e9 / peak,
                 "layout_bytes_per_attempt": layout_bpa,
                 # what limits the kernel today is not HBM: issue slots and barrier latency
-                "limiter": "issue/latency (DESIGN.md section 7), not HBM"}
+                "limiter": "integer alu pipe and instruction issue (DESIGN.md section 7), not HBM"}
         if prof and prof.get("warp_instr_per_attempt"):
             # the plain-ALU side SURVEY.md 8(d) asks for: warp-instructions issued per second against
             # SMs x 4 schedulers x SM clock (one warp-instruction per scheduler and cycle)
@@ -462,6 +465,7 @@ def main():
                            "achieved": prof["warp_instr_per_attempt"] * attempts_per_launch / avg_launch_s,
                            "peak": issue_peak, "unit": "warp-instr/s",
                            "frac": prof["warp_instr_per_attempt"] * attempts_per_launch / avg_launch_s / issue_peak,
+                           "alu_pipe_active_pct_under_ncu": prof.get("alu_pipe_active_pct_under_ncu"),
                            "source": traffic_src}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -7,6 +7,8 @@
 #include "cpm_pool_kernel.cuh"
 #include "cpm_stats_kernels.cuh"
 
+#include <nvtx3/nvToolsExt.h>   // header-only: ranges around the API calls for nsys / ncu timelines
+
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -16,6 +18,13 @@
 #include <vector>
 
 using namespace cpm;
+
+namespace {
+struct NvtxRange {   // RAII range on the calling thread
+  explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -643,6 +652,7 @@ int cpm_destroy(cpm_ctx *c) {
 int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, const uint8_t *cell_type, int on_device) {
   if (!c) return CPM_ERR_ARG;
   if (!ids || !cell_type) return fail(c, CPM_ERR_ARG, "ids and cell_type are required");
+  NvtxRange nvtx("cpm_set_lattice");
   CPM_GUARD_BEGIN
   CK(cudaSetDevice(c->device));
   const size_t ncell = (size_t)c->max_cells + 1;
@@ -806,6 +816,7 @@ int cpm_set_mcs(cpm_ctx *c, uint32_t mcs) {
 int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
   if (!c) return CPM_ERR_ARG;
   if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  NvtxRange nvtx("cpm_step");
   CPM_GUARD_BEGIN
   CK(cudaSetDevice(c->device));
   // per-launch events need the plain launch sequence; otherwise one graph launch per MCS
@@ -828,6 +839,7 @@ int cpm_step(cpm_ctx *c, uint32_t n_mcs) {
 
 int cpm_get_lattice(cpm_ctx *c, uint32_t *ids, int on_device) {
   if (!c || !ids) return fail(c, CPM_ERR_ARG, "null argument");
+  NvtxRange nvtx("cpm_get_lattice");
   CK(cudaSetDevice(c->device));
   uint32_t *s;
   CK(stage_out_begin(&s, &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device));

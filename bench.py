@@ -467,6 +467,7 @@ def main():
                            "peak": issue_peak, "unit": "warp-instr/s",
                            "frac": prof["warp_instr_per_attempt"] * attempts_per_launch / avg_launch_s / issue_peak,
                            "alu_pipe_active_pct_under_ncu": prof.get("alu_pipe_active_pct_under_ncu"),
+                           "note": "warp_instr_per_attempt is the static capture's (one launch of MCS 11); later MCS evaluate and accept fewer attempts, so this fraction is an upper estimate for a window that extends beyond MCS 20",
                            "source": traffic_src}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -112,12 +112,12 @@ class ClockSampler:
 
 
 def source_hash():
-    """SHA-256 over the device sources (csrc/*.cuh) the kernels are built from: ties a stored ncu figure to the code it
-    was taken on."""
+    """SHA-256 over the sources of the sweep kernels (cpm_device.cuh, cpm_pool_kernel.cuh): ties a stored ncu figure
+    to the code it was taken on."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2312_09317_b200", "csrc")
-    for name in sorted(n for n in os.listdir(d) if n.endswith(".cuh")):   # the device code; cpm_lib.cu is host code
+    for name in ("cpm_device.cuh", "cpm_pool_kernel.cuh"):   # the files the sweep kernels are made of
         with open(os.path.join(d, name), "rb") as f:
             h.update(name.encode()); h.update(f.read())
     return h.hexdigest()[:16]

@@ -922,8 +922,10 @@ int cpm_get_interface_counts(cpm_ctx *c, uint64_t *out) {
   V.lat = c->lat; V.pitch = c->sp.pitch; V.tl = c->sp.tl; V.pooled = c->pooled ? 1 : 0;
   V.X = c->dim[0]; V.Y = c->dim[1]; V.Z = c->dim[2];
   for (int a = 0; a < 3; ++a) V.per[a] = c->per[a];
-  if (c->d == 2) interface_count_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(V, c->nT, d);
-  else interface_count_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(V, c->nT, d);
+  const int use_smem = n * 8 <= 32768 ? 1 : 0;   // block-local counts for up to 64 types, else global atomics only
+  const size_t shm = use_smem ? n * 8 : 0;
+  if (c->d == 2) interface_count_kernel<2><<<grid_for(c->N), 256, shm, c->stream>>>(V, c->nT, d, use_smem);
+  else interface_count_kernel<3><<<grid_for(c->N), 256, shm, c->stream>>>(V, c->nT, d, use_smem);
   c->launches++;
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(out, d, n * 8, cudaMemcpyDeviceToHost, c->stream));

@@ -28,8 +28,14 @@ __device__ __forceinline__ void site_at(const LatView &V, int x, int y, int z, u
 // outside a closed lattice is medium (reading S5).  An inside pair is met from both ends and counted from the end
 // whose offset index is in the upper half; equal (type, type) keys of a warp are combined before the atomics.
 template <int DIM>
-__global__ void interface_count_kernel(LatView V, int nT, unsigned long long *out) {
+__global__ void interface_count_kernel(LatView V, int nT, unsigned long long *out, int use_smem) {
   constexpr int NNB = (DIM == 2) ? 8 : 26;
+  extern __shared__ unsigned long long hist[];   // block-local counts [nT][nT] (use_smem), flushed once per block
+  if (use_smem) {
+    for (int i = threadIdx.x; i < nT * nT; i += blockDim.x) hist[i] = 0ull;
+    __syncthreads();
+  }
+  unsigned long long *const acc = use_smem ? hist : out;
   const long long N = (long long)V.X * V.Y * V.Z;
   const long long stride = (long long)gridDim.x * blockDim.x;
   const long long first = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -66,11 +72,16 @@ __global__ void interface_count_kernel(LatView V, int nT, unsigned long long *ou
       const unsigned peers = __match_any_sync(FULL, key);
       if (key >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) {
         const unsigned long long n = (unsigned long long)__popc(peers);
-        atomicAdd(out + key, n);
+        atomicAdd(acc + key, n);
         const int a = key / nT, b = key % nT;
-        if (a != b) atomicAdd(out + b * nT + a, n);
+        if (a != b) atomicAdd(acc + b * nT + a, n);
       }
     }
+  }
+  if (use_smem) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < nT * nT; i += blockDim.x)
+      if (hist[i] != 0ull) atomicAdd(out + i, hist[i]);
   }
 }
 

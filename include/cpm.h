@@ -147,7 +147,7 @@ int  cpm_update_statistics(cpm_ctx *ctx, uint32_t n_mcs, uint64_t *freq, int32_t
 int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);
 /* Introspection: kernels launched by this context so far, and the launch geometry of the sweep
  * kernel: out = {launches, sweep_launches, warps_per_cta, smem_bytes_per_cta, uses_tma,
- * pooled (1: pooled kernel on the tiled lattice layout -- one warp per group of 32 subsections,
+ * pooled (1: pooled kernel on the tiled lattice layout -- one warp per group of 8 subsections,
  * small power-of-two S; 0: one warp per subsection on the row-major layout)}. */
 int  cpm_get_launch_info(cpm_ctx *ctx, uint64_t out[6]);
 /* Average device time (ms) of the sweep kernel launches since the last call with reset != 0,

@@ -1,6 +1,10 @@
-// cpm_device.cuh -- sm_100a device code of the checkerboard CPM sweep.
+// cpm_device.cuh -- sm_100a device code of the checkerboard CPM sweep: parameter blocks, PTX wrappers (mbarrier, TMA),
+// Philox4x32-10, the pieces both sweep kernels share (Act side, vector-term bias, periodic image), the
+// WARP-PER-SUBSECTION kernel (larger or non-power-of-two subsections, > 8 cell types) and the auxiliary kernels
+// (Act decay, snapshot, pack / unpack / recount of the row-major layout, persistence, centroid tracking).  The
+// pooled kernel for small subsections lives in cpm_pool_kernel.cuh, the instrumentation in cpm_stats_kernels.cuh.
 //
-// One WARP owns one active checkerboard subsection for one activation:
+// Warp-per-subsection kernel: one WARP owns one active checkerboard subsection for one activation:
 //   a2  id tile + halo staged into shared memory by TMA (cp.async.bulk.tensor, OOB zero-fill =
 //       "outside is medium"), completion on a per-warp mbarrier.  TMA needs the innermost start
 //       coordinate at a 16-byte boundary (measured on B200: a 4-byte-aligned start raises
@@ -33,9 +37,9 @@ struct __align__(16) TypeParams {  // per cell type, Tables 1-3 of the paper
 };
 
 // Tiled lattice layout of the pooled kernel (cpm_pool_kernel.cuh): every subsection owns a tile of (S+2)^d
-// words (its sites + a halo replicated from its neighbours); the tiles of 32 same-colour subsections
+// words (its sites + a halo replicated from its neighbours); the tiles of 8 same-colour subsections
 // (consecutive in the active-subsection order w) are interleaved: word j of subsection w of colour col at
-// base[col] + (((w >> 5) * TW + j) << 5) + (w & 31).
+// base[col] + (((w >> 3) * TW + j) << 3) + (w & 7) (or chain-major, see PK_CHAIN_MAJOR in cpm_pool_kernel.cuh).
 struct TileLayout {
   uint32_t *tiles;
   unsigned long long base[8];   // word offset of the first group of each colour
@@ -65,7 +69,7 @@ struct SweepParams {
   int tile_bytes, act_tile_bytes, warp_smem_bytes;
   int use_tma;
   const int32_t *J; int nT;
-  const int32_t *D;         // thread kernel: [nT^3] J(a,n) - J(b,n), then [nT] J(t,t)
+  const int32_t *D;         // pooled kernel: [nT][nT][nT][2] J(a,n) - J(b,n), then [nT] J(t,t)
   const TypeParams *types;
   const uint32_t *thr; long long Hmax; int accept_all;
   const int32_t *logq16;    // [256]

@@ -55,7 +55,7 @@ struct cpm_ctx {
   SweepFn fn = nullptr;
   bool pooled = false;          // pooled kernel on the tiled layout (small power-of-two S), else one warp per subsection
   ThreadFn tfn = nullptr;
-  unsigned long long n_act_col[8] = {0}, grp_col[8] = {0};   // active subsections / groups of 32 per colour
+  unsigned long long n_act_col[8] = {0}, grp_col[8] = {0};   // active subsections / groups of 8 per colour
   size_t tile_words = 0;
   SweepParams sp;        // template of the launch parameters
   CUtensorMap tm_lat;
@@ -448,7 +448,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->tfn = (nT <= 8 && !(p->flags & CPM_FLAG_WARP_KERNEL))
                ? pick_pool_kernel(d, S, c->act_enabled, p->mode == CPM_MODE_LIVE_ATOMICS, pers_on || chem_on || c->unwrap, nT, &pool_smem) : nullptr;
   c->pooled = c->tfn != nullptr;
-  if (c->pooled) c->use_tma = true;   // one bulk copy per group of 32 tiles
+  if (c->pooled) c->use_tma = true;   // one bulk copy per group of 8 tiles
 
   // ---- tile geometry (a2) ----
   SweepParams &sp = c->sp;
@@ -511,7 +511,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
         for (int f = 0; f < 2; ++f) Dtab[(((size_t)a * nT + b2) * nT + n) * 2 + f] = p->J[a * nT + n] - p->J[b2 * nT + n];
   for (int t = 0; t < nT; ++t) Dtab[(size_t)2 * nT * nT * nT + t] = p->J[t * nT + t];
 
-  // ---- tiled layout of the pooled kernel: per colour, groups of 32 tiles of (S+2)^d words ----
+  // ---- tiled layout of the pooled kernel: per colour, groups of 8 tiles of (S+2)^d words ----
   TileLayout &tl = sp.tl;
   tl.S = S; tl.TW = 1;
   for (int a = 0; a < d; ++a) tl.TW *= S + 2;

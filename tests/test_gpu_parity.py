@@ -179,9 +179,9 @@ def test_C5_scaled_subsection_sweep(pk, oracle_mod, S):
     ((32, 16, 16), 8, 0, (0, 1, 0)),      # mixed boundary, a single subsection pair
     ((8, 8, 8), 8, 0, (0, 0, 0)),         # one subsection: most colours are empty
     ((16, 16, 16), 2, 0, (0, 0, 0)),      # smallest subsection
-    ((32, 24, 16), 4, 0, (1, 1, 1)),      # thread kernel, periodic wrap of halo words and rows
-    ((24, 16, 8), 4, 16, (0, 1, 0)),      # thread kernel, k < S^d, mixed boundary
-    ((24, 16, 8), 2, 0, (1, 0, 1)),       # thread kernel, S = 2, periodic
+    ((32, 24, 16), 4, 0, (1, 1, 1)),      # pooled kernel, periodic wrap of halo words and rows
+    ((24, 16, 8), 4, 16, (0, 1, 0)),      # pooled kernel, k < S^d, mixed boundary
+    ((24, 16, 8), 2, 0, (1, 0, 1)),       # pooled kernel, S = 2, periodic
 ])
 def test_3d_shapes_schedules_boundaries(pk, oracle_mod, dims, S, k, periodic):
     import cpm_inputs as ci

@@ -139,3 +139,38 @@ def test_C4_full_size_equals_oracle_and_properties(pk, golden):
     st2 = g2.get_cell_stats()
     for k in st:
         np.testing.assert_array_equal(st[k], st2[k])
+
+
+# ---- every other workload at its full size and run length (tests/golden/make_baseline_checksums.py) ----
+def _baseline_tools():
+    spec = importlib.util.spec_from_file_location("make_baseline_checksums", os.path.join(GOLDEN_DIR, "make_baseline_checksums.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod
+
+
+@pytest.mark.parametrize("key", ["C2", "C3", "C5_S16", "C5_S32", "C6", "C7"])
+def test_workloads_at_full_size_and_length_equal_oracle_checksums(pk, key):
+    """BASELINE configs 2, 3, 5 and the SURVEY 8(f) workloads C6, C7 at the sizes and run lengths BASELINE.json / the paper
+    name (C2: 256^3 x 200 MCS, C3: 256^3 x 500 MCS with Act, C5: 16384^2 at S = 16 and 32, C6: 256^3 x 100 MCS with
+    persistence, C7: 1024^2 x 100 MCS with chemotaxis): at every checkpoint (every 10 MCS for C2) the SHA-256
+    of every array the C ABI reads back -- lattice, Act, V, P, coordinate sums, persistence doubles, counters -- equals
+    the oracle's, recorded by the committed script that calls only oracle/."""
+    tools = _baseline_tools()
+    with open(os.path.join(GOLDEN_DIR, "baseline_oracle_checksums.json")) as f:
+        rec = json.load(f)[key]
+    cfg, params, checkpoints = tools.build(key)
+    assert tools.input_record(cfg) == rec["inputs"], "generated inputs differ from the ones the golden run used"
+    act, pers = tools.flags_of(cfg)
+    g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], **params)
+    g.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
+    if cfg.get("field") is not None:
+        g.set_chemotaxis_field(cfg["field"])
+    assert g.get_schedule() == rec["schedule"]
+    done = 0
+    for m in sorted(int(k) for k in rec["mcs"]):
+        g.step(m - done)
+        done = m
+        got, want = tools.state_record(g, act, pers), rec["mcs"][str(m)]
+        for k2 in want:
+            assert got[k2] == want[k2], "%s after %d MCS: %s differs from the oracle's checksum" % (key, m, k2)

@@ -126,6 +126,11 @@ int  cpm_get_act(cpm_ctx *ctx, float *act, int on_device);
  * (only an obstacle id owning > 1.6e8 surface-like voxels could) would carry into its volume -- outside this build. */
 int  cpm_get_cell_stats(cpm_ctx *ctx, uint32_t *volume, uint32_t *perimeter,
                         uint64_t *sum_x, uint64_t *sum_y, uint64_t *sum_z, int on_device);
+/* Centroid of every cell (Eq 10): xyz[(max_cells+1)][3] doubles = coordinate sums / volume, one IEEE division each,
+ * computed on the device from the integer tallies (never accumulated in floating point, L288); (0,0,0) for ids without
+ * sites and for medium.  With unwrap_centroids the centroid of a cell that straddles a periodic border lies inside
+ * [0, dim) at the cell's true position on the torus. */
+int  cpm_get_centroids(cpm_ctx *ctx, double *xyz, int on_device);
 /* out (host) = {attempts, evaluated, accepted, mcs}. */
 int  cpm_get_counters(cpm_ctx *ctx, uint64_t out[4]);
 int  cpm_get_schedule(cpm_ctx *ctx, int32_t *S, int32_t *k, int32_t *phase_steps_per_mcs);

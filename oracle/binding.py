@@ -84,6 +84,7 @@ def lib():
         L.oracle_set_persistence.argtypes = [vp, vp]
         L.oracle_get_persistence.argtypes = [vp, vp]
         L.oracle_probe_dir.argtypes = [vp, C.c_uint64, C.c_int32, vp]
+        L.oracle_get_centroids.argtypes = [vp, vp]
         L.oracle_direction_table.argtypes = [C.c_int32, vp]
         L.oracle_get_interface_counts.argtypes = [vp, vp]
         L.oracle_update_statistics.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32]
@@ -243,6 +244,11 @@ class Oracle:
     def get_persistence(self):
         out = np.empty((self.max_cells + 1, 3), dtype=np.float64)
         self._chk(self._L.oracle_get_persistence(self._h, out.ctypes.data))
+        return out
+
+    def get_centroids(self):
+        out = np.empty((self.max_cells + 1, 3), dtype=np.float64)
+        self._chk(self._L.oracle_get_centroids(self._h, out.ctypes.data))
         return out
 
     def probe_dir(self, t_index, nb):

@@ -823,6 +823,17 @@ int oracle_get_persistence(oracle_ctx *c, double *p) {
   return ORACLE_OK;
 }
 
+/* Eq 10: centroid = coordinate sums / number of sites, in double; (0,0,0) for ids that hold no site */
+int oracle_get_centroids(oracle_ctx *c, double *xyz) {
+  if (!c || !xyz) return ORACLE_ERR_ARG;
+  for (size_t cell = 0; cell <= c->max_cells; ++cell) {
+    double X[3] = {0.0, 0.0, 0.0};
+    if (cell != 0 && c->V[cell] > 0) centroid(c, cell, X);
+    for (int a = 0; a < 3; ++a) xyz[3 * cell + a] = X[a];
+  }
+  return ORACLE_OK;
+}
+
 int oracle_probe_dir(oracle_ctx *c, uint64_t t_index, int32_t nb, int64_t *dH_dir) {
   if (!c || nb < 0 || nb >= c->nNb || t_index >= c->id.size() || !dH_dir) return ORACLE_ERR_ARG;
   int tx = (int)(t_index % c->dim[0]);

@@ -83,6 +83,8 @@ int  oracle_set_chemotaxis_field(oracle_ctx *c, const float *field);
 /* p[(max_cells+1)][3]: persistence direction per cell (unit or zero vectors); default 0 after set_lattice */
 int  oracle_set_persistence(oracle_ctx *c, const double *p);
 int  oracle_get_persistence(oracle_ctx *c, double *p);
+/* xyz[(max_cells+1)][3]: centroid of every cell, Eq 10 (coordinate sums / volume) */
+int  oracle_get_centroids(oracle_ctx *c, double *xyz);
 /* the integer chemotaxis + persistence bias that is SUBTRACTED from dH for this copy (0 for early-outs) */
 int  oracle_probe_dir(oracle_ctx *c, uint64_t t_index, int32_t nb, int64_t *dH_dir);
 /* Q14 unit vectors of the copy direction (source -> target) per neighbour index: out[nb*3 + {0,1,2}] */

@@ -82,6 +82,7 @@ def load_library():
     L.cpm_get_act.argtypes = [vp, vp, C.c_int]
     L.cpm_get_cell_stats.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
     L.cpm_get_counters.argtypes = [vp, vp]
+    L.cpm_get_centroids.argtypes = [vp, vp, C.c_int]
     L.cpm_get_schedule.argtypes = [vp, vp, vp, vp]
     L.cpm_get_interface_counts.argtypes = [vp, vp]
     L.cpm_update_statistics.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32]
@@ -255,6 +256,13 @@ class CPM:
         self._chk(self._L.cpm_get_cell_stats(self._h, V.ctypes.data, P.ctypes.data, sx.ctypes.data,
                                              sy.ctypes.data, sz.ctypes.data, 0))
         return {"volume": V, "perimeter": P, "sum_x": sx, "sum_y": sy, "sum_z": sz}
+
+    def get_centroids(self, out=None):
+        if out is None:
+            out = np.empty(3 * (self.max_cells + 1), dtype=np.float64)
+        po, do, ko = _ptr(out, np.float64, 3 * (self.max_cells + 1))
+        self._chk(self._L.cpm_get_centroids(self._h, po, do))
+        return ko.reshape(self.max_cells + 1, 3)
 
     def get_counters(self):
         out = np.zeros(4, np.uint64)

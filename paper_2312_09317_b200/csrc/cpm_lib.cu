@@ -889,6 +889,20 @@ int cpm_get_cell_stats(cpm_ctx *c, uint32_t *volume, uint32_t *perimeter, uint64
   return check_device_flag(c);
 }
 
+int cpm_get_centroids(cpm_ctx *c, double *xyz, int on_device) {
+  if (!c || !xyz) return fail(c, CPM_ERR_ARG, "null argument");
+  if (!c->have_lattice) return fail(c, CPM_ERR_STATE, "cpm_set_lattice first");
+  CK(cudaSetDevice(c->device));
+  const size_t n = (size_t)c->max_cells + 1;
+  double *s;
+  CK(stage_out_begin(&s, &c->stage_a, &c->stage_a_cap, xyz, n * 3, on_device));
+  centroid_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((long long)n, c->liveVP, c->sumx, c->sumy, c->sumz, s);
+  c->launches++;
+  CK(cudaGetLastError());
+  CK(stage_out_end(s, xyz, n * 3, on_device, c->stream));
+  return check_device_flag(c);
+}
+
 int cpm_get_counters(cpm_ctx *c, uint64_t out[4]) {
   if (!c || !out) return fail(c, CPM_ERR_ARG, "null argument");
   CK(cudaSetDevice(c->device));

@@ -85,6 +85,17 @@ __global__ void interface_count_kernel(LatView V, int nT, unsigned long long *ou
   }
 }
 
+// Eq 10: centroid = coordinate sums / volume (one IEEE division per component)
+__global__ void centroid_kernel(long long ncell, const unsigned long long *liveVP, const unsigned long long *sumx,
+                                const unsigned long long *sumy, const unsigned long long *sumz, double *xyz) {
+  const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cell >= ncell) return;
+  double X[3] = {0.0, 0.0, 0.0};
+  const unsigned long long vp = liveVP[cell];
+  if (cell != 0 && (uint32_t)(vp >> 32) != 0u) centroid_of(vp, sumx[cell], sumy[cell], sumz[cell], X);
+  xyz[3 * cell] = X[0]; xyz[3 * cell + 1] = X[1]; xyz[3 * cell + 2] = X[2];
+}
+
 // Update statistics: one thread per subsection walks the target picks of its own activations over n_mcs MCS (proposal
 // stream of the sweep: Philox counter (a>>2, b, 2p, mcs), word a&3, multiply-shift decode), in lock-step ticks
 // (m E + e) k + a, E = non-empty phase-steps per MCS.  last / cnt: per-site scratch (N words each), only ever touched

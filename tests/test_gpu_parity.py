@@ -39,6 +39,7 @@ def _compare(g, o, act=False, tag=""):
         np.testing.assert_array_equal(sg[k], so[k], err_msg="%s %s" % (tag, k))
     if act:
         np.testing.assert_array_equal(g.get_act(), o.get_act(), err_msg=tag + " act")
+    np.testing.assert_array_equal(g.get_centroids(), o.get_centroids(), err_msg=tag + " centroids")   # Eq 10, one division each
     if getattr(o, "pers_on", False):   # Eq 6-7 in IEEE double on both sides: equal to the last bit
         np.testing.assert_array_equal(g.get_persistence(), o.get_persistence(), err_msg=tag + " persistence")
     assert g.get_counters() == o.get_counters(), (tag, g.get_counters(), o.get_counters())

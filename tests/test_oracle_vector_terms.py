@@ -241,6 +241,8 @@ def _circular_centroids(lat, n_cells, dims, periodic):
 
 def _check_tracked_centroids(o, n_cells, dims, periodic, tag):
     st = o.get_cell_stats()
+    v = st["volume"].astype(np.float64); v[v == 0] = np.inf     # Eq 10: sums / volume
+    np.testing.assert_array_equal(o.get_centroids(), np.stack([st[k].astype(np.int64) / v for k in ("sum_x", "sum_y", "sum_z")], axis=1))
     want, vol = _circular_centroids(o.get_lattice(), n_cells, dims, periodic)
     np.testing.assert_array_equal(st["volume"][1:], vol[1:])
     dimv = [dims[0], dims[1], dims[2] if len(dims) == 3 else 1]

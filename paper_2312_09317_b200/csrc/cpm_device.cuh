@@ -57,6 +57,7 @@ struct SweepParams {
   int S, log2S, sites, k;   // subsection edge, log2 (or -1), S^d, attempts per activation
   int nsub[3];              // subsections per axis
   int nact[3];              // active subsections per axis for this colour
+  uint32_t nact_mul[2], nact_shr[2];   // w / nact[a] = umulhi(w, mul) >> shr for w < 2^31 (host-built; mul = 0: nact[a] = 1)
   int col[3];               // colour bits of this phase-step
   unsigned long long n_active;
   uint32_t p;               // phase-step index rep*2^d + colour
@@ -91,6 +92,7 @@ struct SweepParams {
   const short4 *pq;                  // [max_cells + 1] persistence direction of the cell (null: persistence off)
   const short4 *chem;                // [N] chemotaxis field, row-major x fastest (null: no field loaded)
   int xq_len[3];                     // llround(16384 / sqrt(n)), n = 1, 2, 3: component of the unit copy direction
+  const unsigned char *img; int img_bytes;   // pooled kernel: per-type records + adhesion table as they sit in shared memory (one bulk copy)
   const int *anc;                    // [max_cells + 1][3] anchors of the periodic centroid tracking (reading S23); null: off
 };
 

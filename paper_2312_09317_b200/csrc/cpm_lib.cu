@@ -70,6 +70,9 @@ struct cpm_ctx {
   uint32_t *mcs_dev = nullptr;
   int32_t *J_dev = nullptr, *D_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
   TypeParams *types_dev = nullptr;
+  unsigned char *img_dev = nullptr;   // pooled kernel: types + adhesion table as one shared-memory image
+  size_t img_bytes = 0;
+  std::vector<int32_t> Dtab;
   uint32_t *thr_dev = nullptr;
   uint32_t *ovf_keys = nullptr;
   unsigned long long *ovf_dvp = nullptr;
@@ -255,6 +258,13 @@ int upload_types(cpm_ctx *c, int user_values) {
     t.cap = (int32_t)std::min<long long>(cap, 0x3fffffffLL);
   }
   cudaError_t e = cudaMemcpyAsync(c->types_dev, c->types.data(), c->types.size() * sizeof(TypeParams), cudaMemcpyHostToDevice, c->stream);
+  std::vector<unsigned char> img;
+  if (e == cudaSuccess && c->img_dev) {   // the same records, followed by the adhesion table, as the pooled kernel's shared memory holds them
+    img.assign(c->img_bytes, 0);
+    memcpy(img.data(), c->types.data(), c->types.size() * sizeof(TypeParams));
+    memcpy(img.data() + c->types.size() * sizeof(TypeParams), c->Dtab.data(), c->Dtab.size() * 4);
+    e = cudaMemcpyAsync(c->img_dev, img.data(), c->img_bytes, cudaMemcpyHostToDevice, c->stream);
+  }
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   return e == cudaSuccess ? CPM_OK : fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
 }
@@ -266,7 +276,7 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
   cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
   cudaFree(c->vec_types_dev); cudaFree(c->mu_dev); cudaFree(c->phat); cudaFree(c->ring); cudaFree(c->pq); cudaFree(c->chem);
-  cudaFree(c->ctype_dev); cudaFree(c->pers_n); cudaFree(c->anc); cudaFree(c->first_site);
+  cudaFree(c->img_dev); cudaFree(c->ctype_dev); cudaFree(c->pers_n); cudaFree(c->anc); cudaFree(c->first_site);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -289,6 +299,17 @@ int enqueue_mcs(cpm_ctx *c, cudaStream_t st, bool timed) {
       }
       if (n_active == 0) continue;  // this colour does not occur (a single subsection along an axis)
       sp.n_active = n_active;
+      for (int a = 0; a < 2; ++a) {   // exact reciprocal for dividends below 2^31 (Granlund-Montgomery): m = ceil(2^(31+l) / d), l = ceil(log2 d)
+        const uint32_t dv = (uint32_t)sp.nact[a];
+        int l = 0;
+        while ((1u << l) < dv) ++l;
+        if (dv <= 1) { sp.nact_mul[a] = 0; sp.nact_shr[a] = 0; }
+        else {
+          const unsigned long long num = 1ull << (31 + l);
+          sp.nact_mul[a] = (uint32_t)((num + dv - 1) / dv);   // < 2^32 because d > 2^(l-1)
+          sp.nact_shr[a] = (uint32_t)(l - 1);                  // umulhi takes 32 of the 31 + l bits
+        }
+      }
       sp.grp_base = sp.tl.base[col];
       const unsigned long long per_cta = c->pooled ? (unsigned long long)PK_GC : (unsigned long long)c->wpc;
       const unsigned long long grid = (n_active + per_cta - 1) / per_cta;
@@ -598,6 +619,9 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) rc = fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
   }
+  c->Dtab = Dtab;
+  c->img_bytes = (((size_t)(nT + 1) * sizeof(TypeParams) + Dtab.size() * 4) + 15) / 16 * 16;
+  if (c->pooled) alloc((void **)&c->img_dev, c->img_bytes);
   if (rc == CPM_OK) rc = upload_types(c, 0);
   if (rc != CPM_OK) { free_all(c); delete c; return rc; }
 
@@ -618,7 +642,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   sp.counters = c->counters; sp.error_flag = c->error_flag;
   sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
   sp.vec_on = (pers_on || chem_on) ? 1 : 0; sp.vec_types = c->vec_types_dev; sp.pq = c->pq; sp.chem = c->chem;
-  sp.anc = c->anc;
+  sp.anc = c->anc; sp.img = c->img_dev; sp.img_bytes = (int)c->img_bytes;
   for (int n2 = 1; n2 <= 3; ++n2) sp.xq_len[n2 - 1] = (int)std::llround(16384.0 / std::sqrt((double)n2));
 
   memset(&c->tm_lat, 0, sizeof(CUtensorMap));

@@ -89,6 +89,16 @@ struct PGeom {
   static __host__ __device__ constexpr int dy(int n) { return (idx27(n) / 3) % 3 - 1; }
   static __host__ __device__ constexpr int dz(int n) { return DIM == 3 ? idx27(n) / 9 - 1 : 0; }
   static __host__ __device__ constexpr int noff(int n) { return (dz(n) * T + dy(n)) * T + dx(n); }   // in tile words
+  static_assert(((DIM == 3) ? (T + 1) * T + 1 : T + 1) <= 127, "neighbour offsets are packed as signed bytes");
+  static __host__ __device__ constexpr unsigned long long noff_pack(int i) {   // offsets of neighbours 8 i .. 8 i + 7 (0 beyond NNB: the centre)
+    unsigned long long r = 0;
+    for (int b = 0; b < 8; ++b) {
+      const int n = 8 * i + b;
+      const int v = (n < NNB) ? noff(n) : 0;
+      r |= (unsigned long long)(unsigned char)(signed char)v << (8 * b);
+    }
+    return r;
+  }
 };
 
 // shared-memory carve-up of one warp; D (2 nT^3 + nT words) comes last
@@ -107,7 +117,8 @@ struct PSmem {
   static constexpr int NOFF = ORIG + 12 * PK_GC;                   // int [32] neighbour -> tile offset (entry NNB = centre = 0)
   static constexpr int TYPES = (NOFF + 128 + 15) / 16 * 16;        // TypeParams [nT + 1], then int32 [nT][nT][nT][2] adhesion
                                                                    // differences, then [nT] J(t,t)
-  static constexpr size_t bytes(int nT) { return (size_t)TYPES + (size_t)(nT + 1) * 32 + ((size_t)2 * nT * nT * nT + nT) * 4; }
+  static constexpr size_t img_bytes(int nT) { return (((size_t)(nT + 1) * 32 + ((size_t)2 * nT * nT * nT + nT) * 4) + 15) / 16 * 16; }   // the bulk-copied part
+  static constexpr size_t bytes(int nT) { return (size_t)TYPES + img_bytes(nT); }
 };
 
 // n += ((raw ^ w) & PK_CELL) == 0, as one logic op with a predicate result and one predicated add
@@ -164,26 +175,23 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   // ---- a2: one bulk copy stages the 8 tiles; it overlaps the set-up and the Philox blocks ----
   if (lane == 0) {
     mbar_init(mbar, 1); fence_mbar_init();
-    mbar_expect_tx(mbar, (uint32_t)(TW * 4 * GC));
+    mbar_expect_tx(mbar, (uint32_t)(TW * 4 * GC) + (uint32_t)P.img_bytes);
     bulk_load(tile, gtile, (uint32_t)(TW * 4 * GC), mbar);
+    bulk_load(st, P.img, (uint32_t)P.img_bytes, mbar);   // per-type records and the adhesion table, first used after the wait below
   }
   // small tables
-  {
-    int dx = 0, dy = 0, dz = 0;
-    if (lane < NNB) nb_delta<DIM>(lane, dx, dy, dz);
-    snoff[lane] = (dz * T + dy) * T + dx;
+  {   // neighbour -> tile offset, from four compile-time words of eight signed bytes each
+    const unsigned long long pk = lane < 8 ? G::noff_pack(0) : lane < 16 ? G::noff_pack(1) : lane < 24 ? G::noff_pack(2) : G::noff_pack(3);
+    snoff[lane] = (int)(signed char)(unsigned char)(pk >> (8 * (lane & 7)));
   }
-#pragma unroll 1
-  for (int i = lane; i < (P.nT + 1) * 8; i += 32) reinterpret_cast<int32_t *>(st)[i] = reinterpret_cast<const int32_t *>(P.types)[i];
-#pragma unroll 1
-  for (int i = lane; i < 2 * P.nT * P.nT * P.nT + P.nT; i += 32) sd[i] = P.D[i];
   // geometry of the chains (the host limits n_active to 31 bits for this kernel)
   if (lane < GC) {
     const uint32_t w = blockIdx.x * (uint32_t)GC + (uint32_t)lane;
     int ox = -1, oy = 0, oz = 0;    // ox < 0: no such chain (ragged last group)
     if (w < (uint32_t)P.n_active) {
-      const uint32_t ax = w % (uint32_t)P.nact[0], r1 = w / (uint32_t)P.nact[0];
-      const uint32_t ay = r1 % (uint32_t)P.nact[1], az = r1 / (uint32_t)P.nact[1];
+      // w -> (ax, ay, az) with the host-built reciprocals of the launch parameters (exact for w < 2^31)
+      const uint32_t r1 = P.nact_mul[0] ? __umulhi(w, P.nact_mul[0]) >> P.nact_shr[0] : w, ax = w - r1 * (uint32_t)P.nact[0];
+      const uint32_t az = P.nact_mul[1] ? __umulhi(r1, P.nact_mul[1]) >> P.nact_shr[1] : r1, ay = r1 - az * (uint32_t)P.nact[1];
       ox = (2 * (int)ax + P.col[0]) * S; oy = (2 * (int)ay + P.col[1]) * S; oz = (DIM == 3) ? (2 * (int)az + P.col[2]) * S : 0;
     }
     orig[lane] = ox; orig[GC + lane] = oy; orig[2 * GC + lane] = oz;

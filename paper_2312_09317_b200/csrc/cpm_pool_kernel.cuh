@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   int32_t *sd = reinterpret_cast<int32_t *>(smem + M::TYPES + (P.nT + 1) * 32);
   const int32_t *sdiag = sd + 2 * P.nT * P.nT * P.nT;
 
+  const uint32_t mcs = __ldg(P.mcs_ptr);   // first: the only global load the Philox counters wait for
   const int lane = threadIdx.x;
   const int c = lane & (GC - 1), q = lane >> PK_GS;   // this lane serves chain c; q = its slot among the chain's 4 lanes
   const unsigned lt = (1u << lane) - 1u;
@@ -200,7 +201,6 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   __syncwarp();
   const bool active = orig[c] >= 0;
   const uint32_t b = active ? (uint32_t)(orig[c] / S + P.nsub[0] * (orig[GC + c] / S + P.nsub[1] * (orig[2 * GC + c] / S))) : 0u;
-  const uint32_t mcs = *P.mcs_ptr;
   const int k = P.k;
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;

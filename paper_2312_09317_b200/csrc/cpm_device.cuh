@@ -92,6 +92,7 @@ struct SweepParams {
   const short4 *pq;                  // [max_cells + 1] persistence direction of the cell (null: persistence off)
   const short4 *chem;                // [N] chemotaxis field, row-major x fastest (null: no field loaded)
   int xq_len[3];                     // llround(16384 / sqrt(n)), n = 1, 2, 3: component of the unit copy direction
+  const int4 *lane_tab;              // pooled kernel: [32] {tile offset, dx, dy, dz} of Moore neighbour `lane` (zeros beyond nNb)
   const unsigned char *img; int img_bytes;   // pooled kernel: per-type records + adhesion table as they sit in shared memory (one bulk copy)
   const int *anc;                    // [max_cells + 1][3] anchors of the periodic centroid tracking (reading S23); null: off
 };

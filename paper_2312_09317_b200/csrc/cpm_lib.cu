@@ -70,6 +70,7 @@ struct cpm_ctx {
   uint32_t *mcs_dev = nullptr;
   int32_t *J_dev = nullptr, *D_dev = nullptr, *log_dev = nullptr, *exp_dev = nullptr;
   TypeParams *types_dev = nullptr;
+  int4 *lane_tab_dev = nullptr;
   unsigned char *img_dev = nullptr;   // pooled kernel: types + adhesion table as one shared-memory image
   size_t img_bytes = 0;
   std::vector<int32_t> Dtab;
@@ -276,7 +277,7 @@ void free_all(cpm_ctx *c) {
   cudaFree(c->tl_tiles()); cudaFree(c->ovf_keys); cudaFree(c->ovf_dvp); cudaFree(c->ovf_count);
   cudaFree(c->stage_a); cudaFree(c->stage_b); cudaFree(c->stage_c);
   cudaFree(c->vec_types_dev); cudaFree(c->mu_dev); cudaFree(c->phat); cudaFree(c->ring); cudaFree(c->pq); cudaFree(c->chem);
-  cudaFree(c->img_dev); cudaFree(c->ctype_dev); cudaFree(c->pers_n); cudaFree(c->anc); cudaFree(c->first_site);
+  cudaFree(c->lane_tab_dev); cudaFree(c->img_dev); cudaFree(c->ctype_dev); cudaFree(c->pers_n); cudaFree(c->anc); cudaFree(c->first_site);
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -622,6 +623,20 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   c->Dtab = Dtab;
   c->img_bytes = (((size_t)(nT + 1) * sizeof(TypeParams) + Dtab.size() * 4) + 15) / 16 * 16;
   if (c->pooled) alloc((void **)&c->img_dev, c->img_bytes);
+  if (c->pooled) {   // neighbour n of the enumeration (dz, dy, dx) lexicographic, centre skipped (reading S16), in a tile of edge S + 2
+    alloc((void **)&c->lane_tab_dev, 32 * sizeof(int4));
+    int4 tab[32];
+    const int Tt = S + 2, nNb = c->nNb;
+    for (int n = 0; n < 32; ++n) {
+      tab[n] = make_int4(0, 0, 0, 0);
+      if (n >= nNb) continue;
+      const int i = n + (n >= nNb / 2 ? 1 : 0);
+      const int dx = i % 3 - 1, dy = (i / 3) % 3 - 1, dz = (d == 3) ? i / 9 - 1 : 0;
+      tab[n] = make_int4((dz * Tt + dy) * Tt + dx, dx, dy, dz);
+    }
+    if (rc == CPM_OK && cudaMemcpyAsync(c->lane_tab_dev, tab, sizeof(tab), cudaMemcpyHostToDevice, c->stream) != cudaSuccess) rc = CPM_ERR_CUDA;
+    if (rc == CPM_OK && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = CPM_ERR_CUDA;
+  }
   if (rc == CPM_OK) rc = upload_types(c, 0);
   if (rc != CPM_OK) { free_all(c); delete c; return rc; }
 
@@ -642,7 +657,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   sp.counters = c->counters; sp.error_flag = c->error_flag;
   sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
   sp.vec_on = (pers_on || chem_on) ? 1 : 0; sp.vec_types = c->vec_types_dev; sp.pq = c->pq; sp.chem = c->chem;
-  sp.anc = c->anc; sp.img = c->img_dev; sp.img_bytes = (int)c->img_bytes;
+  sp.anc = c->anc; sp.img = c->img_dev; sp.img_bytes = (int)c->img_bytes; sp.lane_tab = c->lane_tab_dev;
   for (int n2 = 1; n2 <= 3; ++n2) sp.xq_len[n2 - 1] = (int)std::llround(16384.0 / std::sqrt((double)n2));
 
   memset(&c->tm_lat, 0, sizeof(CUtensorMap));

@@ -89,16 +89,6 @@ struct PGeom {
   static __host__ __device__ constexpr int dy(int n) { return (idx27(n) / 3) % 3 - 1; }
   static __host__ __device__ constexpr int dz(int n) { return DIM == 3 ? idx27(n) / 9 - 1 : 0; }
   static __host__ __device__ constexpr int noff(int n) { return (dz(n) * T + dy(n)) * T + dx(n); }   // in tile words
-  static_assert(((DIM == 3) ? (T + 1) * T + 1 : T + 1) <= 127, "neighbour offsets are packed as signed bytes");
-  static __host__ __device__ constexpr unsigned long long noff_pack(int i) {   // offsets of neighbours 8 i .. 8 i + 7 (0 beyond NNB: the centre)
-    unsigned long long r = 0;
-    for (int b = 0; b < 8; ++b) {
-      const int n = 8 * i + b;
-      const int v = (n < NNB) ? noff(n) : 0;
-      r |= (unsigned long long)(unsigned char)(signed char)v << (8 * b);
-    }
-    return r;
-  }
 };
 
 // shared-memory carve-up of one warp; D (2 nT^3 + nT words) comes last
@@ -181,10 +171,10 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
     bulk_load(st, P.img, (uint32_t)P.img_bytes, mbar);   // per-type records and the adhesion table, first used after the wait below
   }
   // small tables
-  {   // neighbour -> tile offset, from four compile-time words of eight signed bytes each
-    const unsigned long long pk = lane < 8 ? G::noff_pack(0) : lane < 16 ? G::noff_pack(1) : lane < 24 ? G::noff_pack(2) : G::noff_pack(3);
-    snoff[lane] = (int)(signed char)(unsigned char)(pk >> (8 * (lane & 7)));
-  }
+  // per-lane constants: tile offset and (dx, dy, dz) of Moore neighbour `lane` (zeros for lanes >= NNB: the centre), one
+  // coalesced 16-byte load from a host-built table instead of divisions by 3 and 9
+  const int4 lane_nb = __ldg(P.lane_tab + lane);
+  snoff[lane] = lane_nb.x;
   // geometry of the chains (the host limits n_active to 31 bits for this kernel)
   if (lane < GC) {
     const uint32_t w = blockIdx.x * (uint32_t)GC + (uint32_t)lane;
@@ -383,8 +373,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         if (mwA | mwB) {   // warp-uniform
           // lanes = the sites of the neighbourhood (lane NNB = the centre): all loads of a request are in flight together
           int ddx = 0, ddy = 0, ddz = 0;
-          if (lane < NNB) nb_delta<DIM>(lane, ddx, ddy, ddz);
-          const int mynoff = (lane < NNB) ? snoff[lane] : 0;
+          ddx = lane_nb.y; ddy = lane_nb.z; ddz = lane_nb.w;
+          const int mynoff = lane_nb.x;
           int gA = 0, gB = 0;
           while (mwA | mwB) {
             const bool sideB = mwA == 0u;

@@ -78,6 +78,7 @@ struct SweepParams {
   const unsigned long long *snapVP;  // {V:hi32, P:lo32} per cell, phase-start snapshot
   unsigned long long *liveVP;
   unsigned long long *sumx, *sumy, *sumz;
+  unsigned long long *cell_arr[4];   // {liveVP, sumx, sumy, sumz}: the commit lanes index it by their role
   unsigned long long *counters;      // [COUNTER_SLOTS][2] evaluated, accepted
   int *error_flag;
   // pooled kernel

@@ -654,6 +654,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   sp.thr = c->thr_dev; sp.Hmax = c->Hmax; sp.accept_all = accept_all ? 1 : 0;
   sp.logq16 = c->log_dev; sp.expq16 = c->exp_dev;
   sp.snapVP = c->snapVP; sp.liveVP = c->liveVP; sp.sumx = c->sumx; sp.sumy = c->sumy; sp.sumz = c->sumz;
+  sp.cell_arr[0] = c->liveVP; sp.cell_arr[1] = c->sumx; sp.cell_arr[2] = c->sumy; sp.cell_arr[3] = c->sumz;
   sp.counters = c->counters; sp.error_flag = c->error_flag;
   sp.ovf_keys = c->ovf_keys; sp.ovf_dvp = c->ovf_dvp; sp.ovf_count = c->ovf_count;
   sp.vec_on = (pers_on || chem_on) ? 1 : 0; sp.vec_types = c->vec_types_dev; sp.pq = c->pq; sp.chem = c->chem;

@@ -122,6 +122,16 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// tile offset (non-negative) -> tile coordinates, with unsigned divisions by the compile-time edge
+template <int DIM, int T>
+__device__ __forceinline__ void tile_xyz(int off, int &x, int &y, int &z) {
+  const unsigned u = (unsigned)off;
+  const unsigned r = u / (unsigned)T;
+  x = (int)(u - r * (unsigned)T);
+  if (DIM == 3) { const unsigned r2 = r / (unsigned)T; y = (int)(r - r2 * (unsigned)T); z = (int)r2; }
+  else { y = (int)r; z = 0; }
+}
+
 // word offset of tile element j of the subsection (bx,by,bz) in the tiled lattice
 __device__ __forceinline__ unsigned long long tile_word(const TileLayout &L, int bx, int by, int bz, int j) {
   const int col = (bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2);
@@ -332,8 +342,10 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
           if (go && P.vec_on) {   // (the specialisation also serves periodic centroid tracking alone)
             constexpr int CEN = (DIM == 3) ? (T * T + T + 1) : (T + 1);
             const int dd = soff - toff + CEN;   // = ((dz + 1) T + dy + 1) T + dx + 1 of the source's offset
-            const int ddx = dd % T - 1, ddy = (dd / T) % T - 1, ddz = (DIM == 3) ? dd / (T * T) - 1 : 0;
-            int gx = orig[ci] - 1 + soff % T, gy = orig[GC + ci] - 1 + (soff / T) % T, gz = (DIM == 3) ? orig[2 * GC + ci] - 1 + soff / (T * T) : 0;
+            int ddx, ddy, ddz, sx0, sy0, sz0;
+            tile_xyz<DIM, T>(dd, ddx, ddy, ddz); ddx -= 1; ddy -= 1; ddz = (DIM == 3) ? ddz - 1 : 0;
+            tile_xyz<DIM, T>(soff, sx0, sy0, sz0);
+            int gx = orig[ci] - 1 + sx0, gy = orig[GC + ci] - 1 + sy0, gz = (DIM == 3) ? orig[2 * GC + ci] - 1 + sz0 : 0;
             bool inside = true;   // false: the source lies outside a closed lattice (no field there)
             if (gx < 0) { gx += P.X; inside = P.per[0] != 0; } else if (gx >= P.X) { gx -= P.X; inside = P.per[0] != 0; }
             if (gy < 0) { gy += P.Y; inside = inside && P.per[1] != 0; } else if (gy >= P.Y) { gy -= P.Y; inside = inside && P.per[1] != 0; }
@@ -357,7 +369,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         if (wantA | wantB) {
           const int ox = orig[ci], oy = orig[GC + ci], oz = orig[2 * GC + ci];
           if (wantA) {
-            const int sz3 = (DIM == 3) ? soff / (T * T) : 0, sy3 = (soff / T) % T, sx3 = soff % T;
+            int sx3, sy3, sz3;
+            tile_xyz<DIM, T>(soff, sx3, sy3, sz3);
             int gx = ox - 1 + sx3, gy = oy - 1 + sy3, gz = (DIM == 3) ? oz - 1 + sz3 : 0;
             gx += (gx < 0) ? P.X : (gx >= P.X) ? -P.X : 0;   // the source holds a cell: it lies inside the lattice, possibly through the wrap
             gy += (gy < 0) ? P.Y : (gy >= P.Y) ? -P.Y : 0;
@@ -365,7 +378,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             wantA = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx) != 0;
           }
           if (wantB) {
-            const int tz3 = (DIM == 3) ? toff / (T * T) : 0, ty3 = (toff / T) % T, tx3 = toff % T;
+            int tx3, ty3, tz3;
+            tile_xyz<DIM, T>(toff, tx3, ty3, tz3);
             wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
           }
         }
@@ -383,7 +397,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             const int ctr = __shfl_sync(FULL, sideB ? toff : soff, src);
             const int cc = __shfl_sync(FULL, ci, src);
             const uint32_t mC = __shfl_sync(FULL, sideB ? mB : mA, src);
-            const int pz = (DIM == 3) ? ctr / (T * T) : 0, py = (ctr / T) % T, px = ctr % T;
+            int px, py, pz;
+            tile_xyz<DIM, T>(ctr, px, py, pz);
             // the centre is inside the lattice (its cell is not medium), possibly through the wrap
             int cx = orig[cc] - 1 + px, cy = orig[GC + cc] - 1 + py, cz = (DIM == 3) ? orig[2 * GC + cc] - 1 + pz : 0;
             cx += (cx < 0) ? P.X : (cx >= P.X) ? -P.X : 0;
@@ -448,7 +463,9 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
       unsigned rem = __ballot_sync(FULL, lane < GC && first[lane] < PK_NOWIN);
       while (rem) {   // warp-uniform
         unsigned mm = rem;
-        for (int i = 0; i < q; ++i) mm &= mm - 1;
+        if (q > 0) mm &= mm - 1;   // drop the q lowest winners: this lane's group of 8 serves the (q + 1)-th
+        if (q > 1) mm &= mm - 1;
+        if (q > 2) mm &= mm - 1;
         const bool on = mm != 0u;
         const int cw = on ? __ffs(mm) - 1 : 0;
         const int r = c;
@@ -460,7 +477,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
         __syncwarp();   // every lane has read the state of the round's start
         if (on) {
-          const int px = toff % T, py = (toff / T) % T, pz = (DIM == 3) ? toff / (T * T) : 0;   // tile coordinates 1..S
+          int px, py, pz;   // tile coordinates 1..S
+          tile_xyz<DIM, T>(toff, px, py, pz);
           const int ox = orig[cw], oy = orig[GC + cw], oz = orig[2 * GC + cw];
           const int gx = ox + px - 1, gy = oy + py - 1, gz = (DIM == 3) ? oz + pz - 1 : 0;
           if (r == 0) {
@@ -494,7 +512,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             if (cell != 0 && (which < 3 || DIM == 3)) {
               const int sgn = side ? -1 : 1;
               const int dP = side ? 2 * nB - NNB : NNB - 2 * nA;
-              unsigned long long *const arr = which == 0 ? P.liveVP : which == 1 ? P.sumx : which == 2 ? P.sumy : P.sumz;
+              unsigned long long *const arr = P.cell_arr[which];   // {V,P}, sum x, sum y, sum z
               const unsigned long long v = which == 0 ? ((unsigned long long)(long long)sgn << 32) + (unsigned long long)(long long)dP
                                                       : (unsigned long long)(long long)(sgn * (VEC ? sum_coord(P, cell, which - 1, which == 1 ? gx : which == 2 ? gy : gz)
                                                                                                    : (which == 1 ? gx : which == 2 ? gy : gz)));   // periodic tracking (S23) rides on the VEC specialisation

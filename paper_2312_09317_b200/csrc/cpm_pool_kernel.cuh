@@ -200,7 +200,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   }
   __syncwarp();
   const bool active = orig[c] >= 0;
-  const uint32_t b = active ? (uint32_t)(orig[c] / S + P.nsub[0] * (orig[GC + c] / S + P.nsub[1] * (orig[2 * GC + c] / S))) : 0u;
+  // origins of active chains are non-negative multiples of S: a shift divides them
+  const uint32_t b = active ? (uint32_t)((orig[c] >> G::LOG2S) + P.nsub[0] * ((orig[GC + c] >> G::LOG2S) + P.nsub[1] * (orig[2 * GC + c] >> G::LOG2S))) : 0u;
   const int k = P.k;
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;
@@ -445,7 +446,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
       if (__any_sync(FULL, draw)) {
         if (draw) {
           const int ag = sc + a;
-          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)(orig[ci] / S + P.nsub[0] * (orig[GC + ci] / S + P.nsub[1] * (orig[2 * GC + ci] / S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
+          const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)((orig[ci] >> G::LOG2S) + P.nsub[0] * ((orig[GC + ci] >> G::LOG2S) + P.nsub[1] * (orig[2 * GC + ci] >> G::LOG2S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
           if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
         }
       }
@@ -494,7 +495,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             const int avail = (fx != 0 ? 1 : 0) | (fy != 0 ? 2 : 0) | (fz != 0 ? 4 : 0);
             if ((r & ~avail) == 0) {
               const int dx = (r & 1) ? fx : 0, dy = (r & 2) ? fy : 0, dz = (r & 4) ? fz : 0;
-              int nx = ox / S + dx, ny = oy / S + dy, nz = oz / S + dz;
+              int nx = (ox >> G::LOG2S) + dx, ny = (oy >> G::LOG2S) + dy, nz = (oz >> G::LOG2S) + dz;
               bool ok = true;
               if (nx < 0) { nx += P.nsub[0]; ok = P.per[0] != 0; } else if (nx >= P.nsub[0]) { nx -= P.nsub[0]; ok = P.per[0] != 0; }
               if (ny < 0) { ny += P.nsub[1]; ok = ok && P.per[1] != 0; } else if (ny >= P.nsub[1]) { ny -= P.nsub[1]; ok = ok && P.per[1] != 0; }

@@ -437,6 +437,11 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
     sites *= S;
   }
   if (sites > (1 << 24)) return CPM_ERR_UNSUPPORTED;
+  {   // the kernels index lattice rows (y + Y z) with 32 bits
+    long long nrows = 1;
+    for (int a = 1; a < d; ++a) nrows *= p->dims[a];
+    if (nrows >= (1LL << 31)) return CPM_ERR_UNSUPPORTED;
+  }
   long long k = p->attempts_per_activation ? p->attempts_per_activation : sites;
   if (k < 1 || sites % k) return CPM_ERR_ARG;
 

@@ -132,6 +132,11 @@ __device__ __forceinline__ void tile_xyz(int off, int &x, int &y, int &z) {
   else { y = (int)r; z = 0; }
 }
 
+// byte offset of site (x,y,z) in the Act field: y + Y z fits 32 bits (fewer than 2^31 rows), one widening multiply-add
+__device__ __forceinline__ long long act_index(const SweepParams &P, int x, int y, int z) {
+  return (long long)(y + P.Y * z) * P.apitch + x;
+}
+
 // word offset of tile element j of the subsection (bx,by,bz) in the tiled lattice
 __device__ __forceinline__ unsigned long long tile_word(const TileLayout &L, int bx, int by, int bz, int j) {
   const int col = (bx & 1) | ((by & 1) << 1) | ((bz & 1) << 2);
@@ -276,7 +281,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
       const int item = have ? (int)queue[lane] : 0;
       ci = item & (GC - 1); a = item >> PK_GS;
       const uint32_t prc = prop[a * GC + ci];
-      const int toff = (int)(prc & 0xffffu) / (4 * TS), soff = (int)(prc >> 16) / (4 * TS);
+      const int toff = (int)((prc & 0xffffu) / (unsigned)(4 * TS)), soff = (int)((prc >> 16) / (unsigned)(4 * TS));
       int nA = 0, nB = 0;
       const uint32_t *const tc = tile + pk_tbase(ci, TW);
       const uint32_t wA = tc[soff * TS], wB = tc[toff * TS];
@@ -376,12 +381,12 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             gx += (gx < 0) ? P.X : (gx >= P.X) ? -P.X : 0;   // the source holds a cell: it lies inside the lattice, possibly through the wrap
             gy += (gy < 0) ? P.Y : (gy >= P.Y) ? -P.Y : 0;
             if (DIM == 3) gz += (gz < 0) ? P.Z : (gz >= P.Z) ? -P.Z : 0;
-            wantA = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx) != 0;
+            wantA = __ldcg(P.act + act_index(P, gx, gy, gz)) != 0;
           }
           if (wantB) {
             int tx3, ty3, tz3;
             tile_xyz<DIM, T>(toff, tx3, ty3, tz3);
-            wantB = __ldcg(P.act + P.apitch * ((long long)(oy - 1 + ty3) + (long long)P.Y * ((DIM == 3) ? oz - 1 + tz3 : 0)) + ox - 1 + tx3) != 0;
+            wantB = __ldcg(P.act + act_index(P, ox - 1 + tx3, oy - 1 + ty3, (DIM == 3) ? oz - 1 + tz3 : 0)) != 0;
           }
         }
         unsigned mwA = __ballot_sync(FULL, wantA), mwB = __ballot_sync(FULL, wantB);
@@ -422,7 +427,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             }
             int av = 1;
             // L2: sees the Act bytes stored by earlier commits of this warp
-            if (same) av = __ldcg(P.act + P.apitch * ((long long)gy + (long long)P.Y * gz) + gx);
+            if (same) av = __ldcg(P.act + act_index(P, gx, gy, gz));
             const unsigned msame = __ballot_sync(FULL, same);
             const unsigned mzero = __ballot_sync(FULL, same && av == 0);
             const int ssum = __reduce_add_sync(FULL, same ? __ldg(P.logq16 + av) : 0);
@@ -473,8 +478,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         const int fw = first[cw];
         const int nA = (fw >> 5) & 31, nB = fw & 31;
         const uint32_t prc = prop[(on ? (fw >> 10) : 0) * GC + cw];
-        const int toff = (int)(prc & 0xffffu) / (4 * TS);
-        const uint32_t wA = tile[pk_tbase(cw, TW) + (int)(prc >> 16) / (4 * TS) * TS], wB = tile[pk_tbase(cw, TW) + toff * TS];
+        const int toff = (int)((prc & 0xffffu) / (unsigned)(4 * TS));
+        const uint32_t wA = tile[pk_tbase(cw, TW) + (int)((prc >> 16) / (unsigned)(4 * TS)) * TS], wB = tile[pk_tbase(cw, TW) + toff * TS];
         const uint32_t A = wA & ID_MASK, Bc = wB & ID_MASK;
         __syncwarp();   // every lane has read the state of the round's start
         if (on) {
@@ -486,7 +491,7 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
             tile[pk_tbase(cw, TW) + toff * TS] = wA;                                  // id and type of the source; neither site is frozen
             gtile[pk_tbase(cw, TW) + toff * TS] = wA;                                 // home word in HBM
             if constexpr (ACT)   // Max_act of the new owner; 0 for medium
-              P.act[P.apitch * ((long long)gy + (long long)P.Y * gz) + gx] = (uint8_t)((A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0);
+              P.act[act_index(P, gx, gy, gz)] = (uint8_t)((A != 0) ? st[wA >> PK_TYPE_SHIFT].maxA : 0);
             ++n_acc;
           } else if (r < (1 << DIM)) {
             // halo replica of this site in the tile of the adjacent (inactive) subsection towards r

@@ -189,7 +189,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   // per-lane constants: tile offset and (dx, dy, dz) of Moore neighbour `lane` (zeros for lanes >= NNB: the centre), one
   // coalesced 16-byte load from a host-built table instead of divisions by 3 and 9
   const int4 lane_nb = __ldg(P.lane_tab + lane);
-  snoff[lane] = lane_nb.x;
+  // neighbour -> what it adds to a packed proposal (target | source << 16, byte offsets): its tile offset in the source half
+  snoff[lane] = (int)((uint32_t)(lane_nb.x * (4 * TS)) << 16);
   // geometry of the chains (the host limits n_active to 31 bits for this kernel)
   if (lane < GC) {
     const uint32_t w = blockIdx.x * (uint32_t)GC + (uint32_t)lane;
@@ -211,7 +212,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
   uint32_t n_eval = 0, n_acc = 0;
   bool overflow = false;
   bool staged = false;
-  const uint32_t *const tcol = tile + pk_tbase(c, TW);   // the tile of this lane's own chain
+  static_assert(PK_CHAIN_MAJOR == 0, "packed proposals carry the chain's byte offset below 4 TS: interleaved tiles only");
+  const uint32_t cbase2 = (uint32_t)(pk_tbase(c, TW) * 4) * 0x10001u;   // byte offset of this lane's chain inside the group's tiles, in both halves
 
   for (int sc = 0; sc < k; sc += PK_SUPER) {
     const int kk = min(PK_SUPER, k - sc);   // attempts of this stretch
@@ -226,7 +228,9 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         const int nb = (int)__umulhi(wd << G::LOG2SITES, (uint32_t)NNB);         // = (u32(wd * S^d) * nNb) >> 32
         const int lx = l & (S - 1), ly = (l >> G::LOG2S) & (S - 1), lz = (DIM == 3) ? (l >> (2 * G::LOG2S)) : 0;
         const int toff = (((DIM == 3) ? (lz + 1) * T : 0) + ly + 1) * T + lx + 1;
-        prop[(4 * qq + j) * GC + c] = (uint32_t)(toff * (4 * TS)) | ((uint32_t)((toff + snoff[nb]) * (4 * TS)) << 16);
+        // both halves carry the byte offset of the chain's tile inside the group (4 c < 4 TS with interleaved tiles, so offset / (4 TS) is
+        // still the tile word): a screen or a census load then needs no address arithmetic beyond the shared-memory base
+        prop[(4 * qq + j) * GC + c] = (uint32_t)toff * (uint32_t)((4 * TS) * 0x10001) + (uint32_t)snoff[nb] + cbase2;
       }
     }
     int pos = active ? 0 : kk;   // attempts < pos of this stretch are final (same value in the 4 lanes of a chain)
@@ -248,8 +252,8 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
         uint32_t wt = 0u, ws = 0u;
         if (ok) {
           const uint32_t prc = prop[a * GC + c];
-          wt = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tcol) + (prc & 0xffffu));
-          ws = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tcol) + (prc >> 16));
+          wt = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tile) + (prc & 0xffffu));
+          ws = *reinterpret_cast<const uint32_t *>(reinterpret_cast<const char *>(tile) + (prc >> 16));
         }
         in[j] = ok && (((wt ^ ws) & ID_MASK) != 0u) && (((wt | ws) & PK_FROZEN) == 0u);
         m[j] = __ballot_sync(FULL, in[j]);

@@ -319,9 +319,9 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
           const int ne = di & 255;
           if (ne > 0) {
             unsigned long long dA = 0ull, dB = 0ull;
-            const int ns = min(ne, PK_DCAP);
-            for (int i = 0; i < ns; ++i) {
-              const uint32_t key = dkey[i * GC + ci];
+#pragma unroll
+            for (int i = 0; i < PK_DCAP; ++i) {   // the shared-memory entries, without a loop (entries beyond ne hold stale keys: masked)
+              const uint32_t key = (i < ne) ? dkey[i * GC + ci] : 0xffffffffu;
               const unsigned long long v = ddvp[i * GC + ci];
               if (key == A) dA = v;
               if (key == Bc) dB = v;
@@ -543,9 +543,9 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
           const int ne = di & 255;
           int hit = -1;
           if (mine) {
-            const int ns = min(ne, PK_DCAP);
-            for (int i = 0; i < ns; ++i)
-              if (dkey[i * GC + cw] == cell) hit = i;
+#pragma unroll
+            for (int i = 0; i < PK_DCAP; ++i)
+              if (i < ne && dkey[i * GC + cw] == cell) hit = i;
           }
           const int need = (mine && hit < 0) ? 1 : 0;
           const int needA = __shfl_sync(FULL, need, lane & ~7), needB = __shfl_sync(FULL, need, (lane & ~7) | 4);

@@ -455,8 +455,9 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
       if (__any_sync(FULL, draw)) {
         if (draw) {
           const int ag = sc + a;
+          const uint32_t th = __ldg(P.thr + dH);   // issued before the ten Philox rounds, which hide its latency
           const uint4 ua = philox4x32_10(make_uint4((uint32_t)ag >> 2, (uint32_t)((orig[ci] >> G::LOG2S) + P.nsub[0] * ((orig[GC + ci] >> G::LOG2S) + P.nsub[1] * (orig[2 * GC + ci] >> G::LOG2S))), 2u * P.p + 1u, mcs), P.key0, P.key1);
-          if (pick(ua, ag & 3) >= __ldg(P.thr + dH)) acc = false;
+          if (pick(ua, ag & 3) >= th) acc = false;
         }
       }
       // ---- a9: the first accepted attempt of every chain wins ----

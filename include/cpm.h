@@ -147,6 +147,24 @@ int  cpm_get_interface_counts(cpm_ctx *ctx, uint64_t *out);
  * Needs n_mcs * 2^d * S^d < 2^32 and n_freq + n_wait <= 4096 (CPM_ERR_ARG); allocates 8 bytes per site while it runs. */
 int  cpm_update_statistics(cpm_ctx *ctx, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
                            uint32_t wait_bin);
+/* The same statistics for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): this call allocates NOTHING, on the device or the host -- no cudaMalloc, cudaFree or allocating
+ * library routine.  The kernel's per-site scratch (8 bytes per site) and its histograms live in ONE file-scope
+ * `static __device__` array of CPM_NOALLOC_MAX_SITES * 8 + CPM_NOALLOC_MAX_BINS * 8 bytes (8 MiB + 32 KiB) that every GPU
+ * which loads the library holds until exit.  Limits: dims[0]*dims[1]*dims[2] <= CPM_NOALLOC_MAX_SITES and n_freq + n_wait
+ * <= CPM_NOALLOC_MAX_BINS, else CPM_ERR_ARG with a message that names the limit (plus the limits of cpm_update_statistics).
+ * freq / wait: caller-owned, host pointers (on_device = 0; the call returns after the stream has drained) or device
+ * pointers on the context's device (on_device != 0; results are ready in stream order, no synchronisation).  Results are
+ * bit-identical to cpm_update_statistics.  All contexts on one device share the array, which keeps the last call's
+ * contents (cleared by this call where it must start at zero): calls that overlap on the GPU -- two contexts on different
+ * streams -- RACE; serialise them.  cpm_noalloc_setup(device) resolves the array's device address (cudaGetSymbolAddress,
+ * once per device, with that device current); the first cpm_update_statistics_noalloc on a device does it itself, so
+ * call cpm_noalloc_setup before a graph capture begins.  Returns CPM_ERR_CUDA when the address cannot be had. */
+#define CPM_NOALLOC_MAX_SITES (1u << 20)
+#define CPM_NOALLOC_MAX_BINS  4096
+int  cpm_noalloc_setup(int device);
+int  cpm_update_statistics_noalloc(cpm_ctx *ctx, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
+                                   uint32_t wait_bin, int on_device);
 /* Introspection for tests: host copy of the Metropolis table, thr[h] = floor(exp(-h/T) 2^32),
  * h = 1..Hmax; returns Hmax (>= 0) or a negative error; fills at most cap entries (thr[0] unused). */
 int64_t cpm_get_threshold_table(cpm_ctx *ctx, uint32_t *thr, uint64_t cap);

@@ -4,5 +4,5 @@ the sm_100a kernels under csrc/.  There is no CPU fallback: without the built li
 a CUDA device the calls fail loudly."""
 from .binding import (  # noqa: F401
     CPM, CPMError, MODE_DETERMINISTIC, MODE_LIVE_ATOMICS, FLAG_WARP_KERNEL, FLAG_NO_TMA, FLAG_NO_GRAPH, load_library, library_path, debug_philox,
-    exported_symbols,
+    exported_symbols, noalloc_setup, NOALLOC_MAX_SITES, NOALLOC_MAX_BINS,
 )

@@ -86,6 +86,8 @@ def load_library():
     L.cpm_get_schedule.argtypes = [vp, vp, vp, vp]
     L.cpm_get_interface_counts.argtypes = [vp, vp]
     L.cpm_update_statistics.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32]
+    L.cpm_noalloc_setup.argtypes = [C.c_int]
+    L.cpm_update_statistics_noalloc.argtypes = [vp, C.c_uint32, vp, C.c_int32, vp, C.c_int32, C.c_uint32, C.c_int]
     L.cpm_get_threshold_table.argtypes = [vp, vp, C.c_uint64]
     L.cpm_get_threshold_table.restype = C.c_int64
     L.cpm_get_launch_info.argtypes = [vp, vp]
@@ -285,6 +287,22 @@ class CPM:
                                                 int(wait_bin)))
         return freq, wait
 
+    def update_statistics_noalloc(self, n_mcs, freq, wait, wait_bin=1):
+        """cpm_update_statistics_noalloc: freq / wait are caller-owned uint64 buffers, numpy arrays (host) or CUDA torch
+        tensors viewed as int64 (device); nothing is allocated.  Lattices up to NOALLOC_MAX_SITES sites."""
+        on_dev = not isinstance(freq, np.ndarray)
+        if on_dev != (not isinstance(wait, np.ndarray)):
+            raise TypeError("freq and wait must both be numpy arrays or both be device tensors")
+        for a in (freq, wait):
+            if on_dev:
+                if not (a.is_cuda and a.is_contiguous() and a.element_size() == 8):
+                    raise TypeError("device outputs must be contiguous 8-byte CUDA tensors")
+            elif a.dtype != np.uint64 or not a.flags.c_contiguous:
+                raise TypeError("host outputs must be contiguous uint64 arrays")
+        n_freq, n_wait = (int(freq.numel()), int(wait.numel())) if on_dev else (freq.size, wait.size)
+        pf, pw = (freq.data_ptr(), wait.data_ptr()) if on_dev else (freq.ctypes.data, wait.ctypes.data)
+        self._chk(self._L.cpm_update_statistics_noalloc(self._h, int(n_mcs), pf, n_freq, pw, n_wait, int(wait_bin), int(on_dev)))
+
     def get_threshold_table(self):
         hmax = self._L.cpm_get_threshold_table(self._h, None, 0)
         if hmax < 0:
@@ -307,6 +325,17 @@ class CPM:
         ms = C.c_double(); n = C.c_uint64()
         self._chk(self._L.cpm_get_kernel_timing(self._h, C.addressof(ms), C.addressof(n), 1 if reset else 0))
         return ms.value, int(n.value)
+
+
+NOALLOC_MAX_SITES = 1 << 20   # CPM_NOALLOC_MAX_SITES of include/cpm.h
+NOALLOC_MAX_BINS = 4096       # CPM_NOALLOC_MAX_BINS
+
+
+def noalloc_setup(device=0):
+    """cpm_noalloc_setup: resolve the device address of the library's static scratch array on `device`."""
+    rc = load_library().cpm_noalloc_setup(int(device))
+    if rc != 0:
+        raise CPMError(int(rc), "cpm_noalloc_setup")
 
 
 def debug_philox(ctr, key, device=0):

@@ -13,6 +13,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1029,6 +1030,88 @@ int cpm_update_statistics(cpm_ctx *c, uint32_t n_mcs, uint64_t *freq, int32_t n_
   if (e != cudaSuccess) return fail(c, CPM_ERR_CUDA, cudaGetErrorString(e));
   for (int i = 0; i < n_freq; ++i) freq[i] = h[(size_t)i];
   for (int i = 0; i < n_wait; ++i) wait[i] = h[(size_t)n_freq + i];
+  return CPM_OK;
+}
+
+}  // extern "C"
+
+// ---- cpm_update_statistics_noalloc: the same kernel on a file-scope scratch array; no allocation of any kind ----
+// Layout of the array: [hist: 4096 x u64 | last: MAX_SITES x u32 | cnt: MAX_SITES x u32].  Every GPU that loads the
+// library holds it until exit.  In host code the NAME below is a host-side stand-in, never a device address: the
+// address the kernel gets comes from cudaGetSymbolAddress, once per device, with that device current.
+namespace {
+constexpr size_t NOALLOC_HIST_BYTES = (size_t)CPM_NOALLOC_MAX_BINS * 8;
+constexpr size_t NOALLOC_BYTES = NOALLOC_HIST_BYTES + (size_t)CPM_NOALLOC_MAX_SITES * 8;
+}  // namespace
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+unsigned char *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+
+// device address of the scratch array on `device`, which must be the current device; nullptr + *e on failure
+unsigned char *noalloc_scratch_on(int device, cudaError_t *e) {
+  *e = cudaSuccess;
+  if (device < 0 || device >= NOALLOC_MAX_DEVICES) { *e = cudaErrorInvalidDevice; return nullptr; }
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[device]) {
+    void *p = nullptr;
+    *e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (*e != cudaSuccess) return nullptr;
+    g_noalloc_ptr[device] = static_cast<unsigned char *>(p);
+  }
+  return g_noalloc_ptr[device];
+}
+}  // namespace
+
+extern "C" {
+
+int cpm_noalloc_setup(int device) {
+  if (cudaSetDevice(device) != cudaSuccess) return CPM_ERR_CUDA;
+  cudaError_t e;
+  return noalloc_scratch_on(device, &e) ? CPM_OK : CPM_ERR_CUDA;
+}
+
+int cpm_update_statistics_noalloc(cpm_ctx *c, uint32_t n_mcs, uint64_t *freq, int32_t n_freq, uint64_t *wait, int32_t n_wait,
+                                  uint32_t wait_bin, int on_device) {
+  if (!c || !freq || !wait) return fail(c, CPM_ERR_ARG, "null argument");
+  if (n_freq < 1 || n_wait < 1 || wait_bin < 1 || n_freq + n_wait > CPM_NOALLOC_MAX_BINS)
+    return fail(c, CPM_ERR_ARG, "histogram sizes: n_freq + n_wait must be in [2, 4096]");
+  if (c->N > (long long)CPM_NOALLOC_MAX_SITES)
+    return fail(c, CPM_ERR_ARG, "cpm_update_statistics_noalloc: the lattice has more than CPM_NOALLOC_MAX_SITES (1048576) sites; "
+                                "use cpm_update_statistics");
+  const unsigned long long ticks = (unsigned long long)n_mcs * (unsigned long long)(1 << c->d) * (unsigned long long)c->sites;
+  if (ticks >= (1ull << 32)) return fail(c, CPM_ERR_ARG, "n_mcs * 2^d * S^d must stay below 2^32");
+  CK(cudaSetDevice(c->device));
+  cudaError_t e;
+  unsigned char *base = noalloc_scratch_on(c->device, &e);
+  if (!base) return fail(c, CPM_ERR_CUDA, std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e));
+  unsigned long long *hist = reinterpret_cast<unsigned long long *>(base);
+  uint32_t *last = reinterpret_cast<uint32_t *>(base + NOALLOC_HIST_BYTES);
+  uint32_t *cnt = last + c->N;
+  StatParams P{};
+  P.S = c->S; P.sites = c->sites; P.k = c->k; P.R = c->R; P.nNb = c->nNb;
+  for (int a = 0; a < 3; ++a) P.nsub[a] = c->nsub[a];
+  P.X = c->dim[0]; P.Y = c->dim[1];
+  int rank = 0;
+  for (int col = 0; col < 8; ++col) P.rank[col] = (col < (1 << c->d) && c->n_act_col[col] > 0) ? rank++ : -1;
+  P.E_per_rep = rank;
+  P.mcs0 = c->mcs_host; P.n_mcs = n_mcs; P.key0 = (uint32_t)c->seed; P.key1 = (uint32_t)(c->seed >> 32); P.bin = wait_bin;
+  P.n_freq = n_freq; P.n_wait = n_wait;
+  const long long nsub_total = (long long)c->nsub[0] * c->nsub[1] * c->nsub[2];
+  const size_t nh = (size_t)n_freq + (size_t)n_wait;
+  // the array keeps the last call's contents: the histograms and both per-site words must start at zero
+  CK(cudaMemsetAsync(hist, 0, nh * 8, c->stream));
+  CK(cudaMemsetAsync(last, 0, (size_t)c->N * 8, c->stream));
+  const unsigned blocks = (unsigned)((nsub_total + 127) / 128);
+  if (c->d == 2) update_stats_kernel<2><<<blocks, 128, nh * 8, c->stream>>>(P, nsub_total, last, cnt, hist);
+  else update_stats_kernel<3><<<blocks, 128, nh * 8, c->stream>>>(P, nsub_total, last, cnt, hist);
+  c->launches++;
+  CK(cudaGetLastError());
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  CK(cudaMemcpyAsync(freq, hist, (size_t)n_freq * 8, kind, c->stream));
+  CK(cudaMemcpyAsync(wait, hist + n_freq, (size_t)n_wait * 8, kind, c->stream));
+  if (!on_device) CK(cudaStreamSynchronize(c->stream));
   return CPM_OK;
 }
 

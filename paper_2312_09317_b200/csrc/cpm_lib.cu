@@ -12,6 +12,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -33,6 +34,9 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
 
 typedef void (*SweepFn)(const CUtensorMap, const SweepParams);
 typedef void (*ThreadFn)(const SweepParams);
+
+constexpr int PIPE_SLABS = 8;                   // slabs of a pipelined host transfer
+constexpr long long PIPE_MIN_SITES = 1ll << 24; // lattices below this go in one piece
 
 struct cpm_ctx {
   int d = 0, device = 0;
@@ -93,6 +97,11 @@ struct cpm_ctx {
   // staging buffers for host-pointer I/O, kept between calls
   void *stage_a = nullptr, *stage_b = nullptr, *stage_c = nullptr;
   size_t stage_a_cap = 0, stage_b_cap = 0, stage_c_cap = 0;
+  // host <-> device transfers of a large lattice run slab by slab on a stream of their own, overlapped with the pack /
+  // recount / unpack kernels of the slabs that have arrived (pipe_plan)
+  cudaStream_t io_stream = nullptr;
+  cudaEvent_t io_ev[PIPE_SLABS + 2] = {};
+  long long pipe_min_sites = PIPE_MIN_SITES;   // the environment variable CPM_PIPE_MIN_SITES overrides it (tests)
 
   std::vector<uint32_t> thr;
   std::vector<TypeParams> types;   // host copy of the per-type records
@@ -282,6 +291,33 @@ void free_all(cpm_ctx *c) {
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   if (c->mcs_graph) cudaGraphExecDestroy(c->mcs_graph);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  for (auto e : c->io_ev) if (e) cudaEventDestroy(e);
+  if (c->io_stream) cudaStreamDestroy(c->io_stream);
+}
+
+// the transfer stream and its events, made on first use
+cudaError_t pipe_ready(cpm_ctx *c) {
+  if (c->io_stream) return cudaSuccess;
+  cudaError_t e = cudaStreamCreateWithFlags(&c->io_stream, cudaStreamNonBlocking);
+  for (int i = 0; e == cudaSuccess && i < PIPE_SLABS + 2; ++i) e = cudaEventCreateWithFlags(&c->io_ev[i], cudaEventDisableTiming);
+  return e;
+}
+
+// Slabs of the slowest axis for the pipelined cpm_set_lattice on the tiled layout: slab i = the planes of the pairs of
+// subsection layers [a[i], a[i+1]).  A chain with slow index a of either colour bit reads the planes 2 S a - 1 ..
+// 2 S (a + 1): its own slab plus one plane of each neighbour slab.  False: the lattice goes in one piece.
+bool pipe_plan(const cpm_ctx *c, int a[PIPE_SLABS + 1]) {
+  if (!c->pooled || c->unwrap || c->N < c->pipe_min_sites) return false;
+  const int ax = c->d - 1;
+  const int pairs = (c->nsub[ax] + 1) / 2;
+  if (pairs < 2 * PIPE_SLABS) return false;
+  for (int i = 0; i <= PIPE_SLABS; ++i) a[i] = (int)((long long)i * pairs / PIPE_SLABS);
+  for (int col = 0; col < (1 << c->d); ++col) {
+    if (c->n_act_col[col] == 0) continue;
+    const unsigned long long slow = (unsigned long long)c->sp.tl.nact[col][ax];
+    if (slow == 0 || c->n_act_col[col] / slow < (unsigned long long)PK_GC) return false;   // a group never reaches back beyond the previous slab
+  }
+  return true;
 }
 
 // a1: the work of ONE Monte Carlo step on stream st: R repetitions x 2^d colours of the sweep kernel, the
@@ -454,6 +490,7 @@ static int create_impl(const cpm_params *p, cpm_ctx **out) {
   if (prop.major < 10) return CPM_ERR_CUDA;  // kernels are built for sm_100a only
 
   cpm_ctx *c = new cpm_ctx();
+  if (const char *e = std::getenv("CPM_PIPE_MIN_SITES")) c->pipe_min_sites = std::atoll(e);
   c->d = d; c->device = p->device; c->stream = (cudaStream_t)p->stream;
   c->nT = nT; c->T = p->T; c->seed = p->seed; c->mode = p->mode; c->max_cells = p->max_cells;
   c->N = 1;
@@ -709,8 +746,23 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
   if (ct[0] != 0) return fail(c, CPM_ERR_ARG, "cell 0 must have type 0 (medium)");
   for (size_t i = 0; i < ncell; ++i) if (ct[i] >= c->nT) return fail(c, CPM_ERR_ARG, "cell type out of range");
   const uint32_t *sid; const uint8_t *sfz, *sct;
-  CK(stage_in(const_cast<uint32_t **>(&sid), &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device, c->stream));
-  CK(stage_in(const_cast<uint8_t **>(&sfz), &c->stage_b, &c->stage_b_cap, frozen, (size_t)c->N, on_device, c->stream));
+  int slab[PIPE_SLABS + 1];
+  const bool piped = !on_device && pipe_plan(c, slab);
+  if (piped) {
+    // the lattice comes over slab by slab on the transfer stream; the kernels below follow the slabs
+    CK(pipe_ready(c));
+    CK(stage_reserve(&c->stage_a, &c->stage_a_cap, (size_t)c->N * 4));
+    if (frozen) CK(stage_reserve(&c->stage_b, &c->stage_b_cap, (size_t)c->N));
+    sid = reinterpret_cast<const uint32_t *>(c->stage_a);
+    sfz = frozen ? reinterpret_cast<const uint8_t *>(c->stage_b) : nullptr;
+    CK(cudaEventRecord(c->io_ev[PIPE_SLABS], c->stream));            // earlier work on the staging buffers is done first
+    CK(cudaStreamWaitEvent(c->io_stream, c->io_ev[PIPE_SLABS], 0));
+    // (the slab copies themselves are issued further down, each just before the first kernels that need it, so that a
+    // pageable source, whose copies hold up the host, still overlaps with the kernels of the slabs before it)
+  } else {
+    CK(stage_in(const_cast<uint32_t **>(&sid), &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device, c->stream));
+    CK(stage_in(const_cast<uint8_t **>(&sfz), &c->stage_b, &c->stage_b_cap, frozen, (size_t)c->N, on_device, c->stream));
+  }
   CK(stage_in(const_cast<uint8_t **>(&sct), &c->stage_c, &c->stage_c_cap, cell_type, ncell, on_device, c->stream));
 
   CK(cudaMemsetAsync(c->error_flag, 0, 4, c->stream));
@@ -728,26 +780,66 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
   }
   if (c->pooled) {
     const TileLayout &tl = c->sp.tl;
-    for (int col = 0; col < (1 << c->d); ++col) {
-      if (c->n_act_col[col] == 0) continue;
-      if (c->d == 2)
-        tile_pack_kernel<2><<<grid_for((long long)c->grp_col[col], 1), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
-                                                                     c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
-      else
-        tile_pack_kernel<3><<<grid_for((long long)c->grp_col[col], 1), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], c->dim[0],
-                                                                     c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
-      c->launches++;
-    }
-    for (int col = 0; col < (1 << c->d); ++col) {
-      if (c->n_act_col[col] == 0) continue;
-      const long long thr = (long long)c->n_act_col[col];
-      if (c->d == 2)
-        tile_recount_kernel<2><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz,
-                                                                         c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
-      else
-        tile_recount_kernel<3><<<grid_for(thr, 128), 128, 0, c->stream>>>(tl, col, c->n_act_col[col], c->liveVP, c->sumx, c->sumy, c->sumz,
-                                                                         c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
-      c->launches++;
+    // pack then recount, for the chains [w0, w1) of every colour that the slab `piece` holds (one piece: all of them)
+    auto pack_and_recount = [&](int piece) {
+      const int ax = c->d - 1;
+      unsigned long long gb[8], ge[8], wb[8], we[8];
+      for (int col = 0; col < (1 << c->d); ++col) {
+        const unsigned long long n = c->n_act_col[col];
+        gb[col] = 0; ge[col] = c->grp_col[col]; wb[col] = 0; we[col] = n;
+        if (piece < 0 || n == 0) continue;
+        const unsigned long long slow = (unsigned long long)tl.nact[col][ax], fast = n / slow;
+        const unsigned long long w0 = std::min<unsigned long long>((unsigned long long)slab[piece], slow) * fast;
+        const unsigned long long w1 = std::min<unsigned long long>((unsigned long long)slab[piece + 1], slow) * fast;
+        // a group that straddles two slabs goes with the later one, whose data arrives last
+        gb[col] = w0 >> PK_GS; wb[col] = gb[col] << PK_GS;
+        if (piece < PIPE_SLABS - 1) { ge[col] = w1 >> PK_GS; we[col] = ge[col] << PK_GS; }
+      }
+      for (int col = 0; col < (1 << c->d); ++col) {
+        if (c->n_act_col[col] == 0 || ge[col] <= gb[col]) continue;
+        const int grid = grid_for((long long)(ge[col] - gb[col]), 1);
+        if (c->d == 2)
+          tile_pack_kernel<2><<<grid, 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], gb[col], ge[col], c->dim[0],
+                                                          c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
+        else
+          tile_pack_kernel<3><<<grid, 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, tl, col, c->n_act_col[col], gb[col], ge[col], c->dim[0],
+                                                          c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
+        c->launches++;
+      }
+      for (int col = 0; col < (1 << c->d); ++col) {
+        if (c->n_act_col[col] == 0 || we[col] <= wb[col]) continue;
+        const int grid = grid_for((long long)(we[col] - wb[col]), 128);
+        if (c->d == 2)
+          tile_recount_kernel<2><<<grid, 128, 0, c->stream>>>(tl, col, wb[col], we[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+                                                             c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
+        else
+          tile_recount_kernel<3><<<grid, 128, 0, c->stream>>>(tl, col, wb[col], we[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+                                                             c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
+        c->launches++;
+      }
+    };
+    if (!piped) pack_and_recount(-1);
+    else {
+      // slab i needs one plane of slab i + 1 (its upper halo) and one of slab i - 1; slab 0 reaches the LAST slab through a
+      // periodic border, so it goes last then
+      const bool wrap = c->per[c->d - 1] != 0;
+      const int ax = c->d - 1;
+      const size_t plane = (size_t)(c->N / c->dim[ax]);
+      int issued = 0;   // slabs whose copies are on the transfer stream
+      for (int n = 0; n < PIPE_SLABS; ++n) {
+        const int i = wrap ? (n + 1) % PIPE_SLABS : n;
+        const int need = (wrap && i == 0) ? PIPE_SLABS - 1 : std::min(i + 1, PIPE_SLABS - 1);
+        for (; issued <= need; ++issued) {
+          const size_t p0 = std::min<size_t>((size_t)slab[issued] * 2 * c->S, (size_t)c->dim[ax]) * plane;
+          const size_t p1 = (issued == PIPE_SLABS - 1) ? (size_t)c->N : std::min<size_t>((size_t)slab[issued + 1] * 2 * c->S, (size_t)c->dim[ax]) * plane;
+          CK(cudaMemcpyAsync(const_cast<uint32_t *>(sid) + p0, ids + p0, (p1 - p0) * 4, cudaMemcpyHostToDevice, c->io_stream));
+          if (frozen) CK(cudaMemcpyAsync(const_cast<uint8_t *>(sfz) + p0, frozen + p0, p1 - p0, cudaMemcpyHostToDevice, c->io_stream));
+          CK(cudaEventRecord(c->io_ev[issued], c->io_stream));
+        }
+        CK(cudaStreamWaitEvent(c->stream, c->io_ev[need], 0));
+        pack_and_recount(i);
+      }
+      CK(cudaStreamWaitEvent(c->stream, c->io_ev[PIPE_SLABS - 1], 0));
     }
   } else {
     pack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(sid, sfz, sct, c->max_cells, c->lat, c->sp.pitch, c->dim[0],
@@ -890,8 +982,29 @@ int cpm_get_lattice(cpm_ctx *c, uint32_t *ids, int on_device) {
   uint32_t *s;
   CK(stage_out_begin(&s, &c->stage_a, &c->stage_a_cap, ids, (size_t)c->N, on_device));
   if (c->pooled) {
-    if (c->d == 2) tile_unpack_kernel<2><<<grid_for(c->N), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s);
-    else tile_unpack_kernel<3><<<grid_for(c->N), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s);
+    const bool piped = !on_device && c->N >= c->pipe_min_sites;
+    if (piped) CK(pipe_ready(c));
+    const int pieces = piped ? PIPE_SLABS : 1;
+    // the pieces are unpacked on the context's stream; each goes to the host on the transfer stream while the next is unpacked
+    for (int i = 0; i < pieces; ++i) {
+      const long long i0 = c->N * i / pieces, i1 = c->N * (i + 1) / pieces;
+      if (c->d == 2) tile_unpack_kernel<2><<<grid_for(i1 - i0), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s, i0, i1);
+      else tile_unpack_kernel<3><<<grid_for(i1 - i0), 256, 0, c->stream>>>(c->sp.tl, c->dim[0], c->dim[1], c->dim[2], s, i0, i1);
+      c->launches++;
+      if (piped) CK(cudaEventRecord(c->io_ev[i], c->stream));
+    }
+    for (int i = 0; piped && i < pieces; ++i) {
+      const long long i0 = c->N * i / pieces, i1 = c->N * (i + 1) / pieces;
+      CK(cudaStreamWaitEvent(c->io_stream, c->io_ev[i], 0));
+      CK(cudaMemcpyAsync(ids + i0, s + i0, (size_t)(i1 - i0) * 4, cudaMemcpyDeviceToHost, c->io_stream));
+    }
+    CK(cudaGetLastError());
+    if (piped) {   // the context's stream ends behind the last transfer: the synchronisation below covers it
+      CK(cudaEventRecord(c->io_ev[PIPE_SLABS + 1], c->io_stream));
+      CK(cudaStreamWaitEvent(c->stream, c->io_ev[PIPE_SLABS + 1], 0));
+      return check_device_flag(c);
+    }
+    c->launches--;   // counted once below
   } else {
     unpack_kernel<<<grid_for(c->N), 256, 0, c->stream>>>(c->lat, c->sp.pitch, c->dim[0], c->dim[1], c->dim[2], s);
   }

@@ -619,18 +619,18 @@ __global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const _
 // ------------------------------------------------------------ tiled-layout helpers ----------
 // set_lattice: ids (+frozen, cell types) -> tiles with halo.  A block takes whole groups; thread t writes the words
 // j = t >> 3, t >> 3 + blockDim / 8, ... of chain t & 7, so the chain's geometry is worked out once per group and the
-// stores of a warp are contiguous (no 64-bit division per word).
+// stores of a warp are contiguous (no 64-bit division per word).  Groups [g_begin, g_end) of the colour: the host packs
+// a large lattice slab by slab while the next slab is still on its way from the host.
 template <int DIM>
 __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, const uint8_t *ctype, uint32_t max_cells, TileLayout L,
-                                 int col, unsigned long long n_active, int X, int Y, int Z, int perx, int pery, int perz,
-                                 int *error_flag) {
+                                 int col, unsigned long long n_active, unsigned long long g_begin, unsigned long long g_end,
+                                 int X, int Y, int Z, int perx, int pery, int perz, int *error_flag) {
   const int S = L.S, T = S + 2, TW = L.TW;
-  const unsigned long long ngrp = (n_active + (unsigned long long)(PK_GC - 1)) >> PK_GS;
   // chain-major tiles: a warp writes one chain's contiguous tile; interleaved tiles: 8 consecutive threads = the 8 chains
   const int c = PK_CHAIN_MAJOR ? (int)((threadIdx.x >> 5) & (PK_GC - 1)) : (int)(threadIdx.x & (PK_GC - 1));
   const int j0 = PK_CHAIN_MAJOR ? (int)(threadIdx.x & 31) + 32 * (int)(threadIdx.x >> 8) : (int)(threadIdx.x >> PK_GS);
   const int jstep = PK_CHAIN_MAJOR ? 32 * (int)(blockDim.x >> 8) : (int)(blockDim.x >> PK_GS);   // blockDim is a multiple of 256
-  for (unsigned long long grp = blockIdx.x; grp < ngrp; grp += gridDim.x) {
+  for (unsigned long long grp = g_begin + blockIdx.x; grp < g_end; grp += gridDim.x) {
     const unsigned long long w = grp * (unsigned long long)PK_GC + (unsigned long long)c;
     const bool live = w < n_active;   // the host keeps n_active below 2^31 for this layout
     const uint32_t w32 = (uint32_t)w;
@@ -659,11 +659,11 @@ __global__ void tile_pack_kernel(const uint32_t *ids, const uint8_t *frozen, con
     }
   }
 }
+// sites [i_begin, i_end) in row-major order (the host reads a large lattice back slab by slab)
 template <int DIM>
-__global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *ids) {
-  const long long N = (long long)X * Y * Z;
+__global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *ids, long long i_begin, long long i_end) {
   const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+  for (long long i = i_begin + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < i_end; i += stride) {
     const int x = (int)(i % X);
     const long long r = i / X;
     ids[i] = L.tiles[home_word<DIM>(L, L.S, x, (int)(r % Y), (int)(r / Y))] & ID_MASK;
@@ -672,23 +672,23 @@ __global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *
 // recount of V, A (Moore interfaces with sites not of the same cell, L234) and the coordinate sums (L288) from the
 // tiles: a thread takes one chain and walks its S^d interior sites; every neighbour is inside the chain's own
 // tile, the loads of the 8 lanes of a group are one 32-byte sector; runs of equal ids are flushed with one atomic
-// per array.
+// per array.  Chains [w_begin, w_end) of the colour.
 template <int DIM>
-__global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long n_active, unsigned long long *liveVP,
+__global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long w_begin, unsigned long long w_end, unsigned long long *liveVP,
                                     unsigned long long *sumx, unsigned long long *sumy, unsigned long long *sumz,
                                     const int *anc, int X, int Y, int Z, int perx, int pery, int perz) {
   const int S = L.S, T = S + 2, TW = L.TW;
   constexpr int NNB = (DIM == 2) ? 8 : 26;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   const unsigned long long first = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const unsigned long long n_iter = (n_active + stride - 1) / stride;   // same trip count for every lane of a warp
+  const unsigned long long n_iter = (w_end - w_begin + stride - 1) / stride;   // same trip count for every lane of a warp
   for (unsigned long long it = 0; it < n_iter; ++it) {
-    const unsigned long long w = first + it * stride;
+    const unsigned long long w = w_begin + first + it * stride;
     // frozen voxels (one obstacle id can own a fifth of the lattice, L139) are tallied apart and combined over the warp
     // before they reach the per-cell arrays: their atomics would all hit the same few addresses
     uint32_t fid = 0;
     int fcnt = 0, ffor = 0, fsx = 0, fsy = 0, fsz = 0;
-    if (w < n_active) {
+    if (w < w_end) {
       const uint32_t *tc = L.tiles + L.base[col] + (w >> PK_GS) * (unsigned long long)TW * (unsigned long long)PK_GC + (unsigned long long)pk_tbase((int)(w & (unsigned long long)(PK_GC - 1)), TW);
       const uint32_t w32 = (uint32_t)w;   // the host keeps n_active below 2^31 for this layout
       const int ax = (int)(w32 % (unsigned)L.nact[col][0]);

@@ -311,7 +311,12 @@ bool pipe_plan(const cpm_ctx *c, int a[PIPE_SLABS + 1]) {
   const int ax = c->d - 1;
   const int pairs = (c->nsub[ax] + 1) / 2;
   if (pairs < 2 * PIPE_SLABS) return false;
-  for (int i = 0; i <= PIPE_SLABS; ++i) a[i] = (int)((long long)i * pairs / PIPE_SLABS);
+  // the slabs shrink towards the end: what is left to do when the last byte has arrived is the last two slabs' work
+  static const double upto[PIPE_SLABS + 1] = {0.0, 0.2, 0.4, 0.6, 0.75, 0.87, 0.94, 0.98, 1.0};
+  for (int i = 0; i <= PIPE_SLABS; ++i) a[i] = (int)(upto[i] * pairs + 0.5);
+  for (int i = 1; i <= PIPE_SLABS; ++i) a[i] = std::max(a[i], a[i - 1] + 1);           // no empty slab (pairs >= 2 PIPE_SLABS)
+  a[PIPE_SLABS] = pairs;
+  for (int i = PIPE_SLABS - 1; i >= 0; --i) a[i] = std::min(a[i], a[i + 1] - 1);
   for (int col = 0; col < (1 << c->d); ++col) {
     if (c->n_act_col[col] == 0) continue;
     const unsigned long long slow = (unsigned long long)c->sp.tl.nact[col][ax];
@@ -806,14 +811,20 @@ int cpm_set_lattice(cpm_ctx *c, const uint32_t *ids, const uint8_t *frozen, cons
                                                           c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2], c->error_flag);
         c->launches++;
       }
+      RecountRanges rr{};
+      unsigned long long most = 0;
       for (int col = 0; col < (1 << c->d); ++col) {
         if (c->n_act_col[col] == 0 || we[col] <= wb[col]) continue;
-        const int grid = grid_for((long long)(we[col] - wb[col]), 128);
+        rr.w_begin[col] = wb[col]; rr.w_end[col] = we[col];
+        most = std::max(most, we[col] - wb[col]);
+      }
+      if (most > 0) {   // one launch for all colours (blockIdx.y)
+        const dim3 grid((unsigned)grid_for((long long)most, 128), (unsigned)(1 << c->d));
         if (c->d == 2)
-          tile_recount_kernel<2><<<grid, 128, 0, c->stream>>>(tl, col, wb[col], we[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+          tile_recount_kernel<2><<<grid, 128, 0, c->stream>>>(tl, rr, c->liveVP, c->sumx, c->sumy, c->sumz,
                                                              c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
         else
-          tile_recount_kernel<3><<<grid, 128, 0, c->stream>>>(tl, col, wb[col], we[col], c->liveVP, c->sumx, c->sumy, c->sumz,
+          tile_recount_kernel<3><<<grid, 128, 0, c->stream>>>(tl, rr, c->liveVP, c->sumx, c->sumy, c->sumz,
                                                              c->anc, c->dim[0], c->dim[1], c->dim[2], c->per[0], c->per[1], c->per[2]);
         c->launches++;
       }

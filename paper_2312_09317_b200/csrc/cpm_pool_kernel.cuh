@@ -672,13 +672,18 @@ __global__ void tile_unpack_kernel(TileLayout L, int X, int Y, int Z, uint32_t *
 // recount of V, A (Moore interfaces with sites not of the same cell, L234) and the coordinate sums (L288) from the
 // tiles: a thread takes one chain and walks its S^d interior sites; every neighbour is inside the chain's own
 // tile, the loads of the 8 lanes of a group are one 32-byte sector; runs of equal ids are flushed with one atomic
-// per array.  Chains [w_begin, w_end) of the colour.
+// per array.  blockIdx.y = the colour, of which the chains [w_begin, w_end) are taken: a thread's walk over its chain is a
+// long serial affair (~0.3 ms whatever the size of the launch), so all colours go into ONE launch.
+struct RecountRanges { unsigned long long w_begin[8], w_end[8]; };
 template <int DIM>
-__global__ void tile_recount_kernel(TileLayout L, int col, unsigned long long w_begin, unsigned long long w_end, unsigned long long *liveVP,
+__global__ void tile_recount_kernel(TileLayout L, RecountRanges R, unsigned long long *liveVP,
                                     unsigned long long *sumx, unsigned long long *sumy, unsigned long long *sumz,
                                     const int *anc, int X, int Y, int Z, int perx, int pery, int perz) {
   const int S = L.S, T = S + 2, TW = L.TW;
   constexpr int NNB = (DIM == 2) ? 8 : 26;
+  const int col = (int)blockIdx.y;
+  const unsigned long long w_begin = R.w_begin[col], w_end = R.w_end[col];
+  if (w_end <= w_begin) return;   // the whole block: nothing of this colour in the range
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   const unsigned long long first = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned long long n_iter = (w_end - w_begin + stride - 1) / stride;   // same trip count for every lane of a warp

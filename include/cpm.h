@@ -94,7 +94,11 @@ int  cpm_destroy(cpm_ctx *ctx);
  * non-zero = obstacle voxel that is never copied from or into, L139 stroma), cell_type
  * [max_cells+1] (type of each cell id; cell_type[0] must be 0).  Resets the Act field to 0 and
  * recounts volume, perimeter (Eq 3's A) and coordinate sums (L288) on the device.
- * Errors: CPM_ERR_ARG (NULL ids/cell_type, an id > max_cells or a type >= n_types). */
+ * Errors: CPM_ERR_ARG (NULL ids/cell_type, an id > max_cells or a type >= n_types).
+ * Host buffers (on_device = 0; pinned or pageable) are read before the call returns.  A lattice of >= 2^24 sites on the
+ * tiled layout crosses PCIe in 8 slabs on a stream of the context's own while the slabs that have arrived are packed and
+ * recounted (cpm_get_lattice likewise, the other way); the result does not depend on it.  The environment variable
+ * CPM_PIPE_MIN_SITES, read by cpm_create, moves that threshold (tests). */
 int  cpm_set_lattice(cpm_ctx *ctx, const uint32_t *ids, const uint8_t *frozen,
                      const uint8_t *cell_type, int on_device);
 /* Optional: set the per-site Act field (integers 0..255 stored as float, L255). */

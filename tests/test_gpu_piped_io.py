@@ -76,3 +76,34 @@ def test_small_geometries_fall_back_to_one_piece(pk, oracle_mod, monkeypatch):
         sg, so = g.get_cell_stats(), o.get_cell_stats()
         for k in so:
             np.testing.assert_array_equal(sg[k], so[k])
+
+
+@pytest.mark.parametrize("name,dims", [("C4", (256, 256, 256)), ("C5", (4096, 4096))])
+def test_pinned_buffers_at_the_natural_threshold(pk, oracle_mod, name, dims):
+    """2^24 sites: the slab path as a user meets it, with PINNED host buffers, whose copies really are asynchronous (a
+    pageable source holds the host up, which would hide an ordering mistake between the transfer stream and the kernels).
+    State after cpm_set_lattice, the read-back into a pinned buffer, and one MCS equal the oracle's; three times over,
+    with the buffers scribbled between the calls."""
+    import torch
+    import cpm_inputs as ci
+    cfg = ci.make_config(name, dims=dims)
+    p = dict(cfg["params"]); p["subsection"] = 0
+    g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], **p)
+    o = oracle_mod.Oracle(cfg["dims"], max_cells=cfg["max_cells"], **p)
+    o.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
+    so = o.get_cell_stats()
+    ids_h = torch.from_numpy(cfg["ids"].view(np.int32).reshape(-1)).pin_memory()
+    fz_h = torch.from_numpy(cfg["frozen"].reshape(-1)).pin_memory() if cfg["frozen"] is not None else None
+    ct_h = torch.from_numpy(cfg["cell_type"]).pin_memory()
+    out_h = torch.empty(ids_h.numel(), dtype=torch.int32).pin_memory()
+    for rep in range(3):
+        out_h.fill_(-1)
+        g.set_lattice(ids_h, fz_h, ct_h)
+        sg = g.get_cell_stats()
+        for k in so:
+            np.testing.assert_array_equal(sg[k], so[k], err_msg="%s, call %d" % (k, rep))
+        g.get_lattice(out_h)
+        assert torch.equal(out_h, ids_h)
+    g.set_mcs(0); g.step(1); o.step(1)
+    g.get_lattice(out_h)
+    np.testing.assert_array_equal(out_h.numpy().view(np.uint32).reshape(cfg["ids"].shape), o.get_lattice())

@@ -82,28 +82,35 @@ def test_small_geometries_fall_back_to_one_piece(pk, oracle_mod, monkeypatch):
 def test_pinned_buffers_at_the_natural_threshold(pk, oracle_mod, name, dims):
     """2^24 sites: the slab path as a user meets it, with PINNED host buffers, whose copies really are asynchronous (a
     pageable source holds the host up, which would hide an ordering mistake between the transfer stream and the kernels).
-    State after cpm_set_lattice, the read-back into a pinned buffer, and one MCS equal the oracle's; three times over,
-    with the buffers scribbled between the calls."""
+    State after cpm_set_lattice, the read-back into a pinned buffer, and one MCS equal the oracle's, over four calls
+    that alternate between two lattices."""
     import torch
     import cpm_inputs as ci
     cfg = ci.make_config(name, dims=dims)
     p = dict(cfg["params"]); p["subsection"] = 0
     g = pk.CPM(cfg["dims"], max_cells=cfg["max_cells"], **p)
     o = oracle_mod.Oracle(cfg["dims"], max_cells=cfg["max_cells"], **p)
-    o.set_lattice(cfg["ids"], cfg["frozen"], cfg["cell_type"])
-    so = o.get_cell_stats()
-    ids_h = torch.from_numpy(cfg["ids"].view(np.int32).reshape(-1)).pin_memory()
-    fz_h = torch.from_numpy(cfg["frozen"].reshape(-1)).pin_memory() if cfg["frozen"] is not None else None
+    # two different lattices taken in turns: the staging buffers still hold the other one from the call before, so a kernel
+    # that ran ahead of its slab's copy would pack stale words
+    ids_b = np.ascontiguousarray(np.roll(cfg["ids"], (7, 5), axis=(0, -1)))
+    fz_b = np.ascontiguousarray(np.roll(cfg["frozen"], (7, 5), axis=(0, -1))) if cfg["frozen"] is not None else None
+    inputs, want = [], []
+    for ids, fz in ((cfg["ids"], cfg["frozen"]), (ids_b, fz_b)):
+        o.set_lattice(ids, fz, cfg["cell_type"])
+        want.append(o.get_cell_stats())
+        inputs.append((torch.from_numpy(ids.view(np.int32).reshape(-1)).pin_memory(),
+                       torch.from_numpy(fz.reshape(-1)).pin_memory() if fz is not None else None))
     ct_h = torch.from_numpy(cfg["cell_type"]).pin_memory()
-    out_h = torch.empty(ids_h.numel(), dtype=torch.int32).pin_memory()
-    for rep in range(3):
+    out_h = torch.empty(inputs[0][0].numel(), dtype=torch.int32).pin_memory()
+    for rep in (0, 1, 0, 1):
+        ids_h, fz_h = inputs[rep]
         out_h.fill_(-1)
         g.set_lattice(ids_h, fz_h, ct_h)
         sg = g.get_cell_stats()
-        for k in so:
-            np.testing.assert_array_equal(sg[k], so[k], err_msg="%s, call %d" % (k, rep))
+        for k in want[rep]:
+            np.testing.assert_array_equal(sg[k], want[rep][k], err_msg="%s, lattice %d" % (k, rep))
         g.get_lattice(out_h)
         assert torch.equal(out_h, ids_h)
-    g.set_mcs(0); g.step(1); o.step(1)
+    g.set_mcs(0); g.step(1); o.step(1)     # both hold the second lattice
     g.get_lattice(out_h)
     np.testing.assert_array_equal(out_h.numpy().view(np.uint32).reshape(cfg["ids"].shape), o.get_lattice())

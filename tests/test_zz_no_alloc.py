@@ -68,7 +68,7 @@ def test_noalloc_statistics_device_outputs(pk):
 
 
 def test_noalloc_statistics_allocates_no_device_memory(pk):
-    """Free device memory is the same before and after the calls (the array was placed when the library loaded)."""
+    """Free device memory does not shrink over the calls (the array was placed when the library loaded)."""
     import torch
     g = _ctx(pk, "C1", (256, 256), subsection=8)
     f = np.zeros(8, np.uint64); w = np.zeros(64, np.uint64)
@@ -78,7 +78,7 @@ def test_noalloc_statistics_allocates_no_device_memory(pk):
     for _ in range(3):
         g.update_statistics_noalloc(2, f, w)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info(0)[0] == free0
+    assert torch.cuda.mem_get_info(0)[0] >= free0   # nothing was taken (a context of an earlier test freed in between may add)
 
 
 def test_noalloc_statistics_refuses_sizes_beyond_the_maximum(pk):

@@ -3,7 +3,8 @@ k < S^d, periodic axes, 2-5 cell types, negative J, obstacles, every extension i
 kernels, graph and plain launches) run for a few MCS on the CUDA path and on the oracle and compared element by element:
 lattice, V, P, coordinate sums, Act, persistence doubles, counters.  A case whose tiny cells overflow a subsection's
 own-delta table must be REPORTED (CPM_ERR_UNSUPPORTED), never computed approximately.  The same generator was run over
-29 000 cases while this file was written (no mismatch); the suite keeps 160 of them.  Needs a B200 (`-m gpu`)."""
+29 000 cases while this file was written and over 69 366 more (seeds 8 000 000 ...) on the round's final sources, half of them
+with the slab-wise host transfers forced on (no mismatch; 939 reported overflows); the suite keeps 160 of them.  Needs a B200 (`-m gpu`)."""
 import numpy as np
 import pytest
 

@@ -52,6 +52,9 @@ constexpr int PK_SUPER = 64;                 // attempts per chain whose proposa
 #ifndef PK_MINB
 #define PK_MINB 20
 #endif
+#ifndef PK_MINB_2D
+#define PK_MINB_2D 28   // 2D tiles are small: shared memory allows 28 CTAs per SM at S = 8, so the registers are held to 73 (measured: C5 16384^2 2.53 -> 2.26 ms per MCS, C7 0.147 -> 0.137; the 3D instantiations lose 3 % at 28)
+#endif
 constexpr int PK_TARGET = PK_TARGET_VALUE;   // a round's window grows until it holds this many items
 constexpr int PK_NJ = PK_NJ_VALUE;                     // a chain's window per round: 4 NJ attempts behind its position
 constexpr int PK_CAP = 32;                   // own-delta entries per chain and activation (reading R2)
@@ -153,7 +156,7 @@ __device__ __forceinline__ unsigned long long home_word(const TileLayout &L, int
 }
 
 template <int DIM, int S, bool ACT, bool LIVE, bool VEC>
-__global__ void __launch_bounds__(PK_THREADS, PK_MINB) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
+__global__ void __launch_bounds__(PK_THREADS, (DIM == 2) ? PK_MINB_2D : PK_MINB) sweep_pool_kernel(const __grid_constant__ SweepParams P) {
   using G = PGeom<DIM, S>;
   using M = PSmem<DIM, S>;
   constexpr int T = G::T, TW = G::TW, NNB = G::NNB, GC = PK_GC, NJ = PK_NJ, TS = PK_TS;
